@@ -1,0 +1,245 @@
+"""numpy/ctypes wrapper around ``sparda_oracle.c`` -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Argument marshalling only; every number is computed by the plain C loops in
+``sparda_oracle.c`` (which cites the paper passage each function follows).  ``decode_pipeline``
+(o10) is the one function written here: it is Algorithm 2 lines 4-7 run strictly
+in order, calling o3-o6 layer by layer.
+
+bf16 tensors are numpy ``uint16`` arrays holding the raw upper halves of fp32 values.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sparda_oracle.c")
+_LIB = os.path.join(_HERE, "libsparda_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain C11 + OpenMP over independent units)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-std=c11", "-O2", "-fopenmp", "-fPIC", "-shared", "-fno-fast-math",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.sparda_oracle_bf16_to_double.restype = ctypes.c_double
+        _lib.sparda_oracle_bf16_to_double.argtypes = [ctypes.c_uint16]
+        _lib.sparda_oracle_double_to_bf16.restype = ctypes.c_uint16
+        _lib.sparda_oracle_double_to_bf16.argtypes = [ctypes.c_double]
+        _lib.sparda_oracle_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _u16(a) -> np.ndarray:
+    a = np.ascontiguousarray(a)
+    assert a.dtype == np.uint16, a.dtype
+    return a
+
+
+def _i64(x):
+    return ctypes.c_int64(int(x))
+
+
+def _i32(x):
+    return ctypes.c_int(int(x))
+
+
+def threads() -> int:
+    return int(_load().sparda_oracle_threads())
+
+
+def set_threads(n: int) -> None:
+    _load().sparda_oracle_set_threads(_i32(n))
+
+
+# ---- bf16 helpers -------------------------------------------------------------------------
+def bf16_bits_to_f64(a: np.ndarray) -> np.ndarray:
+    """Exact widening of raw bf16 bits to float64 (numpy only, used by tests and callers)."""
+    a = np.ascontiguousarray(a, dtype=np.uint16)
+    return (a.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+def double_to_bf16(x: float) -> int:
+    return int(_load().sparda_oracle_double_to_bf16(ctypes.c_double(x)))
+
+
+def from_torch(t) -> np.ndarray:
+    """torch.bfloat16 CPU tensor -> uint16 bits (no copy of values, no arithmetic)."""
+    import torch
+    assert t.dtype == torch.bfloat16 and t.device.type == "cpu"
+    return t.contiguous().view(torch.int16).numpy().view(np.uint16)
+
+
+def to_torch(a: np.ndarray):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).view(torch.bfloat16)
+
+
+# ---- o1 .. o9 -----------------------------------------------------------------------------
+def pool_keys(kv: np.ndarray) -> np.ndarray:
+    """o1 (Eq.2, kernel = stride = S).  kv [R][Nb][2][S][D] -> Kpool [R][Nb][D]."""
+    kv = _u16(kv)
+    R, Nb, two, S, D = kv.shape
+    assert two == 2
+    out = np.empty((R, Nb, D), dtype=np.uint16)
+    _load().sparda_oracle_pool_keys(_p(kv), _i64(R), _i64(Nb), _i32(S), _i32(D), _p(out))
+    return out
+
+
+def forecast_project(X: np.ndarray, WF: np.ndarray, Hkv: int, D: int) -> np.ndarray:
+    """o2 (Eq.3).  X [B][hidden], WF [hidden][Hkv*D] -> F [B*Hkv][D]."""
+    X, WF = _u16(X), _u16(WF)
+    B, hidden = X.shape
+    assert WF.shape == (hidden, Hkv * D)
+    out = np.empty((B * Hkv, D), dtype=np.uint16)
+    _load().sparda_oracle_forecast_project(_p(X), _p(WF), _i64(B), _i64(hidden), _i32(Hkv), _i32(D), _p(out))
+    return out
+
+
+def score(F: np.ndarray, kpool: np.ndarray) -> np.ndarray:
+    """o3 (Eq.4).  F [R][D], Kpool [R][Nb][D] -> s [R][Nb] fp32."""
+    F, kpool = _u16(F), _u16(kpool)
+    R, Nb, D = kpool.shape
+    assert F.shape == (R, D)
+    out = np.empty((R, Nb), dtype=np.float32)
+    _load().sparda_oracle_score(_p(F), _p(kpool), _i64(R), _i64(Nb), _i32(D), _p(out))
+    return out
+
+
+def topk(scores: np.ndarray, k: int, n_cand: int | None = None) -> np.ndarray:
+    """o4 (P:L78 f_top).  s [R][Nb] fp32 -> ids [R][k] int32 ascending, -1 padded."""
+    scores = np.ascontiguousarray(scores, dtype=np.float32)
+    R, Nb = scores.shape
+    n_cand = Nb if n_cand is None else n_cand
+    assert 0 <= n_cand <= Nb
+    out = np.empty((R, k), dtype=np.int32)
+    _load().sparda_oracle_topk(_p(scores), _i64(R), _i64(Nb), _i64(n_cand), _i32(k), _p(out))
+    return out
+
+
+def forecast_select(F: np.ndarray, kpool: np.ndarray, k: int, n_cand: int | None = None):
+    """o3 + o4: returns (ids, scores)."""
+    s = score(F, kpool)
+    return topk(s, k, n_cand), s
+
+
+def gather(kv: np.ndarray, ids: np.ndarray, pool: np.ndarray | None = None) -> np.ndarray:
+    """o5.  kv [R][Nb][2][S][D], ids [R][k] -> pool [R][k][2][S][D]; -1 slots untouched."""
+    kv = _u16(kv)
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    R, Nb, two, S, D = kv.shape
+    k = ids.shape[1]
+    assert ids.shape[0] == R
+    if pool is None:
+        pool = np.zeros((R, k, 2, S, D), dtype=np.uint16)
+    assert pool.shape == (R, k, 2, S, D) and pool.dtype == np.uint16 and pool.flags.c_contiguous
+    _load().sparda_oracle_gather(_p(kv), _p(ids), _i64(R), _i64(Nb), _i32(k), _i32(S), _i32(D), _p(pool))
+    return pool
+
+
+def sparse_attn(Q: np.ndarray, pool: np.ndarray, ids: np.ndarray, pool_is_indexed: bool = False):
+    """o6 (Eq.5).  Q [B][Hq][D], pool [R][n_slots][2][S][D], ids [R][k] -> (O bf16 bits, O float64)."""
+    Q, pool = _u16(Q), _u16(pool)
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    B, Hq, D = Q.shape
+    R, n_slots, two, S, D2 = pool.shape
+    assert two == 2 and D2 == D and R % B == 0
+    Hkv = R // B
+    k = ids.shape[1]
+    assert ids.shape[0] == R
+    if not pool_is_indexed:
+        assert n_slots == k
+    else:
+        assert ids.max(initial=-1) < n_slots
+    O = np.empty((B, Hq, D), dtype=np.uint16)
+    O64 = np.empty((B, Hq, D), dtype=np.float64)
+    _load().sparda_oracle_sparse_attn(_p(Q), _p(pool), _p(ids), _i32(1 if pool_is_indexed else 0), _i64(B), _i32(Hq),
+                                      _i32(Hkv), _i32(D), _i32(S), _i32(k), _i64(n_slots), _p(O), _p(O64))
+    return O, O64
+
+
+def dense_attn(Q: np.ndarray, kv: np.ndarray):
+    """o7 (textbook).  Q [B][Hq][D], kv [R][Nb][2][S][D] -> (O bf16 bits, O float64)."""
+    Q, kv = _u16(Q), _u16(kv)
+    B, Hq, D = Q.shape
+    R, Nb, two, S, D2 = kv.shape
+    assert two == 2 and D2 == D and R % B == 0
+    O = np.empty((B, Hq, D), dtype=np.uint16)
+    O64 = np.empty((B, Hq, D), dtype=np.float64)
+    _load().sparda_oracle_dense_attn(_p(Q), _p(kv), _i64(B), _i32(Hq), _i32(R // B), _i32(D), _i32(S), _i64(Nb),
+                                     _p(O), _p(O64))
+    return O, O64
+
+
+def prefill_select(F: np.ndarray, kpool: np.ndarray, k: int, row0: int = 0, n_rows: int | None = None,
+                   S: int = 64, want_scores: bool = False):
+    """o8 (Alg.1 l.2, causal rule q8).  F [Hkv][T][D], Kpool [Hkv][Nb][D] -> ids [Hkv][n_rows][k]."""
+    F, kpool = _u16(F), _u16(kpool)
+    Hkv, T, D = F.shape
+    Nb = kpool.shape[1]
+    assert kpool.shape == (Hkv, Nb, D)
+    n_rows = T - row0 if n_rows is None else n_rows
+    assert 0 <= row0 and row0 + n_rows <= T
+    ids = np.empty((Hkv, n_rows, k), dtype=np.int32)
+    sc = np.empty((Hkv, n_rows, Nb), dtype=np.float32) if want_scores else None
+    _load().sparda_oracle_prefill_select(_p(F), _p(kpool), _i32(Hkv), _i64(T), _i64(Nb), _i32(D), _i32(S),
+                                         _i64(row0), _i64(n_rows), _i32(k), _p(ids),
+                                         _p(sc) if want_scores else None)
+    return (ids, sc) if want_scores else ids
+
+
+def prefill_select_baseline(Q: np.ndarray, kpool: np.ndarray, k: int, row0: int = 0, n_rows: int | None = None,
+                            S: int = 64, want_scores: bool = False):
+    """o9 (Eq.6 left).  Q [Hq][T][D], Kpool [Hkv][Nb][D] -> ids [Hkv][n_rows][k]."""
+    Q, kpool = _u16(Q), _u16(kpool)
+    Hq, T, D = Q.shape
+    Hkv, Nb, _ = kpool.shape
+    assert Hq % Hkv == 0
+    n_rows = T - row0 if n_rows is None else n_rows
+    ids = np.empty((Hkv, n_rows, k), dtype=np.int32)
+    sc = np.empty((Hkv, n_rows, Nb), dtype=np.float32) if want_scores else None
+    _load().sparda_oracle_prefill_select_baseline(_p(Q), _p(kpool), _i32(Hq), _i32(Hkv), _i64(T), _i64(Nb), _i32(D),
+                                                  _i32(S), _i64(row0), _i64(n_rows), _i32(k), _p(ids),
+                                                  _p(sc) if want_scores else None)
+    return (ids, sc) if want_scores else ids
+
+
+# ---- o10 ----------------------------------------------------------------------------------
+def decode_pipeline(layers, k: int):
+    """o10: Algorithm 2 lines 4-7 for L layers, strictly in order, no overlap.
+
+    ``layers`` is a list of dicts with uint16 arrays ``kv`` [R][Nb][2][S][D], ``kpool`` [R][Nb][D],
+    ``F`` [R][D], ``Q`` [B][Hq][D]; layer 0 additionally has ``F0cur`` [R][D].
+    Layer 0: same-layer selection with F0cur, attention straight from its own cache.
+    Layer l >= 1: ids_l = f_top(F_{l-1} Kpool_l^T, k) (reading q9); gather; attention.
+    F of the last layer is unused.  Returns per-layer dicts {ids, scores, pool, O, O64}.
+    """
+    out = []
+    for l, lay in enumerate(layers):
+        f = lay["F0cur"] if l == 0 else layers[l - 1]["F"]
+        ids, s = forecast_select(f, lay["kpool"], k)
+        if l == 0:
+            pool = None
+            O, O64 = sparse_attn(lay["Q"], lay["kv"], ids, pool_is_indexed=True)
+        else:
+            pool = gather(lay["kv"], ids)
+            O, O64 = sparse_attn(lay["Q"], pool, ids, pool_is_indexed=False)
+        out.append({"ids": ids, "scores": s, "pool": pool, "O": O, "O64": O64})
+    return out

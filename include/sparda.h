@@ -1,0 +1,169 @@
+/*
+ * sparda.h -- C ABI of libsparda: SparDA's decode-time hot path, hand-written CUDA for sm_100a (B200).
+ *
+ * Citations: P:L<n> = line n of the paper text (arxiv 2606.04511, "SparDA: Sparse Decoupled Attention
+ * for Efficient Long-Context LLM Inference"); section / equation / algorithm named beside it.
+ *
+ * The path (Algorithm 2, lines 4-7), per layer l of one decode step:
+ *   4  B_{l+1} <- f_top(F_l Kpool_{l+1}^T, k)      sparda_forecast_select      (Eq.4)
+ *   5  launch prefetch of B_{l+1}, CPU -> GPU       sparda_prefetch_launch      (Sec.4.3)
+ *   6  wait for the KV entries of B_l               events, sparda_decode_step
+ *   7  O_l <- Attn(Q_l, K_l[B_l], V_l[B_l])         sparda_sparse_decode        (Eq.5)
+ * plus the selection line of the prefill step (Algorithm 1 line 2): sparda_prefill_select and the
+ * multi-head softmax selector it replaces: sparda_prefill_select_baseline.
+ *
+ * Conventions
+ *  - Plain C linkage, plain pointers and sizes.  "device" = pointer valid in device code on the current
+ *    CUDA device; "host-mapped" = device-visible pointer to pinned (page-locked, mapped) host memory
+ *    (cudaHostAlloc / cudaHostRegister; with UVA the host pointer itself).  All tensor pointers must be
+ *    16-byte aligned (ids: 4-byte).
+ *  - bf16 = raw upper 16 bits of an IEEE fp32, row-major, innermost dimension contiguous.
+ *  - Shapes use B batch, Hq query heads, Hkv KV heads (= GQA groups), G = Hq/Hkv, R = B*Hkv rows,
+ *    D head dim (= Forecast width), S block size (64), Nb blocks per row, k = topk.
+ *    KV cache / host_kv : [R][Nb][2][S][D] bf16, plane 0 = K, plane 1 = V: one block's K+V is one
+ *                         contiguous 2*S*D*2-byte run (32 KiB at D=128).
+ *    dev_pool           : [R][k][2][S][D] bf16, slot i of row r holds block ids[r][i].
+ *    Kpool              : [R][Nb][D] bf16, one mean-pooled key per block (Eq.2, kernel=stride=S).
+ *    F                  : [R][D] bf16, one Forecast head per GQA group.
+ *    Q, O               : [B][Hq][D] bf16; head h belongs to group h / G.
+ *    ids                : [R][k] int32, ascending block ids, -1 padded.
+ *  - Ownership: the caller owns every tensor and every stream; the library owns only the workspace
+ *    allocated by sparda_create (split-K partials, score scratch, tickets, events).  No call
+ *    allocates after sparda_create, synchronises the host, or copies results to the host.
+ *  - `stream` arguments are cudaStream_t values passed as void* (torch: stream.cuda_stream).  Calls on
+ *    one context must be issued from one host thread at a time.  Work is enqueued asynchronously; a
+ *    return of SPARDA_OK means "enqueued", errors of the kernels themselves surface at the next CUDA
+ *    synchronisation.
+ *  - Errors: negative return codes below; sparda_strerror() names them, sparda_last_cuda_error() returns
+ *    the CUDA error text of the last SPARDA_ECUDA on the calling context.  There is no CPU fallback
+ *    and no other backend: on a device that is not sm_100 sparda_create returns SPARDA_EUNSUPPORTED.
+ */
+#ifndef SPARDA_H_
+#define SPARDA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPARDA_OK 0
+#define SPARDA_EINVAL (-1)       /* null / misaligned pointer, shape outside the supported set */
+#define SPARDA_EUNSUPPORTED (-2) /* device is not sm_100 (B200) */
+#define SPARDA_ECUDA (-3)        /* a CUDA runtime / driver call failed; see sparda_last_cuda_error */
+#define SPARDA_ENOMEM (-4)       /* workspace allocation failed in sparda_create */
+
+#define SPARDA_GATHER_TMA 0 /* persistent single-thread-per-CTA bulk-copy (TMA) ring: host -> smem -> HBM */
+#define SPARDA_GATHER_LDG 1 /* persistent warps issuing 16-byte vector loads from mapped host memory */
+
+typedef struct sparda_ctx sparda_ctx; /* opaque */
+
+typedef struct {
+    int batch;       /* B  >= 1 */
+    int n_q_heads;   /* Hq, multiple of n_kv_heads; G = Hq/Hkv in {1,2,4,8,16} */
+    int n_kv_heads;  /* Hkv */
+    int head_dim;    /* D in {64, 128} */
+    int block_size;  /* S, must be 64 */
+    int max_blocks;  /* largest Nb any call will pass (<= 8192) */
+    int topk;        /* largest k any call will pass (<= 256) */
+    int gather_ctas; /* persistent gather grid size; 0 = default (4 for TMA, 16 for LDG; Table 7) */
+    int gather_mode; /* SPARDA_GATHER_TMA or SPARDA_GATHER_LDG */
+    int attn_splits; /* split-K CTAs per row for sparse_decode; 0 = auto from B, Hkv, k and the SM count */
+    int max_layers;  /* largest n_layers sparda_decode_step will see (events are pre-created); 0 = 64 */
+} sparda_config;
+
+/* One decoder layer's tensors for sparda_decode_step (Algorithm 2). */
+typedef struct {
+    const void* F;     /* [R][D] device.  Forecast produced in this layer; selects B_{l+1}.  Unused for
+                          the last layer.                                                            */
+    const void* Q;     /* [B][Hq][D] device.                                                                   */
+    const void* Kpool; /* [R][Nb][D] device: this layer's pooled keys (kept on GPU).            */
+    const void* kv;    /* this layer's KV cache [R][Nb][2][S][D]: layer 0 = device pointer (layer-0 cache stays
+                          on GPU); layers >= 1 = host-mapped pointer (pinned CPU memory) */
+    void* O;           /* [B][Hq][D] device, written.                                                          */
+    int32_t* ids;      /* [R][k] device, written: B_l.                                                         */
+} sparda_layer;
+
+#define SPARDA_STEP_OVERLAP 0    /* gather on prefetch_stream, overlapped with the compute stream (the method) */
+#define SPARDA_STEP_SERIAL 1     /* same kernels, everything on compute_stream in Algorithm-2 order (no overlap) */
+
+/* Create a context for one shape family on the current device.  Allocates the workspace (split-K partials
+ * R*max_splits*16*(D+2) floats, score scratch R*max_blocks floats, tickets, 2*max_layers events).
+ * Returns SPARDA_OK, SPARDA_EINVAL, SPARDA_EUNSUPPORTED, SPARDA_ENOMEM or SPARDA_ECUDA; *out is set only on
+ * success.  Destroy with sparda_destroy (synchronises the device first).                                     */
+int sparda_create(const sparda_config* cfg, sparda_ctx** out);
+int sparda_destroy(sparda_ctx* ctx);
+
+/* (a0) Key compression, Eq.2 with kernel = stride = S: Kpool[r,j,:] = bf16(mean_t K[r,j,t,:]),
+ * fp32 sum in ascending t, one rounding.  kv: device pointer to [R][n_blocks][2][S][D] (a staged chunk of the
+ * cache); kpool: device [R][n_blocks][D].  n_rows may be any positive count (not tied to the context's R).
+ * Pre-condition of the path ("kept on GPU and updated incrementally"), not on the timed path.  */
+int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_blocks, void* kpool, void* stream);
+
+/* (a1+a2) Forecast indexer, Eq.4: s[r,j] = sum_d F[r,d]*Kpool[r,j,d] (raw logits, fp32
+ * accumulate, no softmax, no scale) for candidate blocks j in [0, n_cand); ids_out[r] = the min(topk, n_cand)
+ * best blocks, ties to the lowest block id, emitted in ascending block id and padded with -1.
+ * F [R][D], Kpool [R][n_blocks][D], ids_out [R][topk]: device.  0 <= n_cand <= n_blocks <= max_blocks,
+ * 1 <= topk <= cfg.topk.  One kernel launch on `stream`.                                                      */
+int sparda_forecast_select(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
+                           int32_t* ids_out, void* stream);
+
+/* (a3) Prefetch launch, Alg.2 l.5, Sec.4.3: one persistent kernel on `stream` (the prefetch
+ * stream) copies, for every (r, i) with ids[r][i] >= 0, the 2*S*D*2 bytes of block ids[r][i] of host_kv
+ * [R][n_blocks][2][S][D] (host-mapped; a device pointer also works) to slot i of dev_pool [R][topk][2][S][D].
+ * ids is a DEVICE pointer read when the kernel runs, so the launch can be enqueued before the selection has
+ * executed; the caller orders it after the select and before the attention with events.  Slots whose id is -1
+ * are left untouched.  Exact byte copy.                                                                       */
+int sparda_prefetch_launch(sparda_ctx* ctx, const void* host_kv, int n_blocks, const int32_t* ids, int topk,
+                           void* dev_pool, void* stream);
+
+/* (a5/a6) Block-sparse GQA attention with the real query, Eq.5, Alg.2 l.7:
+ * O[b,h,:] = bf16( softmax_t( q_h . k_t / sqrt(D) ) V ) over every token t of every selected block of row
+ * r = b*Hkv + h/G; bf16 tensor-core products, fp32 softmax and accumulation, one rounding; no causal mask
+ * inside a block (the query sits after the context).  Slots with id -1 are skipped; a row with no valid slot
+ * gives O = 0.
+ *   pool_is_indexed = 0: dev_pool is [R][topk][2][S][D] and slot i holds block ids[r][i] (n_slots = topk);
+ *   pool_is_indexed = 1: dev_pool is a device-resident cache [R][n_slots][2][S][D] addressed through ids
+ *                        (layer 0).
+ * Split-K flash-decode: grid = attn_splits x R CTAs, partials merged by the last CTA of each row.            */
+int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, int topk,
+                         int pool_is_indexed, int n_slots, void* O, void* stream);
+
+/* (a4 + a6) One decode step over n_layers layers in Algorithm-2 order with the one-layer-ahead
+ * pipeline: layer 0 selects with F0cur against its own Kpool and attends straight from its device-resident
+ * cache; for l >= 1, ids_l = f_top(F_{l-1} Kpool_l^T) is selected during layer l-1, gathered
+ * into dev_pool[l & 1] on prefetch_stream and attended in layer l after an event wait.  The pool is
+ * double-buffered: gather l+1 may start only after attention l-1 released its buffer.
+ * mode = SPARDA_STEP_OVERLAP or SPARDA_STEP_SERIAL (same kernels on one stream; results are bit-identical).
+ * Capturable into a CUDA graph (no host synchronisation, events are pre-created).                             */
+int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
+                       int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
+                       int mode);
+
+/* (a7) Chunked-prefill selection with the Forecast indexer, Alg.1 l.2: for query positions
+ * i = row0 .. row0+n_rows-1 of every group g, scores = F[g,i,:] . Kpool[g,j,:] for the causal candidates
+ * j < (i+1)/S (a block is visible once its last token <= i), top-k as in forecast_select.
+ * F [Hkv][T][D], Kpool [Hkv][n_blocks][D], ids_out [Hkv][n_rows][topk]: device.  Dense bf16 contraction on
+ * tcgen05 tensor cores (fp32 accumulators in TMEM) with a fused per-row top-k epilogue.                       */
+int sparda_prefill_select(sparda_ctx* ctx, const void* F, const void* Kpool, int T, int n_blocks, int row0,
+                          int n_rows, int topk, int32_t* ids_out, void* stream);
+
+/* (a7') The comparison selector (Eq.6 left term): per query head h of group g,
+ * softmax_j(Q[h,i,:] . Kpool[g,j,:] / sqrt(D)) over the same causal candidates, summed over the G heads,
+ * then the same top-k.  Q [Hq][T][D] device.                                                                  */
+int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* Kpool, int T, int n_blocks, int row0,
+                                   int n_rows, int topk, int32_t* ids_out, void* stream);
+
+/* Introspection used by bench.py / tests: number of kernels this context has launched since creation, the
+ * resolved tunables, and error text.                                                                          */
+int64_t sparda_launch_count(const sparda_ctx* ctx);
+int sparda_get_attn_splits(const sparda_ctx* ctx, int topk);
+int sparda_get_gather_ctas(const sparda_ctx* ctx);
+const char* sparda_strerror(int code);
+const char* sparda_last_cuda_error(const sparda_ctx* ctx);
+const char* sparda_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPARDA_H_ */

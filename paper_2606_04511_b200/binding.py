@@ -1,0 +1,183 @@
+"""Thin ctypes binding of libsparda (include/sparda.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI.  torch is used for device / pinned
+memory and streams.  There is no fallback: if ``libsparda.so`` is missing or a call fails, a
+``SpardaError`` is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsparda.so")
+
+GATHER_TMA, GATHER_LDG = 0, 1
+STEP_OVERLAP, STEP_SERIAL = 0, 1
+
+EXPORTS = [
+    "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_select", "sparda_prefetch_launch",
+    "sparda_sparse_decode", "sparda_decode_step", "sparda_prefill_select", "sparda_prefill_select_baseline",
+    "sparda_launch_count", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
+    "sparda_last_cuda_error", "sparda_version",
+]
+
+
+class SpardaError(RuntimeError):
+    pass
+
+
+class SpardaConfig(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int) for n in (
+        "batch", "n_q_heads", "n_kv_heads", "head_dim", "block_size", "max_blocks", "topk", "gather_ctas",
+        "gather_mode", "attn_splits", "max_layers")]
+
+
+class SpardaLayer(ctypes.Structure):
+    _fields_ = [("F", ctypes.c_void_p), ("Q", ctypes.c_void_p), ("Kpool", ctypes.c_void_p), ("kv", ctypes.c_void_p),
+                ("O", ctypes.c_void_p), ("ids", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libsparda.so (built in-tree by ``build.build()``); fail loudly if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise SpardaError(f"{LIB_PATH} not found: build it with `python -m paper_2606_04511_b200.build` "
+                              "(there is no CPU or PyTorch fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64
+        L.sparda_create.argtypes = [ctypes.POINTER(SpardaConfig), ctypes.POINTER(vp)]
+        L.sparda_destroy.argtypes = [vp]
+        L.sparda_pool_keys.argtypes = [vp, vp, i64, i32, vp, vp]
+        L.sparda_forecast_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+        L.sparda_prefetch_launch.argtypes = [vp, vp, i32, vp, i32, vp, vp]
+        L.sparda_sparse_decode.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
+        L.sparda_decode_step.argtypes = [vp, ctypes.POINTER(SpardaLayer), i32, vp, i32, i32, vp, vp, vp, vp, i32]
+        L.sparda_prefill_select.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
+        L.sparda_prefill_select_baseline.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
+        L.sparda_launch_count.argtypes = [vp]
+        L.sparda_launch_count.restype = i64
+        L.sparda_get_attn_splits.argtypes = [vp, i32]
+        L.sparda_get_gather_ctas.argtypes = [vp]
+        for f in ("sparda_strerror", "sparda_last_cuda_error", "sparda_version"):
+            getattr(L, f).restype = ctypes.c_char_p
+        L.sparda_strerror.argtypes = [i32]
+        L.sparda_last_cuda_error.argtypes = [vp]
+        _lib = L
+    return _lib
+
+
+def _ptr(t) -> int:
+    if t is None:
+        return 0
+    if isinstance(t, int):
+        return t
+    assert t.is_contiguous(), "tensors crossing the C ABI must be contiguous"
+    return t.data_ptr()
+
+
+def _stream(s) -> int:
+    if s is None:
+        return torch.cuda.current_stream().cuda_stream
+    return s.cuda_stream if hasattr(s, "cuda_stream") else int(s)
+
+
+class Sparda:
+    """One libsparda context (one shape family on the current device)."""
+
+    def __init__(self, batch, n_q_heads, n_kv_heads, head_dim, max_blocks, topk, block_size=64, gather_ctas=0,
+                 gather_mode=GATHER_TMA, attn_splits=0, max_layers=0):
+        self._h = ctypes.c_void_p()
+        self.cfg = SpardaConfig(batch, n_q_heads, n_kv_heads, head_dim, block_size, max_blocks, topk, gather_ctas,
+                                gather_mode, attn_splits, max_layers)
+        self._L = lib()
+        rc = self._L.sparda_create(ctypes.byref(self.cfg), ctypes.byref(self._h))
+        if rc != 0:
+            self._h = ctypes.c_void_p()
+            raise SpardaError(f"sparda_create: {self._L.sparda_strerror(rc).decode()}")
+        self.rows = batch * n_kv_heads
+
+    @classmethod
+    def from_config(cls, cfg, **kw):
+        return cls(cfg.batch, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.n_blocks, cfg.topk,
+                   block_size=cfg.block_size, **kw)
+
+    def close(self):
+        if self._h:
+            self._L.sparda_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc != 0:
+            msg = self._L.sparda_strerror(rc).decode()
+            if rc == -3:
+                msg += ": " + self._L.sparda_last_cuda_error(self._h).decode()
+            raise SpardaError(f"{what}: {msg}")
+
+    # ---- entry points (same names as include/sparda.h without the prefix) ----
+    def pool_keys(self, kv, n_rows, n_blocks, kpool, stream=None):
+        self._check(self._L.sparda_pool_keys(self._h, _ptr(kv), n_rows, n_blocks, _ptr(kpool), _stream(stream)), "pool_keys")
+
+    def forecast_select(self, F, Kpool, n_blocks, topk, ids_out, n_cand=None, stream=None):
+        n_cand = n_blocks if n_cand is None else n_cand
+        self._check(self._L.sparda_forecast_select(self._h, _ptr(F), _ptr(Kpool), n_blocks, n_cand, topk, _ptr(ids_out),
+                                                   _stream(stream)), "forecast_select")
+
+    def prefetch_launch(self, host_kv, n_blocks, ids, topk, dev_pool, stream=None):
+        self._check(self._L.sparda_prefetch_launch(self._h, _ptr(host_kv), n_blocks, _ptr(ids), topk, _ptr(dev_pool),
+                                                   _stream(stream)), "prefetch_launch")
+
+    def sparse_decode(self, Q, dev_pool, ids, topk, O, pool_is_indexed=False, n_slots=None, stream=None):
+        n_slots = topk if n_slots is None else n_slots
+        self._check(self._L.sparda_sparse_decode(self._h, _ptr(Q), _ptr(dev_pool), _ptr(ids), topk,
+                                                 1 if pool_is_indexed else 0, n_slots, _ptr(O), _stream(stream)),
+                    "sparse_decode")
+
+    def make_layers(self, layers):
+        """layers: list of dicts with tensors F, Q, Kpool, kv, O, ids -> ctypes array (keeps no references)."""
+        arr = (SpardaLayer * len(layers))()
+        for i, l in enumerate(layers):
+            arr[i] = SpardaLayer(_ptr(l["F"]), _ptr(l["Q"]), _ptr(l["Kpool"]), _ptr(l["kv"]), _ptr(l["O"]), _ptr(l["ids"]))
+        return arr
+
+    def decode_step(self, layer_array, F0cur, n_blocks, topk, pool0, pool1, compute_stream=None, prefetch_stream=None,
+                    mode=STEP_OVERLAP):
+        self._check(self._L.sparda_decode_step(self._h, layer_array, len(layer_array), _ptr(F0cur), n_blocks, topk,
+                                               _ptr(pool0), _ptr(pool1), _stream(compute_stream),
+                                               _stream(prefetch_stream), mode), "decode_step")
+
+    def prefill_select(self, F, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, stream=None):
+        self._check(self._L.sparda_prefill_select(self._h, _ptr(F), _ptr(Kpool), T, n_blocks, row0, n_rows, topk,
+                                                  _ptr(ids_out), _stream(stream)), "prefill_select")
+
+    def prefill_select_baseline(self, Q, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, stream=None):
+        self._check(self._L.sparda_prefill_select_baseline(self._h, _ptr(Q), _ptr(Kpool), T, n_blocks, row0, n_rows, topk,
+                                                           _ptr(ids_out), _stream(stream)), "prefill_select_baseline")
+
+    # ---- introspection ----
+    @property
+    def launch_count(self) -> int:
+        return int(self._L.sparda_launch_count(self._h))
+
+    def attn_splits(self, topk) -> int:
+        return int(self._L.sparda_get_attn_splits(self._h, topk))
+
+    @property
+    def gather_ctas(self) -> int:
+        return int(self._L.sparda_get_gather_ctas(self._h))
+
+
+def version() -> str:
+    return lib().sparda_version().decode()

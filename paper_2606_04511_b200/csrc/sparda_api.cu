@@ -1,0 +1,257 @@
+// libsparda: context, argument validation and the Algorithm-2 stream choreography (include/sparda.h).
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "sparda_internal.cuh"
+
+int sparda_set_cuda_error(sparda_ctx* ctx, cudaError_t e, const char* where) {
+    if (ctx) snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "%s: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e), where);
+    (void)cudaGetLastError();
+    return SPARDA_ECUDA;
+}
+
+int sparda_resolve_splits(const sparda_ctx* ctx, int topk) {
+    int s = ctx->cfg.attn_splits;
+    if (s <= 0) {
+        // enough CTAs for ~2 per SM, at least one block per consumer warp where possible
+        int want = (2 * ctx->sm_count + ctx->R - 1) / ctx->R;
+        int cap = (topk + SPARDA_ATTN_WARPS - 1) / SPARDA_ATTN_WARPS;
+        s = want < cap ? want : cap;
+        if (s < 1) s = 1;
+    }
+    if (s > topk) s = topk;
+    if (s > ctx->max_splits) s = ctx->max_splits;
+    return s;
+}
+
+extern "C" {
+
+const char* sparda_version(void) { return "libsparda 0.1 (sm_100a)"; }
+
+const char* sparda_strerror(int code) {
+    switch (code) {
+        case SPARDA_OK: return "ok";
+        case SPARDA_EINVAL: return "invalid argument (null or misaligned pointer, or shape outside the supported set)";
+        case SPARDA_EUNSUPPORTED: return "unsupported device (libsparda needs an sm_100 GPU)";
+        case SPARDA_ECUDA: return "CUDA call failed (see sparda_last_cuda_error)";
+        case SPARDA_ENOMEM: return "workspace allocation failed";
+        default: return "unknown error code";
+    }
+}
+
+const char* sparda_last_cuda_error(const sparda_ctx* ctx) { return ctx ? ctx->cuda_err : ""; }
+int64_t sparda_launch_count(const sparda_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int sparda_get_attn_splits(const sparda_ctx* ctx, int topk) { return ctx ? sparda_resolve_splits(ctx, topk) : SPARDA_EINVAL; }
+int sparda_get_gather_ctas(const sparda_ctx* ctx) { return ctx ? ctx->cfg.gather_ctas : SPARDA_EINVAL; }
+
+int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
+    if (!cfg || !out) return SPARDA_EINVAL;
+    const int G = cfg->n_kv_heads > 0 ? cfg->n_q_heads / cfg->n_kv_heads : 0;
+    if (cfg->batch < 1 || cfg->n_kv_heads < 1 || cfg->n_q_heads < 1 || cfg->n_q_heads % cfg->n_kv_heads != 0) return SPARDA_EINVAL;
+    if (!(G == 1 || G == 2 || G == 4 || G == 8 || G == 16)) return SPARDA_EINVAL;
+    if (cfg->head_dim != 64 && cfg->head_dim != 128) return SPARDA_EINVAL;
+    if (cfg->block_size != 64) return SPARDA_EINVAL;
+    if (cfg->max_blocks < 1 || cfg->max_blocks > 8192) return SPARDA_EINVAL;
+    if (cfg->topk < 1 || cfg->topk > 256) return SPARDA_EINVAL;
+    if (cfg->gather_mode != SPARDA_GATHER_TMA && cfg->gather_mode != SPARDA_GATHER_LDG) return SPARDA_EINVAL;
+    if (cfg->gather_ctas < 0 || cfg->gather_ctas > 1024 || cfg->attn_splits < 0 || cfg->max_layers < 0) return SPARDA_EINVAL;
+
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return SPARDA_EUNSUPPORTED;
+    }
+    if (prop.major != 10) return SPARDA_EUNSUPPORTED;
+
+    sparda_ctx* ctx = new (std::nothrow) sparda_ctx();
+    if (!ctx) return SPARDA_ENOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->cfg = *cfg;
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->R = cfg->batch * cfg->n_kv_heads;
+    ctx->G = G;
+    if (ctx->cfg.gather_ctas == 0) ctx->cfg.gather_ctas = cfg->gather_mode == SPARDA_GATHER_TMA ? 4 : 16;
+    ctx->max_layers = cfg->max_layers > 0 ? cfg->max_layers : 64;
+    ctx->max_splits = cfg->topk < 64 ? cfg->topk : 64;
+
+    cudaError_t e;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+        (void)cudaGetLastError();
+        delete ctx;
+        return SPARDA_EUNSUPPORTED;
+    }
+    ctx->encode_fn = fn;
+
+    const size_t D = cfg->head_dim;
+    size_t n_po = (size_t)ctx->R * ctx->max_splits * SPARDA_MAX_G * D;
+    size_t n_ml = (size_t)ctx->R * ctx->max_splits * 2 * SPARDA_MAX_G;
+    size_t n_sc = (size_t)ctx->R * cfg->max_blocks;
+    bool ok = cudaMalloc(&ctx->part_O, n_po * sizeof(float)) == cudaSuccess &&
+              cudaMalloc(&ctx->part_ml, n_ml * sizeof(float)) == cudaSuccess &&
+              cudaMalloc(&ctx->scores, n_sc * sizeof(float)) == cudaSuccess &&
+              cudaMalloc(&ctx->tickets, 2 * (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
+              cudaMemset(ctx->tickets, 0, 2 * (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
+    ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
+    ctx->ev_gather = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
+    ok = ok && ctx->ev_sel && ctx->ev_gather;
+    for (int i = 0; ok && i <= ctx->max_layers; ++i)
+        ok = cudaEventCreateWithFlags(&ctx->ev_sel[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&ctx->ev_gather[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {
+        (void)cudaGetLastError();
+        sparda_destroy(ctx);
+        return SPARDA_ENOMEM;
+    }
+    if (cudaDeviceSynchronize() != cudaSuccess) {
+        (void)cudaGetLastError();
+        sparda_destroy(ctx);
+        return SPARDA_ECUDA;
+    }
+    *out = ctx;
+    return SPARDA_OK;
+}
+
+int sparda_destroy(sparda_ctx* ctx) {
+    if (!ctx) return SPARDA_EINVAL;
+    (void)cudaDeviceSynchronize();
+    cudaFree(ctx->part_O);
+    cudaFree(ctx->part_ml);
+    cudaFree(ctx->scores);
+    cudaFree(ctx->tickets);
+    for (int i = 0; i <= ctx->max_layers; ++i) {
+        if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);
+        if (ctx->ev_gather && ctx->ev_gather[i]) cudaEventDestroy(ctx->ev_gather[i]);
+    }
+    free(ctx->ev_sel);
+    free(ctx->ev_gather);
+    (void)cudaGetLastError();
+    delete ctx;
+    return SPARDA_OK;
+}
+
+int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_blocks, void* kpool, void* stream) {
+    if (!ctx || !sparda_aligned(kv, 16) || !sparda_aligned(kpool, 16) || n_rows < 1 || n_blocks < 1) return SPARDA_EINVAL;
+    if (n_rows * (int64_t)n_blocks > (int64_t)1 << 31) return SPARDA_EINVAL;
+    return sparda_launch_pool_keys(ctx, kv, n_rows, n_blocks, kpool, (cudaStream_t)stream);
+}
+
+int sparda_forecast_select(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
+                           int32_t* ids_out, void* stream) {
+    if (!ctx || !sparda_aligned(F, 16) || !sparda_aligned(Kpool, 16) || !sparda_aligned(ids_out, 4)) return SPARDA_EINVAL;
+    if (n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || n_cand < 0 || n_cand > n_blocks) return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    return sparda_launch_select(ctx, F, Kpool, n_blocks, n_cand, topk, ids_out, (cudaStream_t)stream);
+}
+
+int sparda_prefetch_launch(sparda_ctx* ctx, const void* host_kv, int n_blocks, const int32_t* ids, int topk,
+                           void* dev_pool, void* stream) {
+    if (!ctx || !sparda_aligned(host_kv, 16) || !sparda_aligned(dev_pool, 16) || !sparda_aligned(ids, 4)) return SPARDA_EINVAL;
+    if (n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    return sparda_launch_gather(ctx, host_kv, n_blocks, ids, topk, dev_pool, (cudaStream_t)stream);
+}
+
+int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, int topk,
+                         int pool_is_indexed, int n_slots, void* O, void* stream) {
+    if (!ctx || !sparda_aligned(Q, 16) || !sparda_aligned(dev_pool, 16) || !sparda_aligned(ids, 4) || !sparda_aligned(O, 16))
+        return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    if (pool_is_indexed ? (n_slots < 1 || n_slots > ctx->cfg.max_blocks) : (n_slots != topk)) return SPARDA_EINVAL;
+    return sparda_launch_attn(ctx, Q, dev_pool, ids, topk, pool_is_indexed ? 1 : 0, n_slots, O, (cudaStream_t)stream);
+}
+
+int sparda_prefill_select(sparda_ctx* ctx, const void* F, const void* Kpool, int T, int n_blocks, int row0, int n_rows,
+                          int topk, int32_t* ids_out, void* stream) {
+    if (!ctx || !sparda_aligned(F, 1024) || !sparda_aligned(Kpool, 1024) || !sparda_aligned(ids_out, 16)) return SPARDA_EINVAL;
+    if (T < 1 || n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || row0 < 0 || n_rows < 1 || row0 + (int64_t)n_rows > T) return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    return sparda_launch_prefill_select(ctx, F, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, (cudaStream_t)stream);
+}
+
+int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* Kpool, int T, int n_blocks, int row0,
+                                   int n_rows, int topk, int32_t* ids_out, void* stream) {
+    if (!ctx || !sparda_aligned(Q, 1024) || !sparda_aligned(Kpool, 1024) || !sparda_aligned(ids_out, 16)) return SPARDA_EINVAL;
+    if (T < 1 || n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || row0 < 0 || n_rows < 1 || row0 + (int64_t)n_rows > T) return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    return sparda_launch_prefill_baseline(ctx, Q, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, (cudaStream_t)stream);
+}
+
+// Algorithm 2, lines 4-7, for n_layers layers.  Compute-stream order per layer l:
+//   select B_{l+1} (F_l vs Kpool_{l+1})  ->  record ev_sel[l+1]  ->  [prefetch stream: wait, gather, record ev_gather[l+1]]
+//   ->  wait ev_gather[l]  ->  attention l.
+// Buffer hand-off (double-buffered pool): gather l+1 writes pool[(l+1)&1], last read by attention l-1, which
+// precedes select B_{l+1} on the compute stream, so ev_sel[l+1] also releases the buffer.
+int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
+                       int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
+                       int mode) {
+    if (!ctx || !layers || n_layers < 1 || n_layers > ctx->max_layers || !F0cur) return SPARDA_EINVAL;
+    if (mode != SPARDA_STEP_OVERLAP && mode != SPARDA_STEP_SERIAL) return SPARDA_EINVAL;
+    if (n_layers > 1 && (!dev_pool0 || !dev_pool1)) return SPARDA_EINVAL;
+    cudaStream_t cs = (cudaStream_t)compute_stream;
+    cudaStream_t ps = mode == SPARDA_STEP_OVERLAP ? (cudaStream_t)prefetch_stream : cs;
+    void* pools[2] = {dev_pool0, dev_pool1};
+    int rc;
+    // layer 0: same-layer selection with F0cur
+    rc = sparda_forecast_select(ctx, F0cur, layers[0].Kpool, n_blocks, n_blocks, topk, layers[0].ids, cs);
+    if (rc) return rc;
+    for (int l = 0; l < n_layers; ++l) {
+        if (l + 1 < n_layers) {
+            rc = sparda_forecast_select(ctx, layers[l].F, layers[l + 1].Kpool, n_blocks, n_blocks, topk, layers[l + 1].ids, cs);
+            if (rc) return rc;
+            if (ps != cs) {
+                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], cs));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ps, ctx->ev_sel[l + 1], 0));
+            }
+            rc = sparda_prefetch_launch(ctx, layers[l + 1].kv, n_blocks, layers[l + 1].ids, topk, pools[(l + 1) & 1], ps);
+            if (rc) return rc;
+            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], ps));
+        }
+        if (l == 0) {
+            rc = sparda_sparse_decode(ctx, layers[0].Q, layers[0].kv, layers[0].ids, topk, 1, n_blocks, layers[0].O, cs);
+        } else {
+            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
+            rc = sparda_sparse_decode(ctx, layers[l].Q, pools[l & 1], layers[l].ids, topk, 0, topk, layers[l].O, cs);
+        }
+        if (rc) return rc;
+    }
+    return SPARDA_OK;
+}
+
+}  // extern "C"
+
+// TMA descriptor for a [rows][head_dim] bf16 view of a KV pool / cache: box = 64 rows x 64 elements (128 B),
+// 128-byte swizzle.  Cached per (base, rows, head_dim): encoding costs a few microseconds on the host.
+int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_dim, const CUtensorMap** out) {
+    for (int i = 0; i < ctx->n_tmaps; ++i)
+        if (ctx->tmaps[i].base == base && ctx->tmaps[i].rows == rows && ctx->tmaps[i].head_dim == head_dim) {
+            *out = &ctx->tmaps[i].map;
+            return SPARDA_OK;
+        }
+    int slot = ctx->n_tmaps < SPARDA_MAX_TMAP_CACHE ? ctx->n_tmaps++ : (ctx->next_tmap++ % SPARDA_MAX_TMAP_CACHE);
+    sparda_tmap_entry* e = &ctx->tmaps[slot];
+    typedef CUresult (*encode_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    cuuint64_t gdim[2] = {(cuuint64_t)head_dim, (cuuint64_t)rows};
+    cuuint64_t gstride[1] = {(cuuint64_t)head_dim * 2};
+    cuuint32_t box[2] = {64, 64};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = ((encode_t)ctx->encode_fn)(&e->map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstride, box,
+                                            estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        e->base = nullptr;
+        return SPARDA_ECUDA;
+    }
+    e->base = base;
+    e->rows = rows;
+    e->head_dim = head_dim;
+    *out = &e->map;
+    return SPARDA_OK;
+}

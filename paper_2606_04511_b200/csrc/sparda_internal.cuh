@@ -1,0 +1,180 @@
+// Internal declarations shared by the libsparda translation units (sm_100a only).
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sparda.h"
+
+#define SPARDA_MAX_TMAP_CACHE 16
+#define SPARDA_MAX_G 16        // query heads per group, padded to the M=16 of mma.m16n8k16
+#define SPARDA_ATTN_WARPS 4    // consumer warps (= smem stages) of the sparse-decode CTA
+
+struct sparda_tmap_entry {
+    const void* base;
+    uint64_t rows;
+    int head_dim;
+    CUtensorMap map;
+};
+
+struct sparda_ctx {
+    sparda_config cfg;
+    int sm_count;
+    int R;             // B * Hkv
+    int G;             // Hq / Hkv
+    int max_splits;    // partial slots per row in the workspace
+    // workspace (device)
+    float* part_O;     // [R][max_splits][16][D]
+    float* part_ml;    // [R][max_splits][2][16]  (m in log2 domain, l)
+    float* scores;     // [R][max_blocks] select scratch (orderable keys as uint32)
+    unsigned int* tickets;  // [2][R]: [0] = select, [1] = attention
+    cudaEvent_t* ev_sel;    // [max_layers + 1]
+    cudaEvent_t* ev_gather; // [max_layers + 1]
+    int max_layers;
+    int64_t launches;
+    char cuda_err[256];
+    // TMA descriptor cache (host)
+    sparda_tmap_entry tmaps[SPARDA_MAX_TMAP_CACHE];
+    int n_tmaps, next_tmap;
+    void* encode_fn;   // cuTensorMapEncodeTiled
+};
+
+int sparda_set_cuda_error(sparda_ctx* ctx, cudaError_t e, const char* where);
+#define SPARDA_CUDA_TRY(ctx, call)                                             \
+    do {                                                                       \
+        cudaError_t e__ = (call);                                              \
+        if (e__ != cudaSuccess) return sparda_set_cuda_error(ctx, e__, #call); \
+    } while (0)
+
+static inline bool sparda_aligned(const void* p, uintptr_t a) { return p != nullptr && ((uintptr_t)p & (a - 1)) == 0; }
+
+// launchers implemented in the kernel translation units
+int sparda_launch_pool_keys(sparda_ctx*, const void* kv, int64_t n_rows, int n_blocks, void* kpool, cudaStream_t);
+int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
+                         int32_t* ids, cudaStream_t);
+int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
+                         cudaStream_t);
+int sparda_launch_attn(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
+                       int n_slots, void* O, cudaStream_t);
+int sparda_launch_prefill_select(sparda_ctx*, const void* F, const void* Kpool, int T, int n_blocks, int row0,
+                                 int n_rows, int topk, int32_t* ids, cudaStream_t);
+int sparda_launch_prefill_baseline(sparda_ctx*, const void* Q, const void* Kpool, int T, int n_blocks, int row0,
+                                   int n_rows, int topk, int32_t* ids, cudaStream_t);
+int sparda_get_tmap(sparda_ctx*, const void* base, uint64_t rows, int head_dim, const CUtensorMap** out);
+int sparda_resolve_splits(const sparda_ctx*, int topk);
+
+#ifdef __CUDACC__
+// ------------------------------------------------------------------------------------------------
+// Device helpers (inline PTX for sm_100a)
+// ------------------------------------------------------------------------------------------------
+namespace sparda {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+// 1-D bulk copies (TMA engine, no tensor map)
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void bulk_wait() {
+    asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// 2-D tiled TMA load through a tensor map (coordinates: x = innermost element index, y = row)
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::
+            "r"(smem_u32(smem_dst)),
+        "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+__device__ __forceinline__ void ldmatrix_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2,
+                                                  uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+// D(16x8, fp32) += A(16x16, bf16, row) * B(16x8, bf16, col)
+__device__ __forceinline__ void mma_bf16_16816(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
+
+__device__ __forceinline__ int4 ld_nc_v4(const void* p) {
+    int4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_na_v4(void* p, const int4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w)
+                 : "memory");
+}
+
+// order-preserving map fp32 -> uint32 (larger float <=> larger key)
+__device__ __forceinline__ uint32_t orderable(float f) {
+    uint32_t b = __float_as_uint(f);
+    return b ^ ((b >> 31) ? 0xFFFFFFFFu : 0x80000000u);
+}
+
+}  // namespace sparda
+#endif

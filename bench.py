@@ -1,0 +1,491 @@
+#!/usr/bin/env python
+"""bench.py -- decode tokens/s at 128K context for the SparDA decode hot path on B200 (libsparda).
+
+Contract (driver):  python bench.py --gpus N --steps K --warmup W [--impl reference]
+One JSON line on stdout (rank 0).  A "step" is one decode step of the whole hot path over one batch:
+32 Forecast selections (a1+a2), 31 UVA gathers from pinned host memory (a3), the event hand-off (a4) and 32
+block-sparse GQA attentions (a5/a6) -- Algorithm 2 lines 4-7 for 32 layers.
+
+Workload at N=1: BASELINE.json configs[2] ("32-layer lookahead decode pipeline at 128K", batch 4), the
+configuration the metric "decode tok/s at 128K" is quoted on that fits one GPU box (16 GiB of pinned host
+KV).  configs[3] (batch 32, 137 GB pinned) is reachable with --workload cfg4 [--batch B] and aliases the
+host cache onto fewer resident layers when the box cannot pin that much.
+
+N > 1 (torchrun): every rank runs the same per-GPU workload on its own sequences (batch shards, no
+collective on the data path -- SURVEY 8(e)); value = tokens all ranks decoded / max-over-ranks device time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "decode_tokens_per_s_128k"
+UNIT = "tok/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="sparda", choices=["sparda", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg3", "cfg4"])
+    ap.add_argument("--batch", type=int, default=0, help="override the workload's batch (cfg4 sweep: 8/16/32)")
+    ap.add_argument("--layers", type=int, default=0, help="override the layer count (debug; invalid as a bench value)")
+    ap.add_argument("--gather-ctas", type=int, default=0)
+    ap.add_argument("--gather-mode", default="tma", choices=["tma", "ldg"])
+    ap.add_argument("--host-gib", type=float, default=0.0, help="cap on pinned host KV per rank (GiB); 0 = auto")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-kernels", action="store_true", help="skip the batch-32 per-kernel HBM roofline section")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def workload_config(args):
+    from paper_2606_04511_b200 import synth
+    cfg = synth.CFG3_128K if args.workload == "cfg3" else synth.CFG4_128K
+    if args.batch:
+        cfg = cfg.with_(batch=args.batch)
+    if args.layers:
+        cfg = cfg.with_(n_layers=args.layers)
+    return cfg
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled DURING the timed region
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, gpu_id: str):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", gpu_id, f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(",") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, smax, power, reasons = [], [], [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[0])), smax.append(float(r[1])), power.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(self.NAMES, r[3:7]):
+                if v.strip().lower() == "active":
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline and --impl reference).  The only place bench.py touches oracle/.
+# ------------------------------------------------------------------------------------------------
+def _oracle_layer_step(oracle, lay, prev_F, k, layer0):
+    """One layer of Algorithm 2 lines 4-7 on the CPU oracle: select, gather, attention."""
+    ids, _ = oracle.forecast_select(prev_F, lay["kpool"], k)
+    if layer0:
+        oracle.sparse_attn(lay["Q"], lay["kv"], ids, pool_is_indexed=True)
+    else:
+        pool = oracle.gather(lay["kv"], ids)
+        oracle.sparse_attn(lay["Q"], pool, ids)
+
+
+def _oracle_sample_layers(cfg, n, device="cpu"):
+    """n layers of oracle inputs (uint16 bit arrays), generated with the shared seeded generator; the pooled
+    keys come from the oracle's own pooling (o1), outside the timed region (a0 is a pre-condition)."""
+    import numpy as np
+    import torch
+    from oracle import sparda_oracle as oracle
+    from paper_2606_04511_b200 import synth
+    out = []
+    for l in range(n):
+        L = synth.decode_layer(cfg, l, device=device)
+        bits = {key: L[key].cpu().contiguous().view(torch.int16).numpy().view(np.uint16) for key in ("kv", "F", "Q", "F0cur")}
+        bits["kpool"] = oracle.pool_keys(bits["kv"])
+        out.append(bits)
+    return out
+
+
+def cpu_baseline(cfg, layers_bits, target_s):
+    """Oracle timed on this box's host cores on a bounded sample: whole layers of the decode step, as many as
+    fit in ~target_s seconds, scaled to the full layer count."""
+    from oracle import sparda_oracle as oracle
+    t0 = time.perf_counter()
+    done = 0
+    while done < 4 * cfg.n_layers:                          # whole layer-steps until ~target_s of CPU time
+        l = done % cfg.n_layers
+        lay = layers_bits[l % len(layers_bits)]
+        prev = layers_bits[(l - 1) % len(layers_bits)]
+        _oracle_layer_step(oracle, lay, lay["F0cur"] if l == 0 else prev["F"], cfg.topk, layer0=(l == 0))
+        done += 1
+        if time.perf_counter() - t0 >= target_s:
+            break
+    el = time.perf_counter() - t0
+    per_step_s = el * cfg.n_layers / done
+    return {"value": cfg.batch / per_step_s, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"{done} layer-steps (select + gather + sparse attention, batch {cfg.batch}, 128K, "
+                      f"{cfg.n_layers} per decode step) in {el:.2f} s, scaled to one {cfg.n_layers}-layer step",
+            "seconds_per_decode_step": per_step_s}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = workload_config(args)
+    from oracle import sparda_oracle as oracle
+    oracle.build()
+    n_sample = 2                                            # layer 0 (indexed cache) + one gathered layer per step
+    layers_bits = _oracle_sample_layers(cfg, n_sample)
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        for l in range(n_sample):
+            _oracle_layer_step(oracle, layers_bits[l], layers_bits[0]["F0cur"] if l == 0 else layers_bits[l - 1]["F"],
+                               cfg.topk, layer0=(l == 0))
+        if it >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    per_step_s = statistics.mean(times) * cfg.n_layers / n_sample
+    val = cfg.batch / per_step_s
+    sample = (f"each step = {n_sample} of {cfg.n_layers} layer-steps (layer 0 + one gathered layer) of the oracle at batch "
+              f"{cfg.batch}, 128K, scaled to {cfg.n_layers} layers")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": per_step_s * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "batch": cfg.batch, "context": cfg.context, "layers": cfg.n_layers,
+                       "topk": cfg.topk, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+def measure_h2d_ceiling(torch, host_chunks):
+    """cudaMemcpyAsync pinned host -> device ceiling on this box: the denominator of the gather's roofline.
+    Copies whole pinned layer buffers (>= 256 MiB each) back to back, best of 5 passes, CUDA events."""
+    dev = torch.empty_like(host_chunks[0], device="cuda")
+    nbytes = sum(h.numel() * h.element_size() for h in host_chunks)
+    best = 0.0
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for h in host_chunks:
+            dev.copy_(h, non_blocking=True)
+        e1.record()
+        e1.synchronize()
+        best = max(best, nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return best
+
+
+def bench_kernels_b32(torch, binding, peaks, args):
+    """Per-kernel HBM rooflines at the batch-32 shape of BASELINE.json configs[3] (R = 64 rows, 2048 blocks,
+    top-64, D = 128), where the ideal times (5 us select, 20 us attention) stand clear of the launch floor
+    (SURVEY 8(d)).  Cold HBM: each launch works on the next of NSETS buffer sets, together larger than L2."""
+    from paper_2606_04511_b200 import synth
+    cfg = synth.CFG4_128K
+    R, Nb, k, D = cfg.rows, cfg.n_blocks, cfg.topk, cfg.head_dim
+    ctx = binding.Sparda.from_config(cfg)
+    g = torch.Generator(device="cuda").manual_seed(40)
+    NS_SEL, NS_ATT = 8, 4                                    # 8 x 32 MiB Kpool, 4 x 128 MiB pool: each ring > 126 MB L2
+    kpools = [torch.randn((R, Nb, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(NS_SEL)]
+    Fs = [torch.randn((R, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(NS_SEL)]
+    pools = []
+    for _ in range(NS_ATT):
+        p = torch.empty((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda")
+        p.copy_(torch.randn(p.shape, generator=g, device="cuda", dtype=torch.float32))
+        pools.append(p)
+    Q = torch.randn((cfg.batch, cfg.n_q_heads, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+    O = torch.empty_like(Q)
+    ids = torch.empty((R, k), dtype=torch.int32, device="cuda")
+    ids_att = torch.arange(k, dtype=torch.int32, device="cuda").repeat(R, 1).contiguous()
+    st = torch.cuda.current_stream()
+
+    def timed(fn, n_sets, reps=10):
+        for i in range(2 * n_sets):
+            fn(i % n_sets)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for i in range(reps * n_sets):
+            fn(i % n_sets)
+        e1.record(st)
+        e1.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / (reps * n_sets)
+
+    t_sel = timed(lambda i: ctx.forecast_select(Fs[i], kpools[i], Nb, k, ids), NS_SEL)
+    t_att = timed(lambda i: ctx.sparse_decode(Q, pools[i], ids_att, k, O), NS_ATT)
+    sel_bytes = cfg.kpool_bytes_per_layer + R * D * 2 + R * k * 4
+    att_bytes = cfg.gather_bytes_per_layer + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
+    out = []
+    for name, t, b in (("forecast_select_kernel<128>", t_sel, sel_bytes), ("sparse_decode_kernel<128>", t_att, att_bytes)):
+        out.append({"kernel": name, "workload": "cfg4 shape, batch 32, one layer, cold HBM (rotating buffer sets > L2)",
+                    "bound": "hbm", "us_per_launch": t * 1e6, "algorithmic_bytes": b, "achieved": b / t / 1e9,
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": b / t / 1e9 / peaks["hbm_gbs"],
+                    "frac_of_nominal_8tbs": b / t / 1e9 / 8000.0, "peak_source": peaks["source"], "traffic": None})
+    out[1]["attn_splits"] = ctx.attn_splits(k)
+    ctx.close()
+    del kpools, pools
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_sparda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_04511_b200 import binding, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libsparda has no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    assert args.warmup >= 3, "timing rules: at least 3 warm-up steps"
+    peaks = load_peaks()
+    cfg = workload_config(args)
+    cfg = cfg.with_(seed=cfg.seed + 1000 * rank)             # every rank decodes its own sequences
+    R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
+
+    mode = binding.GATHER_TMA if args.gather_mode == "tma" else binding.GATHER_LDG
+    ctx = binding.Sparda.from_config(cfg, max_layers=NL, gather_ctas=args.gather_ctas, gather_mode=mode)
+
+    # ---- pinned host KV: as many distinct layers as the box can hold, layer l -> l mod resident otherwise
+    import psutil
+    per_layer = cfg.kv_bytes_per_layer
+    avail = psutil.virtual_memory().available / max(1, int(os.environ.get("LOCAL_WORLD_SIZE", world)))
+    cap = args.host_gib * 2**30 if args.host_gib > 0 else 0.5 * avail
+    resident = max(1, min(NL - 1, int(cap // per_layer)))
+    host_kv = [torch.empty((R, Nb, 2, cfg.block_size, D), dtype=torch.bfloat16, pin_memory=True) for _ in range(resident)]
+    dev_layers, host_vals = [], []
+    kv0 = None
+    for l in range(NL):
+        gen_needed = l == 0 or (l - 1) < resident
+        L = synth.decode_layer(cfg, l, device="cuda")        # F/Q always; kv only where it is stored
+        kpool = torch.empty((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+        if l == 0:
+            kv0 = L["kv"]
+            ctx.pool_keys(kv0, R, Nb, kpool)
+            F0 = L["F0cur"]
+            kv = kv0
+        else:
+            slot = (l - 1) % resident
+            if gen_needed:
+                host_kv[slot].copy_(L["kv"])
+                ctx.pool_keys(L["kv"], R, Nb, kpool)
+            else:                                            # aliased layer: pooled keys of the aliased cache
+                kpool.copy_(dev_layers[1 + slot]["Kpool"])
+            kv = host_kv[slot]
+        dev_layers.append({"F": L["F"], "Q": L["Q"], "Kpool": kpool, "kv": kv,
+                           "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                           "ids": torch.full((R, k), -1, dtype=torch.int32, device="cuda")})
+        host_vals.append({"F": L["F"].cpu().pin_memory(), "Q": L["Q"].cpu().pin_memory(),
+                          "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16).pin_memory()})
+        del L
+    torch.cuda.synchronize()
+    F0_host = F0.cpu().pin_memory()
+    pools = [torch.zeros((R, k, 2, cfg.block_size, D), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    arr = ctx.make_layers(dev_layers)
+    arr_host = ctx.make_layers([{**d, **h} for d, h in zip(dev_layers, host_vals)])
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+
+    ceiling = measure_h2d_ceiling(torch, host_kv[:min(4, resident)])
+
+    def step(m=binding.STEP_OVERLAP):
+        ctx.decode_step(arr, F0, Nb, k, pools[0], pools[1], cs, ps, m)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_region(fn, n):
+        """K steps bracketed by barrier + synchronize on both sides, CUDA events on the compute stream."""
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(cs)
+        for _ in range(n):
+            fn()
+        e1.record(cs)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    # ---- timed region: device-resident Q/F/Kpool, KV in pinned host memory (the method's offload tier)
+    for _ in range(args.warmup):
+        step()
+    props = torch.cuda.get_device_properties(local)
+    gpu_id = f"GPU-{props.uuid}" if getattr(props, "uuid", None) else str(local)
+    sampler = ClockSampler(gpu_id) if rank == 0 else None
+    time.sleep(0.15)
+    launches0 = ctx.launch_count
+    ms_total = timed_region(step, args.steps)
+    launches = ctx.launch_count - launches0
+    # keep the sampler running through the e2e region too (same load)
+    def step_host():
+        ctx.decode_step_host(arr_host, F0_host, Nb, k, pools[0], pools[1], cs, ps, binding.STEP_OVERLAP)
+        cs.synchronize()                                     # the caller reads O of this step on the host
+    for _ in range(args.warmup):
+        step_host()
+    ms_e2e = timed_region(step_host, args.steps)
+    clocks = sampler.stop() if sampler else None
+
+    # serialized pipeline (same kernels, one stream): what the overlap buys
+    for _ in range(2):
+        step(binding.STEP_SERIAL)
+    ms_serial = timed_region(lambda: step(binding.STEP_SERIAL), max(3, args.steps // 3)) / max(3, args.steps // 3)
+
+    # ---- per-kernel device times inside the pipeline (second pass over the same K steps, timing events on)
+    ctx.profile_enable(True)
+    prof = {"select": [0.0, 0], "gather": [0.0, 0], "attn": [0.0, 0]}
+    for _ in range(args.steps):
+        step()
+        torch.cuda.synchronize()
+        for kind, (ms, n) in ctx.profile_read().items():
+            prof[kind][0] += ms
+            prof[kind][1] += n
+    ctx.profile_enable(False)
+
+    ms_per_step = ms_total / args.steps
+    tokens = cfg.batch * world
+    value = tokens / (ms_per_step * 1e-3)
+    e2e_value = tokens / (ms_e2e / args.steps * 1e-3)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    def per(kind):
+        ms, n = prof[kind]
+        return ms / n * 1e-3 if n else float("nan")
+    t_sel, t_gat, t_att = per("select"), per("gather"), per("attn")
+    gather_bytes = cfg.gather_bytes_per_layer
+    sel_bytes = cfg.kpool_bytes_per_layer + R * D * 2 + R * k * 4
+    att_bytes = cfg.gather_bytes_per_layer + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
+    roofline = {"kernel": "gather_tma_kernel" if args.gather_mode == "tma" else "gather_ldg_kernel",
+                "bound": "host_link", "achieved": gather_bytes / t_gat / 1e9, "peak": ceiling, "unit": "GB/s",
+                "frac": gather_bytes / t_gat / 1e9 / ceiling, "traffic": None,
+                "peak_source": "cudaMemcpyAsync pinned host->device, measured in this run on this box",
+                "us_per_launch": t_gat * 1e6, "algorithmic_bytes": gather_bytes,
+                "share_of_step": prof["gather"][0] / args.steps / ms_per_step,
+                "note": "dominant kernel of the step; its roofline is the host link, not HBM (DESIGN.md 'Kernels')"}
+    kernels = [
+        {"kernel": "forecast_select_kernel<128>", "workload": f"{cfg.name} in-pipeline", "bound": "hbm",
+         "us_per_launch": t_sel * 1e6, "algorithmic_bytes": sel_bytes, "achieved": sel_bytes / t_sel / 1e9,
+         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": sel_bytes / t_sel / 1e9 / peaks["hbm_gbs"], "traffic": None,
+         "note": "launch-latency-sized at batch 4 (ideal 0.64 us)"},
+        {"kernel": "sparse_decode_kernel<128>", "workload": f"{cfg.name} in-pipeline (pool just written by the gather: L2-warm)",
+         "bound": "hbm", "us_per_launch": t_att * 1e6, "algorithmic_bytes": att_bytes, "achieved": att_bytes / t_att / 1e9,
+         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": att_bytes / t_att / 1e9 / peaks["hbm_gbs"], "traffic": None,
+         "note": "launch-latency-sized at batch 4 (ideal 2.6 us)"},
+    ]
+    if not args.no_kernels:
+        del pools
+        kernels += bench_kernels_b32(torch, binding, peaks, args)
+
+    base = None
+    if not args.no_cpu_baseline and world == 1:
+        from oracle import sparda_oracle as oracle
+        oracle.build()
+        import numpy as np
+        n_s = min(2, NL)
+        bits = []
+        for l in range(n_s):
+            d = dev_layers[l]
+            kvb = (kv0 if l == 0 else d["kv"])
+            bits.append({"kv": kvb.cpu().contiguous().view(torch.int16).numpy().view(np.uint16),
+                         "kpool": d["Kpool"].cpu().view(torch.int16).numpy().view(np.uint16),
+                         "F": d["F"].cpu().view(torch.int16).numpy().view(np.uint16),
+                         "Q": d["Q"].cpu().view(torch.int16).numpy().view(np.uint16),
+                         "F0cur": F0.cpu().view(torch.int16).numpy().view(np.uint16)})
+        base = cpu_baseline(cfg, bits, args.cpu_seconds)
+
+    staged = (R * D * 2) * NL + (cfg.batch * cfg.n_q_heads * D * 2) * NL
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": cfg.name, "batch_per_gpu": cfg.batch, "global_batch": tokens, "context": cfg.context,
+                   "layers": NL, "q_heads": cfg.n_q_heads, "kv_heads": cfg.n_kv_heads, "head_dim": D, "block": cfg.block_size,
+                   "topk": k, "parallelism": f"batch shards x{world}, no collective",
+                   "kv_residency": f"layers 1..{NL - 1} in pinned host memory ({resident} distinct resident layers"
+                                   + ("" if resident >= NL - 1 else f", layer l -> (l-1) mod {resident}") + "), layer 0 in HBM",
+                   "fresh_fetch_fraction": 1.0,
+                   "l2": f"inputs larger than L2: {(cfg.kpool_bytes_per_layer * NL + gather_bytes * (NL - 1)) / 2**20:.0f} MiB touched per step",
+                   "gather": {"mode": args.gather_mode, "ctas": ctx.gather_ctas}, "attn_splits": ctx.attn_splits(k)},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
+                "h2d_bytes_per_step": staged + gather_bytes * (NL - 1), "d2h_bytes_per_step": cfg.batch * cfg.n_q_heads * D * 2 * NL,
+                "h2d_staged_bytes_per_step": staged, "h2d_uva_gather_bytes_per_step": gather_bytes * (NL - 1),
+                "api": "sparda_decode_step_host (pinned host F/Q/O, copies inside the call) + stream sync per step"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "roofline_kernels": kernels,
+        "cpu_baseline": base,
+        "pipeline": {"ms_per_step_overlap": ms_per_step, "ms_per_step_serial": ms_serial,
+                     "us_per_layer_step": ms_per_step * 1e3 / NL,
+                     "us_select": t_sel * 1e6, "us_gather": t_gat * 1e6, "us_attn": t_att * 1e6,
+                     "gather_exposed_us_per_layer": max(0.0, (ms_per_step * 1e3 - (t_sel * NL + t_att * NL) * 1e6) / max(1, NL - 1)),
+                     "host_link_ceiling_gbs": ceiling, "gather_gbs": gather_bytes / t_gat / 1e9,
+                     "tok_s_ceiling_at_host_link": cfg.batch * world / (gather_bytes * (NL - 1) / (ceiling * 1e9))},
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_sparda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

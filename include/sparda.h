@@ -140,6 +140,24 @@ int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers
                        int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
                        int mode);
 
+/* The same step for a caller whose per-step tensors live in HOST memory (the end-to-end form bench.py times):
+ * layers[l].F, .Q and .O and F0cur are HOST pointers (pinned for the copies to be asynchronous); the call
+ * enqueues on compute_stream the host->device copies of F0cur and every layer's F and Q into staging owned by
+ * the context, runs sparda_decode_step on the staged tensors, and enqueues the device->host copy of every
+ * layer's O.  layers[l].Kpool, .kv and .ids keep their sparda_decode_step meaning.  No host synchronisation:
+ * O is valid once compute_stream has drained.  Needs n_layers <= max_layers.                                  */
+int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
+                            int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
+                            int mode);
+
+/* Per-kernel device timing of sparda_decode_step (measurement aid).  While enabled, every kernel
+ * launched by sparda_decode_step is bracketed by timing events on the stream it is launched on (after any
+ * stream wait, so a wait is not counted).  sparda_profile_read synchronises on those events and returns, for
+ * kind 0 = select, 1 = gather, 2 = attention, the summed milliseconds and launch counts of the LAST
+ * sparda_decode_step call.  Not capturable into a CUDA graph while enabled.                                   */
+int sparda_profile_enable(sparda_ctx* ctx, int on);
+int sparda_profile_read(sparda_ctx* ctx, double ms_out[3], int64_t count_out[3]);
+
 /* (a7) Chunked-prefill selection with the Forecast indexer, Alg.1 l.2: for query positions
  * i = row0 .. row0+n_rows-1 of every group g, scores = F[g,i,:] . Kpool[g,j,:] for the causal candidates
  * j < (i+1)/S (a block is visible once its last token <= i), top-k as in forecast_select.

@@ -19,7 +19,8 @@ STEP_OVERLAP, STEP_SERIAL = 0, 1
 
 EXPORTS = [
     "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_select", "sparda_prefetch_launch",
-    "sparda_sparse_decode", "sparda_decode_step", "sparda_prefill_select", "sparda_prefill_select_baseline",
+    "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
+    "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
     "sparda_launch_count", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
     "sparda_last_cuda_error", "sparda_version",
 ]
@@ -59,6 +60,9 @@ def lib() -> ctypes.CDLL:
         L.sparda_prefetch_launch.argtypes = [vp, vp, i32, vp, i32, vp, vp]
         L.sparda_sparse_decode.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_decode_step.argtypes = [vp, ctypes.POINTER(SpardaLayer), i32, vp, i32, i32, vp, vp, vp, vp, i32]
+        L.sparda_decode_step_host.argtypes = L.sparda_decode_step.argtypes
+        L.sparda_profile_enable.argtypes = [vp, i32]
+        L.sparda_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
         L.sparda_prefill_select.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
         L.sparda_prefill_select_baseline.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
         L.sparda_launch_count.argtypes = [vp]
@@ -157,6 +161,23 @@ class Sparda:
         self._check(self._L.sparda_decode_step(self._h, layer_array, len(layer_array), _ptr(F0cur), n_blocks, topk,
                                                _ptr(pool0), _ptr(pool1), _stream(compute_stream),
                                                _stream(prefetch_stream), mode), "decode_step")
+
+    def decode_step_host(self, layer_array, F0cur, n_blocks, topk, pool0, pool1, compute_stream=None,
+                         prefetch_stream=None, mode=STEP_OVERLAP):
+        """F, Q, O of every layer and F0cur are (pinned) HOST tensors; copies are enqueued inside the call."""
+        self._check(self._L.sparda_decode_step_host(self._h, layer_array, len(layer_array), _ptr(F0cur), n_blocks, topk,
+                                                    _ptr(pool0), _ptr(pool1), _stream(compute_stream),
+                                                    _stream(prefetch_stream), mode), "decode_step_host")
+
+    def profile_enable(self, on=True):
+        self._check(self._L.sparda_profile_enable(self._h, 1 if on else 0), "profile_enable")
+
+    def profile_read(self):
+        """-> {"select": (ms, n), "gather": (ms, n), "attn": (ms, n)} of the last decode_step."""
+        ms = (ctypes.c_double * 3)()
+        n = (ctypes.c_int64 * 3)()
+        self._check(self._L.sparda_profile_read(self._h, ms, n), "profile_read")
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(("select", "gather", "attn"))}
 
     def prefill_select(self, F, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, stream=None):
         self._check(self._L.sparda_prefill_select(self._h, _ptr(F), _ptr(Kpool), T, n_blocks, row0, n_rows, topk,

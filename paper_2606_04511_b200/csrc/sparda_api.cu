@@ -1,4 +1,5 @@
 // libsparda: context, argument validation and the Algorithm-2 stream choreography (include/sparda.h).
+#include <alloca.h>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -99,10 +100,16 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
               cudaMemset(ctx->tickets, 0, 2 * (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
     ctx->ev_gather = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
-    ok = ok && ctx->ev_sel && ctx->ev_gather;
+    ctx->ev_prof = (cudaEvent_t*)calloc((size_t)3 * (ctx->max_layers + 1) * 2, sizeof(cudaEvent_t));
+    ok = ok && ctx->ev_sel && ctx->ev_gather && ctx->ev_prof;
     for (int i = 0; ok && i <= ctx->max_layers; ++i)
         ok = cudaEventCreateWithFlags(&ctx->ev_sel[i], cudaEventDisableTiming) == cudaSuccess &&
              cudaEventCreateWithFlags(&ctx->ev_gather[i], cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; ok && i < 3 * (ctx->max_layers + 1) * 2; ++i) ok = cudaEventCreate(&ctx->ev_prof[i]) == cudaSuccess;
+    const size_t f_bytes = (size_t)ctx->R * D * 2, q_bytes = (size_t)cfg->batch * cfg->n_q_heads * D * 2;
+    ok = ok && cudaMalloc(&ctx->stage_F, f_bytes * (ctx->max_layers + 1)) == cudaSuccess &&
+         cudaMalloc(&ctx->stage_Q, q_bytes * ctx->max_layers) == cudaSuccess &&
+         cudaMalloc(&ctx->stage_O, q_bytes * ctx->max_layers) == cudaSuccess;
     if (!ok) {
         (void)cudaGetLastError();
         sparda_destroy(ctx);
@@ -128,8 +135,14 @@ int sparda_destroy(sparda_ctx* ctx) {
         if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);
         if (ctx->ev_gather && ctx->ev_gather[i]) cudaEventDestroy(ctx->ev_gather[i]);
     }
+    for (int i = 0; ctx->ev_prof && i < 3 * (ctx->max_layers + 1) * 2; ++i)
+        if (ctx->ev_prof[i]) cudaEventDestroy(ctx->ev_prof[i]);
+    cudaFree(ctx->stage_F);
+    cudaFree(ctx->stage_Q);
+    cudaFree(ctx->stage_O);
     free(ctx->ev_sel);
     free(ctx->ev_gather);
+    free(ctx->ev_prof);
     (void)cudaGetLastError();
     delete ctx;
     return SPARDA_OK;
@@ -186,6 +199,18 @@ int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* K
 //   ->  wait ev_gather[l]  ->  attention l.
 // Buffer hand-off (double-buffered pool): gather l+1 writes pool[(l+1)&1], last read by attention l-1, which
 // precedes select B_{l+1} on the compute stream, so ev_sel[l+1] also releases the buffer.
+// timing events around one launch of `kind` (0 select, 1 gather, 2 attention) on stream st
+static inline cudaEvent_t* prof_slot(sparda_ctx* ctx, int kind) {
+    return &ctx->ev_prof[((size_t)kind * (ctx->max_layers + 1) + ctx->prof_n[kind]) * 2];
+}
+#define SPARDA_PROF_BEGIN(kind, st) \
+    if (ctx->prof_on) SPARDA_CUDA_TRY(ctx, cudaEventRecord(prof_slot(ctx, kind)[0], st))
+#define SPARDA_PROF_END(kind, st)                                               \
+    if (ctx->prof_on) {                                                         \
+        SPARDA_CUDA_TRY(ctx, cudaEventRecord(prof_slot(ctx, kind)[1], st));     \
+        ctx->prof_n[kind]++;                                                    \
+    }
+
 int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                        int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
                        int mode) {
@@ -196,28 +221,88 @@ int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers
     cudaStream_t ps = mode == SPARDA_STEP_OVERLAP ? (cudaStream_t)prefetch_stream : cs;
     void* pools[2] = {dev_pool0, dev_pool1};
     int rc;
+    ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
     // layer 0: same-layer selection with F0cur
+    SPARDA_PROF_BEGIN(0, cs);
     rc = sparda_forecast_select(ctx, F0cur, layers[0].Kpool, n_blocks, n_blocks, topk, layers[0].ids, cs);
     if (rc) return rc;
+    SPARDA_PROF_END(0, cs);
     for (int l = 0; l < n_layers; ++l) {
         if (l + 1 < n_layers) {
+            SPARDA_PROF_BEGIN(0, cs);
             rc = sparda_forecast_select(ctx, layers[l].F, layers[l + 1].Kpool, n_blocks, n_blocks, topk, layers[l + 1].ids, cs);
             if (rc) return rc;
+            SPARDA_PROF_END(0, cs);
             if (ps != cs) {
                 SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], cs));
                 SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ps, ctx->ev_sel[l + 1], 0));
             }
+            SPARDA_PROF_BEGIN(1, ps);
             rc = sparda_prefetch_launch(ctx, layers[l + 1].kv, n_blocks, layers[l + 1].ids, topk, pools[(l + 1) & 1], ps);
             if (rc) return rc;
+            SPARDA_PROF_END(1, ps);
             if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], ps));
         }
         if (l == 0) {
+            SPARDA_PROF_BEGIN(2, cs);
             rc = sparda_sparse_decode(ctx, layers[0].Q, layers[0].kv, layers[0].ids, topk, 1, n_blocks, layers[0].O, cs);
         } else {
             if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
+            SPARDA_PROF_BEGIN(2, cs);
             rc = sparda_sparse_decode(ctx, layers[l].Q, pools[l & 1], layers[l].ids, topk, 0, topk, layers[l].O, cs);
         }
         if (rc) return rc;
+        SPARDA_PROF_END(2, cs);
+    }
+    return SPARDA_OK;
+}
+
+int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
+                            int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
+                            int mode) {
+    if (!ctx || !layers || n_layers < 1 || n_layers > ctx->max_layers || !F0cur) return SPARDA_EINVAL;
+    cudaStream_t cs = (cudaStream_t)compute_stream;
+    const size_t f_bytes = (size_t)ctx->R * ctx->cfg.head_dim * 2;
+    const size_t q_bytes = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads * ctx->cfg.head_dim * 2;
+    sparda_layer* dl = (sparda_layer*)alloca(sizeof(sparda_layer) * (size_t)n_layers);
+    SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_F + f_bytes * ctx->max_layers, F0cur, f_bytes, cudaMemcpyHostToDevice, cs));
+    for (int l = 0; l < n_layers; ++l) {
+        if (!layers[l].Q || !layers[l].O || (l + 1 < n_layers && !layers[l].F)) return SPARDA_EINVAL;
+        dl[l] = layers[l];
+        dl[l].F = ctx->stage_F + f_bytes * l;
+        dl[l].Q = ctx->stage_Q + q_bytes * l;
+        dl[l].O = ctx->stage_O + q_bytes * l;
+        if (l + 1 < n_layers) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_F + f_bytes * l, layers[l].F, f_bytes, cudaMemcpyHostToDevice, cs));
+        SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_Q + q_bytes * l, layers[l].Q, q_bytes, cudaMemcpyHostToDevice, cs));
+    }
+    int rc = sparda_decode_step(ctx, dl, n_layers, ctx->stage_F + f_bytes * ctx->max_layers, n_blocks, topk, dev_pool0, dev_pool1,
+                                compute_stream, prefetch_stream, mode);
+    if (rc) return rc;
+    for (int l = 0; l < n_layers; ++l)
+        SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(layers[l].O, ctx->stage_O + q_bytes * l, q_bytes, cudaMemcpyDeviceToHost, cs));
+    return SPARDA_OK;
+}
+
+int sparda_profile_enable(sparda_ctx* ctx, int on) {
+    if (!ctx) return SPARDA_EINVAL;
+    ctx->prof_on = on ? 1 : 0;
+    ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
+    return SPARDA_OK;
+}
+
+int sparda_profile_read(sparda_ctx* ctx, double ms_out[3], int64_t count_out[3]) {
+    if (!ctx || !ms_out || !count_out) return SPARDA_EINVAL;
+    for (int k = 0; k < 3; ++k) {
+        double sum = 0.0;
+        for (int i = 0; i < ctx->prof_n[k]; ++i) {
+            cudaEvent_t* e = &ctx->ev_prof[((size_t)k * (ctx->max_layers + 1) + i) * 2];
+            float ms = 0.f;
+            SPARDA_CUDA_TRY(ctx, cudaEventSynchronize(e[1]));
+            SPARDA_CUDA_TRY(ctx, cudaEventElapsedTime(&ms, e[0], e[1]));
+            sum += ms;
+        }
+        ms_out[k] = sum;
+        count_out[k] = ctx->prof_n[k];
     }
     return SPARDA_OK;
 }

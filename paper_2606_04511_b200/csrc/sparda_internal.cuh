@@ -32,6 +32,14 @@ struct sparda_ctx {
     cudaEvent_t* ev_sel;    // [max_layers + 1]
     cudaEvent_t* ev_gather; // [max_layers + 1]
     int max_layers;
+    // host-buffer step staging (device): F [(max_layers+1)][R][D] (slot max_layers = F0cur), Q and O [max_layers][B][Hq][D]
+    char* stage_F;
+    char* stage_Q;
+    char* stage_O;
+    // per-kernel timing of sparda_decode_step: events [kind 0..2][max_layers + 1][start, stop]
+    int prof_on;
+    cudaEvent_t* ev_prof;
+    int prof_n[3];
     int64_t launches;
     char cuda_err[256];
     // TMA descriptor cache (host)

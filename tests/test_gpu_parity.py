@@ -232,6 +232,41 @@ def test_decode_step_pipeline(cfg, sp, oracle):
         parity.check_attn(_bits(Os[l]), want, f"layer {l}")
 
 
+def test_decode_step_host_buffers_and_profile(sp):
+    """The host-buffer form of the step (what bench.py's e2e times) gives bit-identical O to the device form;
+    per-kernel profiling reports one select and one attention per layer and one gather per layer >= 1."""
+    cfg = G16.with_(n_layers=4)
+    ctx = sp.Sparda.from_config(cfg, max_layers=4)
+    R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim
+    dev, host = [], []
+    for l in range(cfg.n_layers):
+        L = synth.decode_layer(cfg, l, device="cuda")
+        kpool = torch.empty((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+        ctx.pool_keys(L["kv"], R, Nb, kpool)
+        kv = L["kv"] if l == 0 else L["kv"].cpu().pin_memory()
+        ids = torch.full((R, k), -9, dtype=torch.int32, device="cuda")
+        dev.append({"F": L["F"], "Q": L["Q"], "Kpool": kpool, "kv": kv, "ids": ids,
+                    "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda")})
+        host.append({"F": L["F"].cpu().pin_memory(), "Q": L["Q"].cpu().pin_memory(), "Kpool": kpool, "kv": kv, "ids": ids,
+                     "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16).pin_memory()})
+        if l == 0:
+            F0 = L["F0cur"]
+    pools = [torch.zeros((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    ctx.profile_enable(True)
+    ctx.decode_step(ctx.make_layers(dev), F0, Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)
+    torch.cuda.synchronize()
+    prof = ctx.profile_read()
+    assert prof["select"][1] == 4 and prof["gather"][1] == 3 and prof["attn"][1] == 4
+    assert all(ms > 0 for ms, _ in prof.values())
+    ctx.profile_enable(False)
+    ctx.decode_step_host(ctx.make_layers(host), F0.cpu().pin_memory(), Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)
+    torch.cuda.synchronize()
+    for d, h in zip(dev, host):
+        assert torch.equal(d["O"].cpu().view(torch.int16), h["O"].view(torch.int16))
+
+
 def test_cfg2_full_size_layer(sp, oracle):
     """BASELINE.json configs[1] at full size: batch 8, 32/2 heads, D=128, 512 blocks, top-64, KV pinned on host."""
     cfg = synth.CFG2_32K

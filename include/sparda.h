@@ -88,7 +88,8 @@ typedef struct {
 #define SPARDA_STEP_SERIAL 1     /* same kernels, everything on compute_stream in Algorithm-2 order (no overlap) */
 
 /* Create a context for one shape family on the current device.  Allocates the workspace (split-K partials
- * R*max_splits*16*(D+2) floats, score scratch R*max_blocks floats, tickets, 2*max_layers events).
+ * R*max_splits*16*(D+2) floats, score scratch R*max_blocks floats, tickets, 2*max_layers events, host-step
+ * staging, a 256 KiB-per-SM score tile for the comparison selector).
  * Returns SPARDA_OK, SPARDA_EINVAL, SPARDA_EUNSUPPORTED, SPARDA_ENOMEM or SPARDA_ECUDA; *out is set only on
  * success.  Destroy with sparda_destroy (synchronises the device first).                                     */
 int sparda_create(const sparda_config* cfg, sparda_ctx** out);
@@ -162,7 +163,9 @@ int sparda_profile_read(sparda_ctx* ctx, double ms_out[3], int64_t count_out[3])
  * i = row0 .. row0+n_rows-1 of every group g, scores = F[g,i,:] . Kpool[g,j,:] for the causal candidates
  * j < (i+1)/S (a block is visible once its last token <= i), top-k as in forecast_select.
  * F [Hkv][T][D], Kpool [Hkv][n_blocks][D], ids_out [Hkv][n_rows][topk]: device.  Dense bf16 contraction on
- * tcgen05 tensor cores (fp32 accumulators in TMEM) with a fused per-row top-k epilogue.                       */
+ * tcgen05 tensor cores (fp32 accumulators in TMEM) with a fused per-row top-k epilogue; scores never leave the
+ * SM.  Supported: n_blocks <= 512 (one 128 x 512 fp32 accumulator fills TMEM), topk <= 64, else SPARDA_EINVAL.
+ * Chunking: any [row0, row0 + n_rows) inside [0, T); one launch per call.                                     */
 int sparda_prefill_select(sparda_ctx* ctx, const void* F, const void* Kpool, int T, int n_blocks, int row0,
                           int n_rows, int topk, int32_t* ids_out, void* stream);
 

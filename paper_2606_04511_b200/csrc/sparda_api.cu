@@ -97,6 +97,7 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
               cudaMalloc(&ctx->part_ml, n_ml * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->scores, n_sc * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->tickets, 2 * (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
+              cudaMalloc(&ctx->pf_scratch, (size_t)ctx->sm_count * 512 * 128 * sizeof(float)) == cudaSuccess &&
               cudaMemset(ctx->tickets, 0, 2 * (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
     ctx->ev_gather = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
@@ -131,6 +132,7 @@ int sparda_destroy(sparda_ctx* ctx) {
     cudaFree(ctx->part_ml);
     cudaFree(ctx->scores);
     cudaFree(ctx->tickets);
+    cudaFree(ctx->pf_scratch);
     for (int i = 0; i <= ctx->max_layers; ++i) {
         if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);
         if (ctx->ev_gather && ctx->ev_gather[i]) cudaEventDestroy(ctx->ev_gather[i]);
@@ -180,7 +182,7 @@ int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, c
 
 int sparda_prefill_select(sparda_ctx* ctx, const void* F, const void* Kpool, int T, int n_blocks, int row0, int n_rows,
                           int topk, int32_t* ids_out, void* stream) {
-    if (!ctx || !sparda_aligned(F, 1024) || !sparda_aligned(Kpool, 1024) || !sparda_aligned(ids_out, 16)) return SPARDA_EINVAL;
+    if (!ctx || !sparda_aligned(F, 16) || !sparda_aligned(Kpool, 16) || !sparda_aligned(ids_out, 16)) return SPARDA_EINVAL;
     if (T < 1 || n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || row0 < 0 || n_rows < 1 || row0 + (int64_t)n_rows > T) return SPARDA_EINVAL;
     if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
     return sparda_launch_prefill_select(ctx, F, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, (cudaStream_t)stream);
@@ -188,7 +190,7 @@ int sparda_prefill_select(sparda_ctx* ctx, const void* F, const void* Kpool, int
 
 int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* Kpool, int T, int n_blocks, int row0,
                                    int n_rows, int topk, int32_t* ids_out, void* stream) {
-    if (!ctx || !sparda_aligned(Q, 1024) || !sparda_aligned(Kpool, 1024) || !sparda_aligned(ids_out, 16)) return SPARDA_EINVAL;
+    if (!ctx || !sparda_aligned(Q, 16) || !sparda_aligned(Kpool, 16) || !sparda_aligned(ids_out, 16)) return SPARDA_EINVAL;
     if (T < 1 || n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || row0 < 0 || n_rows < 1 || row0 + (int64_t)n_rows > T) return SPARDA_EINVAL;
     if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
     return sparda_launch_prefill_baseline(ctx, Q, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, (cudaStream_t)stream);
@@ -309,11 +311,12 @@ int sparda_profile_read(sparda_ctx* ctx, double ms_out[3], int64_t count_out[3])
 
 }  // extern "C"
 
-// TMA descriptor for a [rows][head_dim] bf16 view of a KV pool / cache: box = 64 rows x 64 elements (128 B),
+// TMA descriptor for a [rows][head_dim] bf16 view (KV pool / cache, F, Kpool): box = box_rows x 64 elements (128 B),
 // 128-byte swizzle.  Cached per (base, rows, head_dim): encoding costs a few microseconds on the host.
-int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_dim, const CUtensorMap** out) {
+int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_dim, int box_rows, const CUtensorMap** out) {
     for (int i = 0; i < ctx->n_tmaps; ++i)
-        if (ctx->tmaps[i].base == base && ctx->tmaps[i].rows == rows && ctx->tmaps[i].head_dim == head_dim) {
+        if (ctx->tmaps[i].base == base && ctx->tmaps[i].rows == rows && ctx->tmaps[i].head_dim == head_dim &&
+            ctx->tmaps[i].box_rows == box_rows) {
             *out = &ctx->tmaps[i].map;
             return SPARDA_OK;
         }
@@ -324,7 +327,7 @@ int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_d
                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
     cuuint64_t gdim[2] = {(cuuint64_t)head_dim, (cuuint64_t)rows};
     cuuint64_t gstride[1] = {(cuuint64_t)head_dim * 2};
-    cuuint32_t box[2] = {64, 64};
+    cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = ((encode_t)ctx->encode_fn)(&e->map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstride, box,
                                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -337,6 +340,7 @@ int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_d
     e->base = base;
     e->rows = rows;
     e->head_dim = head_dim;
+    e->box_rows = box_rows;
     *out = &e->map;
     return SPARDA_OK;
 }

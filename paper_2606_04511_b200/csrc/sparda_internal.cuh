@@ -15,6 +15,7 @@ struct sparda_tmap_entry {
     const void* base;
     uint64_t rows;
     int head_dim;
+    int box_rows;
     CUtensorMap map;
 };
 
@@ -29,6 +30,7 @@ struct sparda_ctx {
     float* part_ml;    // [R][max_splits][2][16]  (m in log2 domain, l)
     float* scores;     // [R][max_blocks] select scratch (orderable keys as uint32)
     unsigned int* tickets;  // [2][R]: [0] = select, [1] = attention
+    float* pf_scratch;      // prefill comparison selector: [sm_count][512][128] fp32 group-summed scores (lazy)
     cudaEvent_t* ev_sel;    // [max_layers + 1]
     cudaEvent_t* ev_gather; // [max_layers + 1]
     int max_layers;
@@ -69,7 +71,8 @@ int sparda_launch_prefill_select(sparda_ctx*, const void* F, const void* Kpool, 
                                  int n_rows, int topk, int32_t* ids, cudaStream_t);
 int sparda_launch_prefill_baseline(sparda_ctx*, const void* Q, const void* Kpool, int T, int n_blocks, int row0,
                                    int n_rows, int topk, int32_t* ids, cudaStream_t);
-int sparda_get_tmap(sparda_ctx*, const void* base, uint64_t rows, int head_dim, const CUtensorMap** out);
+// [rows][head_dim] bf16 row-major view, box = box_rows x 64 elements (128 B), 128-byte swizzle
+int sparda_get_tmap(sparda_ctx*, const void* base, uint64_t rows, int head_dim, int box_rows, const CUtensorMap** out);
 int sparda_resolve_splits(const sparda_ctx*, int topk);
 
 #ifdef __CUDACC__

@@ -296,7 +296,7 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     const int D = ctx->cfg.head_dim;
     const uint64_t rows = (uint64_t)ctx->R * n_slots * 2 * S_BLK;
     const CUtensorMap* map;
-    int rc = sparda_get_tmap(ctx, pool, rows, D, &map);
+    int rc = sparda_get_tmap(ctx, pool, rows, D, S_BLK, &map);
     if (rc) return rc;
     AttnParams p;
     p.Q = (const uint32_t*)Q;

@@ -312,3 +312,108 @@ def test_argument_validation(sp):
         ctx.forecast_select(0, t, 64, 8, ids)                        # null pointer
     with pytest.raises(sp.SpardaError):
         ctx.sparse_decode(t, t[4:], ids, 8, t)                       # pool not 16-byte aligned
+
+
+# ------------------------------------------------------------------------------------------------
+# a7 / a7': chunked-prefill selection (tcgen05 GEMM + causal per-row top-k) and the comparison selector
+# ------------------------------------------------------------------------------------------------
+def _prefill_setup(cfg, binding):
+    P = synth.prefill_inputs(cfg, device="cuda")
+    ctx = binding.Sparda(1, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, max(cfg.n_blocks, 1), cfg.topk)
+    kpool = torch.empty((cfg.n_kv_heads, cfg.n_blocks, cfg.head_dim), dtype=torch.bfloat16, device="cuda")
+    ctx.pool_keys(P["kv"], cfg.n_kv_heads, cfg.n_blocks, kpool)
+    torch.cuda.synchronize()
+    return P, ctx, kpool
+
+
+def _check_prefill_rows(gids, want, scores, row0, S=64):
+    """gids / want [Hkv][n][k], scores [Hkv][n][Nb]; causal candidate count per row = (i+1)//S."""
+    Hkv, n, k = want.shape
+    band = 0
+    for g in range(Hkv):
+        ncand = np.minimum(scores.shape[2], (row0 + np.arange(n) + 1) // S)
+        band += parity.check_ids(gids[g], want[g], scores[g], ncand)
+    return band
+
+
+PF_SMALL = synth.PrefillConfig("pf_small", n_q_heads=8, n_kv_heads=2, head_dim=128, seq_len=2048 + 640, topk=8, seed=51)
+PF_D64 = synth.PrefillConfig("pf_d64", n_q_heads=4, n_kv_heads=1, head_dim=64, seq_len=3000, topk=12, seed=52, bias_std=2.0)
+PF_MID = synth.PrefillConfig("pf_mid", n_q_heads=32, n_kv_heads=2, head_dim=128, seq_len=16384 + 200, topk=64, seed=53)
+
+
+@pytest.mark.parametrize("cfg", [PF_SMALL, PF_D64, PF_MID], ids=lambda c: c.name)
+def test_prefill_select(cfg, sp, oracle):
+    P, ctx, kpool = _prefill_setup(cfg, sp)
+    T, k, Hkv = cfg.seq_len, cfg.topk, cfg.n_kv_heads
+    kp_bits, F_bits = _bits(kpool), _bits(P["F"])
+    # whole sequence in the config's chunks, plus a ragged chunk that is not tile-aligned
+    chunks = [(r0, min(cfg.chunk, T - r0)) for r0 in range(0, T, cfg.chunk)] + [(777, 1333)]
+    if cfg is PF_MID:                                             # bound the oracle's work: sampled windows
+        chunks = [(0, 300), (4000, 200), (8191, 130), (T - 257, 257)]
+    for row0, n in chunks:
+        ids = torch.full((Hkv, n, k), -7, dtype=torch.int32, device="cuda")
+        ctx.prefill_select(P["F"], kpool, T, cfg.n_blocks, row0, n, k, ids)
+        torch.cuda.synchronize()
+        want, s = oracle.prefill_select(F_bits, kp_bits, k, row0, n, want_scores=True)
+        _check_prefill_rows(ids.cpu().numpy(), want, s, row0)
+
+
+def test_prefill_select_ties_take_lowest_ids(sp, oracle):
+    """Rows with all-equal scores (F = 0), duplicated pooled keys and +-0 must resolve exactly like the oracle."""
+    cfg = synth.PrefillConfig("pf_ties", n_q_heads=4, n_kv_heads=2, head_dim=128, seq_len=4096, topk=16, seed=54)
+    P, ctx, kpool = _prefill_setup(cfg, sp)
+    F = P["F"].clone()
+    F[0, 1500:1700] = 0                                           # all scores 0 -> ids 0..k-1
+    F[1, 3000:3100, 1:] = 0                                       # scores = F[.,0] * Kpool[j,0]
+    kp = kpool.clone()
+    kp[0, 40:50] = kp[0, 10:20]                                   # duplicated blocks -> exact ties, lower id first
+    kp[1, :, 0] = torch.arange(cfg.n_blocks, device="cuda").to(torch.bfloat16) % 7   # few distinct values: heavy ties
+    ids = torch.empty((2, cfg.seq_len, cfg.topk), dtype=torch.int32, device="cuda")
+    ctx.prefill_select(F, kp, cfg.seq_len, cfg.n_blocks, 0, cfg.seq_len, cfg.topk, ids)
+    torch.cuda.synchronize()
+    want, s = oracle.prefill_select(_bits(F), _bits(kp), cfg.topk, want_scores=True)
+    got = ids.cpu().numpy()
+    np.testing.assert_array_equal(got[0, 1500:1700], want[0, 1500:1700])
+    np.testing.assert_array_equal(got[1, 3000:3100], want[1, 3000:3100])
+    assert np.all(got[0, 1600, :] == np.arange(cfg.topk))
+    _check_prefill_rows(got, want, s, 0)
+
+
+@pytest.mark.parametrize("cfg", [PF_SMALL, PF_D64], ids=lambda c: c.name)
+def test_prefill_select_baseline(cfg, sp, oracle):
+    P, ctx, kpool = _prefill_setup(cfg, sp)
+    T, k, Hkv = cfg.seq_len, cfg.topk, cfg.n_kv_heads
+    for row0, n in [(0, T), (900, 700)]:
+        ids = torch.full((Hkv, n, k), -7, dtype=torch.int32, device="cuda")
+        ctx.prefill_select_baseline(P["Q"], kpool, T, cfg.n_blocks, row0, n, k, ids)
+        torch.cuda.synchronize()
+        want, s = oracle.prefill_select_baseline(_bits(P["Q"]), _bits(kpool), k, row0, n, want_scores=True)
+        _check_prefill_rows(ids.cpu().numpy(), want, s, row0)
+
+
+def test_cfg5_full_size_prefill_sampled(sp, oracle):
+    """BASELINE.json configs[4] at full size (T = 32768, 512 blocks, top-64, 2 groups) in 2048-row chunks as bench.py
+    launches it; the oracle checks sampled row windows (it needs ~1 s per 100 rows at this size)."""
+    cfg = synth.CFG5_PREFILL
+    P, ctx, kpool = _prefill_setup(cfg, sp)
+    T, k, Hkv = cfg.seq_len, cfg.topk, cfg.n_kv_heads
+    ids = torch.full((Hkv, T, k), -7, dtype=torch.int32, device="cuda")
+    # one call per chunk writes [Hkv][chunk][k]; assemble
+    for r0 in range(0, T, cfg.chunk):
+        part = torch.empty((Hkv, cfg.chunk, k), dtype=torch.int32, device="cuda")
+        ctx.prefill_select(P["F"], kpool, T, cfg.n_blocks, r0, cfg.chunk, k, part)
+        ids[:, r0:r0 + cfg.chunk] = part
+    torch.cuda.synchronize()
+    got = ids.cpu().numpy()
+    kp_bits, F_bits = _bits(kpool), _bits(P["F"])
+    band = 0
+    for row0, n in [(0, 130), (4090, 70), (16383, 66), (T - 100, 100)]:
+        want, s = oracle.prefill_select(F_bits, kp_bits, k, row0, n, want_scores=True)
+        band += _check_prefill_rows(got[:, row0:row0 + n], want, s, row0)
+    # properties that hold at any size: ascending, in the causal range, full count
+    valid = got >= 0
+    ncand = np.minimum(cfg.n_blocks, (np.arange(T) + 1) // 64)
+    assert np.array_equal(valid.sum(-1), np.broadcast_to(np.minimum(ncand, k), (Hkv, T)))
+    assert np.all(np.where(valid, got, -1).max(-1) < np.maximum(ncand, 1)[None, :])
+    d = np.diff(np.where(valid, got, np.iinfo(np.int32).max).astype(np.int64), axis=-1)
+    assert np.all(d[valid[..., 1:]] > 0)

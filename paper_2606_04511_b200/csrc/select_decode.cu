@@ -39,35 +39,114 @@ __device__ __forceinline__ uint32_t block_incl_scan_256(uint32_t v, uint32_t* wa
     return v + add;
 }
 
+__device__ __forceinline__ float key_to_float(uint32_t key) {
+    return __uint_as_float(key ^ ((key >> 31) ? 0x80000000u : 0xFFFFFFFFu));
+}
+
+constexpr int SEL_CAND_CAP = 32;  // boundary-bucket size the one-warp exact finish handles
+
 // Exact top-k over keys[0..n) (order-preserving uint32 keys in shared memory), n > k.  Whole CTA (256 threads).
-__device__ void radix_topk_emit(const uint32_t* keys, int n, int k, int32_t* ids_out, uint32_t* hist /*[256]*/,
-                                uint32_t* warp_tot /*[8]*/, uint32_t* bcast /*[2]*/) {
+//
+// Fast path (one histogram pass): 256 equal-width value buckets over the row's [min, max]; the bucket map
+// is monotone (subtract, multiply by a positive constant and truncate are all monotone under IEEE
+// rounding), so every key in a higher bucket is larger than every key in a lower one and equal keys share
+// a bucket.  A suffix scan finds the boundary bucket b* holding the k-th largest; its (<= 32, typically
+// ~4) members are ranked exactly by (key desc, id asc) in one warp, which yields the k-th largest key T
+// and how many keys == T are taken (the lowest ids).  Unlike a radix pass over the top byte of the key
+// (sign + 7 exponent bits: a handful of bins for Gaussian logits) the shared-memory atomics are spread.
+// Fallback (heavy ties / degenerate range): exact MSB-first 8-bit radix select.
+// Emission: index-ordered compaction of {key > T} plus the first krem keys == T, which is exactly
+// "sort by (score desc, id asc), take k, sort by id".
+__device__ void topk_emit(const uint32_t* keys, int n, int k, uint32_t kmin, uint32_t kmax, int32_t* ids_out,
+                          uint32_t* hist /*[256]*/, uint32_t* warp_tot /*[8]*/, uint32_t* bcast /*[4]*/,
+                          uint32_t* cand /*[2 * SEL_CAND_CAP]*/) {
     const int tid = threadIdx.x;
-    uint32_t prefix = 0, mask = 0, krem = (uint32_t)k;
-#pragma unroll 1
-    for (int shift = 24; shift >= 0; shift -= 8) {
+    uint32_t T = 0, krem = 0;
+    // ---- fast path
+    const float flo = key_to_float(kmin), fhi = key_to_float(kmax);
+    const float scale = 256.0f / (fhi - flo);
+    bool fast = (kmax > kmin) && (scale > 0.f) && (scale < INFINITY);
+    auto bucket = [&](uint32_t key) -> int {
+        return (int)fminf((key_to_float(key) - flo) * scale, 255.0f);
+    };
+    if (fast) {
         hist[tid] = 0;
+        if (tid == 0) bcast[2] = 0;
         __syncthreads();
-        for (int i = tid; i < n; i += SEL_THREADS) {
-            uint32_t key = keys[i];
-            if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1u);
-        }
+        for (int i = tid; i < n; i += SEL_THREADS) atomicAdd(&hist[bucket(keys[i])], 1u);
         __syncthreads();
-        // suffix sums over bins: thread t owns bin b = 255 - t, inclusive scan gives #keys with digit >= b
+        // suffix sums: thread t owns bucket b = 255 - t; inclusive scan gives #keys with bucket >= b
         uint32_t mine = hist[255 - tid], tot;
         uint32_t ge = block_incl_scan_256(mine, warp_tot, tot);
         uint32_t gt = ge - mine;
-        if (gt < krem && krem <= ge) {
-            bcast[0] = prefix | ((uint32_t)(255 - tid) << shift);
-            bcast[1] = krem - gt;
+        if (gt < (uint32_t)k && (uint32_t)k <= ge) {
+            bcast[0] = 255 - tid;       // boundary bucket
+            bcast[1] = k - gt;          // how many of its members are selected (>= 1)
+            bcast[3] = mine;            // its population
         }
         __syncthreads();
-        prefix = bcast[0];
-        krem = bcast[1];
-        mask |= 0xFFu << shift;
+        const int bstar = (int)bcast[0];
+        const uint32_t need = bcast[1], pop = bcast[3];
+        if (pop <= SEL_CAND_CAP) {
+            for (int i = tid; i < n; i += SEL_THREADS) {
+                uint32_t key = keys[i];
+                if (bucket(key) == bstar) {
+                    uint32_t s = atomicAdd(&bcast[2], 1u);
+                    cand[2 * s] = key;
+                    cand[2 * s + 1] = (uint32_t)i;
+                }
+            }
+            __syncthreads();
+            if (tid < 32) {
+                const bool have = (uint32_t)tid < pop;
+                const uint32_t mk = have ? cand[2 * tid] : 0u, mi = have ? cand[2 * tid + 1] : 0xFFFFFFFFu;
+                uint32_t rank = 0;
+                for (uint32_t f = 0; f < pop; ++f) {
+                    const uint32_t fk = cand[2 * f], fi = cand[2 * f + 1];
+                    rank += (fk > mk || (fk == mk && fi < mi)) ? 1u : 0u;
+                }
+                const bool is_kth = have && rank == need - 1;
+                const uint32_t who = __ballot_sync(0xffffffffu, is_kth);   // exactly one lane
+                const int src = __ffs(who) - 1;
+                const uint32_t Tk = __shfl_sync(0xffffffffu, mk, src), Ti = __shfl_sync(0xffffffffu, mi, src);
+                const uint32_t eq_taken = __popc(__ballot_sync(0xffffffffu, have && mk == Tk && mi <= Ti));
+                if (tid == 0) { bcast[0] = Tk; bcast[1] = eq_taken; }
+            }
+            __syncthreads();
+            T = bcast[0];
+            krem = bcast[1];
+        } else {
+            fast = false;   // uniform across the CTA (pop is broadcast)
+        }
         __syncthreads();
     }
-    const uint32_t T = prefix;  // k-th largest key; take every key > T and the first `krem` keys == T
+    if (!fast) {
+        uint32_t prefix = 0, mask = 0;
+        krem = (uint32_t)k;
+#pragma unroll 1
+        for (int shift = 24; shift >= 0; shift -= 8) {
+            hist[tid] = 0;
+            __syncthreads();
+            for (int i = tid; i < n; i += SEL_THREADS) {
+                uint32_t key = keys[i];
+                if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1u);
+            }
+            __syncthreads();
+            uint32_t mine = hist[255 - tid], tot;
+            uint32_t ge = block_incl_scan_256(mine, warp_tot, tot);
+            uint32_t gt = ge - mine;
+            if (gt < krem && krem <= ge) {
+                bcast[0] = prefix | ((uint32_t)(255 - tid) << shift);
+                bcast[1] = krem - gt;
+            }
+            __syncthreads();
+            prefix = bcast[0];
+            krem = bcast[1];
+            mask |= 0xFFu << shift;
+            __syncthreads();
+        }
+        T = prefix;  // k-th largest key; take every key > T and the first `krem` keys == T
+    }
     const int per = (n + SEL_THREADS - 1) / SEL_THREADS;
     const int lo = min(tid * per, n), hi = min(lo + per, n);
     uint32_t c = 0;  // low 16 bits: #gt, high 16 bits: #eq  (n <= 8192)
@@ -104,7 +183,9 @@ __global__ void __launch_bounds__(SEL_THREADS) forecast_select_kernel(const uint
     extern __shared__ uint32_t s_keys[];  // [n_cand] (only the selecting CTA uses it)
     __shared__ uint32_t s_hist[256];
     __shared__ uint32_t s_wtot[8];
-    __shared__ uint32_t s_bcast[2];
+    __shared__ uint32_t s_bcast[4];
+    __shared__ uint32_t s_cand[2 * SEL_CAND_CAP];
+    __shared__ uint32_t s_mm[2][SEL_THREADS / 32];
     __shared__ unsigned int s_ticket;
 
     const int r = blockIdx.y;
@@ -155,10 +236,21 @@ __global__ void __launch_bounds__(SEL_THREADS) forecast_select_kernel(const uint
     if (s_ticket != gridDim.x - 1) return;
     __threadfence();
     if (tid == 0) tickets[r] = 0;  // re-arm for the next launch
-    for (int i = tid; i < n_cand; i += SEL_THREADS) s_keys[i] = __ldcg(score_keys + (size_t)r * key_stride + i);
+    uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+    for (int i = tid; i < n_cand; i += SEL_THREADS) {
+        const uint32_t key = __ldcg(score_keys + (size_t)r * key_stride + i);
+        s_keys[i] = key;
+        kmin = min(kmin, key);
+        kmax = max(kmax, key);
+    }
+    kmin = __reduce_min_sync(0xffffffffu, kmin);
+    kmax = __reduce_max_sync(0xffffffffu, kmax);
+    if (lane == 0) { s_mm[0][w] = kmin; s_mm[1][w] = kmax; }
     __syncthreads();
+#pragma unroll
+    for (int i = 0; i < SEL_THREADS / 32; ++i) { kmin = min(kmin, s_mm[0][i]); kmax = max(kmax, s_mm[1][i]); }
     // ---- a2: exact top-k, ascending ids
-    radix_topk_emit(s_keys, n_cand, topk, ids_row, s_hist, s_wtot, s_bcast);
+    topk_emit(s_keys, n_cand, topk, kmin, kmax, ids_row, s_hist, s_wtot, s_bcast, s_cand);
 }
 
 // a0: Kpool[r,j,d] = bf16( (1/S) sum_t K[r,j,t,d] ), fp32 sum in ascending t (Eq.2, kernel = stride = S).

@@ -13,20 +13,6 @@ int sparda_set_cuda_error(sparda_ctx* ctx, cudaError_t e, const char* where) {
     return SPARDA_ECUDA;
 }
 
-int sparda_resolve_splits(const sparda_ctx* ctx, int topk) {
-    int s = ctx->cfg.attn_splits;
-    if (s <= 0) {
-        // enough CTAs for ~2 per SM, at least one block per consumer warp where possible
-        int want = (2 * ctx->sm_count + ctx->R - 1) / ctx->R;
-        int cap = (topk + SPARDA_ATTN_WARPS - 1) / SPARDA_ATTN_WARPS;
-        s = want < cap ? want : cap;
-        if (s < 1) s = 1;
-    }
-    if (s > topk) s = topk;
-    if (s > ctx->max_splits) s = ctx->max_splits;
-    return s;
-}
-
 extern "C" {
 
 const char* sparda_version(void) { return "libsparda 0.1 (sm_100a)"; }
@@ -76,7 +62,11 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     ctx->G = G;
     if (ctx->cfg.gather_ctas == 0) ctx->cfg.gather_ctas = cfg->gather_mode == SPARDA_GATHER_TMA ? 4 : 16;
     ctx->max_layers = cfg->max_layers > 0 ? cfg->max_layers : 64;
-    ctx->max_splits = cfg->topk < 64 ? cfg->topk : 64;
+    {   // partial slots per row of the flat split-K attention: n_parts <= ceil(CTAs / R) + 1
+        int per_row = cfg->attn_splits > 0 ? cfg->attn_splits : (2 * ctx->sm_count + ctx->R - 1) / ctx->R;
+        if (per_row > cfg->topk) per_row = cfg->topk;
+        ctx->max_splits = per_row + 2;
+    }
 
     cudaError_t e;
     void* fn = nullptr;

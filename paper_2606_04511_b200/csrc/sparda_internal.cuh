@@ -9,7 +9,6 @@
 
 #define SPARDA_MAX_TMAP_CACHE 16
 #define SPARDA_MAX_G 16        // query heads per group, padded to the M=16 of mma.m16n8k16
-#define SPARDA_ATTN_WARPS 4    // consumer warps (= smem stages) of the sparse-decode CTA
 
 struct sparda_tmap_entry {
     const void* base;
@@ -73,7 +72,8 @@ int sparda_launch_prefill_baseline(sparda_ctx*, const void* Q, const void* Kpool
                                    int n_rows, int topk, int32_t* ids, cudaStream_t);
 // [rows][head_dim] bf16 row-major view, box = box_rows x 64 elements (128 B), 128-byte swizzle
 int sparda_get_tmap(sparda_ctx*, const void* base, uint64_t rows, int head_dim, int box_rows, const CUtensorMap** out);
-int sparda_resolve_splits(const sparda_ctx*, int topk);
+int sparda_resolve_splits(const sparda_ctx*, int topk);     // average CTAs per row of the attention launch
+int sparda_resolve_attn_ctas(const sparda_ctx*, int topk);  // its grid size
 
 #ifdef __CUDACC__
 // ------------------------------------------------------------------------------------------------
@@ -92,6 +92,7 @@ __device__ __forceinline__ void mbar_fence_init() {
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }

@@ -2,294 +2,476 @@
 // addressed by block id (a6, layer 0).  Eq.5, Alg.2 l.7:
 //   O_h = softmax_t( q_h . k_t / sqrt(D) ) V   over every token t of every selected block of row r = b*Hkv + h/G.
 //
-// Split-K flash-decode.  Grid (splits, R); a CTA owns a contiguous range of pool slots of one row and has
-// SPARDA_ATTN_WARPS consumer warps, each with its own shared-memory stage (one block's K and V tiles,
-// 2*S*D*2 bytes).  Lane 0 of a warp stages the warp's next block with TMA tensor-map loads
-// (cp.async.bulk.tensor.2d, 64x64 boxes, 128-byte swizzle so ldmatrix is bank-conflict free) completing
-// on per-stage mbarriers (K and V separately: QK^T starts when K lands, and the next K load is issued
-// as soon as QK^T has consumed the tile).  The group's G <= 16 query heads are the M = 16 rows of
-// mma.sync.m16n8k16 (bf16 in, fp32 accumulate): S = Q K^T (16 x 64 per block), online softmax in the
-// exp2 domain, O += P V.  Warp partials (m, l, O) are merged through shared memory, CTA partials through
-// an L2-resident workspace by the last CTA of the row (ticket), which rounds once to bf16.
+// Flat split-K flash-decode.  The R*k pool slots of the launch form one flat work list that is cut into
+// gridDim.x equal contiguous ranges (grid = a multiple of the SM count, so there is no wave-quantisation tail);
+// a CTA walks its range row segment by row segment.  NW consumer warps per CTA, each with its own
+// shared-memory stage (one block's K and V tiles, 2*S*D*2 bytes).  Lane 0 of a warp stages the warp's next block
+// with TMA tensor-map loads (cp.async.bulk.tensor.2d, 64x64 boxes, 128-byte swizzle so ldmatrix is bank-conflict
+// free) completing on per-stage mbarriers (K and V separately: QK^T starts when K lands, and the next K load is
+// issued as soon as QK^T has consumed the tile).  The group's G <= 16 query heads are the M = 16 rows of
+// mma.sync.m16n8k16 (bf16 in, fp32 accumulate): S = Q K^T (16 x 64 per block), online softmax in the exp2
+// domain, O += P V.  Warp partials (m, l, O) are merged through shared memory, the CTA partials of one row
+// through an L2-resident workspace by the last CTA to finish that row (ticket), which rounds once to bf16.
 // HBM-bound by design: 16 FLOP per KV byte at G = 16; the tensor pipe idles most of the time.
 #include "sparda_internal.cuh"
+
+#ifdef SPARDA_TRACE
+__device__ unsigned long long* g_trace;   // [gridDim.x][8] globaltimer stamps (debug builds only)
+extern "C" void sparda_debug_set_trace(unsigned long long* p) { cudaMemcpyToSymbol(g_trace, &p, sizeof(p)); }
+#define TRACE(i)                                                                              \
+    if (threadIdx.x == 0) {                                                                   \
+        unsigned long long t__;                                                               \
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));                               \
+        g_trace[blockIdx.x * 8 + (i)] = t__;                                                  \
+    }
+#else
+#define TRACE(i)
+#endif
 
 namespace {
 
 using namespace sparda;
 
-constexpr int NW = SPARDA_ATTN_WARPS;
-constexpr int ATT_THREADS = NW * 32;
 constexpr int S_BLK = 64;
 
-template <int D>
+template <int D, int NW>
 struct AttnSmem {
     static constexpr int TILE_BYTES = S_BLK * D * 2;        // one K (or V) tile
     static constexpr int STAGE_BYTES = 2 * TILE_BYTES;      // K then V
-    static constexpr int OROW = D + 4;                      // padded fp32 row of the warp partial
-    static constexpr int TOTAL = NW * STAGE_BYTES + 1024;   // + slack for 1024-byte alignment
-    static_assert(16 * OROW * 4 <= STAGE_BYTES, "warp partial must fit in the warp's own stage");
+    static constexpr int OROW = D + 4;                      // padded fp32 row of a warp partial
+    static constexpr int XCHG_WARP = 16 * OROW * 4;         // one warp's partial O (16 heads x D fp32)
+    static constexpr int OFF_XCHG = NW * STAGE_BYTES;       // exchange area: separate from the stages, so the next
+                                                            // segment's tiles can be in flight during a merge
+    static constexpr int TOTAL = OFF_XCHG + 2 * NW * XCHG_WARP + 1024;   // two exchange buffers + alignment slack
 };
 
 struct AttnParams {
     const uint32_t* Q;     // bf16 pairs
     const int32_t* ids;
     __nv_bfloat16* O;
-    float* part_O;
-    float* part_ml;
-    unsigned int* tickets;
-    int topk, indexed, n_slots, Hq, Hkv, G, splits, max_splits;
+    float* part_O;         // [R][max_splits][16][D]
+    float* part_ml;        // [R][max_splits][2][16]
+    unsigned int* tickets; // [R]
+    int topk, indexed, n_slots, Hq, Hkv, G, max_splits;
+    int W;                 // R * topk flat slots (< 2^31)
+    int quota, rem;        // W = gridDim.x * quota + rem: CTA c owns quota + (c < rem) slots from c * quota + min(c, rem)
     float scale_log2;
 };
 
-// merge n partials {m[i], l[i], o[i]} -> (M, L, acc); weights exp2(m_i - M)
-template <int D>
-__global__ void __launch_bounds__(ATT_THREADS, 1) sparse_decode_kernel(const __grid_constant__ CUtensorMap tmap, AttnParams p) {
-    using SM = AttnSmem<D>;
+// owner(f): the CTA whose flat range holds slot f (inverse of the map in AttnParams)
+__device__ __forceinline__ int flat_owner(int f, int quota, int rem) {
+    const int thr = rem * (quota + 1);
+    return f < thr ? f / (quota + 1) : rem + (f - thr) / quota;
+}
+
+template <int D, int NW, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __grid_constant__ CUtensorMap tmap, AttnParams p) {
+    using SM = AttnSmem<D, NW>;
+    constexpr int NT = NW * 32;
     constexpr int KSTEPS = D / 16;  // k-steps of Q K^T
     constexpr int DT = D / 8;       // n-tiles of P V
     constexpr int HALVES = D / 64;  // 64-element TMA boxes per row
     extern __shared__ uint8_t smem_raw[];
     __shared__ uint64_t bar_k[NW], bar_v[NW];
-    __shared__ float s_ml[NW][2][16];
-    __shared__ unsigned int s_ticket;
+    __shared__ float s_ml[1][NW][2][16];
+    __shared__ unsigned int s_last;
+    __shared__ uint64_t bar_m;
+    __shared__ __align__(128) float s_pm[16 * 32];
+    __shared__ float s_w[16 * 16], s_run[16], s_resc[16], s_newmax[16];
 
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int r = blockIdx.y, split = blockIdx.x;
-    const int b = r / p.Hkv, g = r % p.Hkv;
     const int gid = lane >> 2, tig = lane & 3;
 
+    TRACE(0);
     if (tid == 0) {
         for (int i = 0; i < NW; ++i) { mbar_init(&bar_k[i], 1); mbar_init(&bar_v[i], 1); }
+        mbar_init(&bar_m, 1);
         mbar_fence_init();
         fence_proxy_async_smem();
         tma_prefetch_desc(&tmap);
     }
     __syncthreads();
 
-    const int bps = (p.topk + p.splits - 1) / p.splits;
-    const int slot_begin = split * bps;
-    const int slot_end = min(p.topk, slot_begin + bps);
-    const int32_t* ids_row = p.ids + (size_t)r * p.topk;
-
     uint8_t* stage = smem + (size_t)w * SM::STAGE_BYTES;
     const uint32_t k_base = smem_u32(stage), v_base = k_base + SM::TILE_BYTES;
-
-    auto next_valid = [&](int s) {
-        while (s < slot_end && __ldg(ids_row + s) < 0) s += NW;
-        return s;
-    };
-    auto tile_row = [&](int slot, int plane) -> int {
-        int idx = p.indexed ? __ldg(ids_row + slot) : slot;
-        return (((r * p.n_slots + idx) * 2 + plane) * S_BLK);
-    };
-    auto issue_k = [&](int slot) {
-        mbar_arrive_expect_tx(&bar_k[w], SM::TILE_BYTES);
-#pragma unroll
-        for (int h = 0; h < HALVES; ++h) tma_load_2d(stage + h * 8192, &tmap, h * 64, tile_row(slot, 0), &bar_k[w]);
-    };
-    auto issue_v = [&](int slot) {
-        mbar_arrive_expect_tx(&bar_v[w], SM::TILE_BYTES);
-#pragma unroll
-        for (int h = 0; h < HALVES; ++h)
-            tma_load_2d(stage + SM::TILE_BYTES + h * 8192, &tmap, h * 64, tile_row(slot, 1), &bar_v[w]);
-    };
-
-    int cur = next_valid(slot_begin + w);
-    if (lane == 0 && cur < slot_end) { issue_k(cur); issue_v(cur); }
-
-    // Q fragments (A operand, 16 heads x D): rows gid and gid+8, zero beyond G
-    uint32_t qa[KSTEPS][4];
-    {
-        const uint32_t* q0 = p.Q + ((size_t)(b * p.Hq + g * p.G + gid) * D) / 2;
-        const uint32_t* q1 = q0 + (size_t)8 * D / 2;
-        const bool v0 = gid < p.G, v1 = gid + 8 < p.G;
-#pragma unroll
-        for (int ks = 0; ks < KSTEPS; ++ks) {
-            int c = ks * 8 + tig;  // uint32 index of columns ks*16 + tig*2
-            qa[ks][0] = v0 ? __ldg(q0 + c) : 0u;
-            qa[ks][1] = v1 ? __ldg(q1 + c) : 0u;
-            qa[ks][2] = v0 ? __ldg(q0 + c + 4) : 0u;
-            qa[ks][3] = v1 ? __ldg(q1 + c + 4) : 0u;
-        }
-    }
-
-    float o[DT][4];
-#pragma unroll
-    for (int i = 0; i < DT; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
-    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
     uint32_t phase = 0;
-
     // per-lane ldmatrix row offsets (swizzle: 16-byte chunk index ^= row & 7; rows are 128 B inside a box)
     const int mi = lane >> 3, ri = lane & 7;
 
-    while (cur < slot_end) {
-        const int nxt = next_valid(cur + NW);
-        // ---- S = Q K^T
-        mbar_wait(&bar_k[w], phase);
-        float s[8][4];
+    const int f_begin = (int)blockIdx.x * p.quota + min((int)blockIdx.x, p.rem);
+    const int f_end = f_begin + p.quota + ((int)blockIdx.x < p.rem ? 1 : 0);
+    struct Seg { int r, s0, s1; };
+    auto seg_at = [&](int f) -> Seg {   // the row segment that starts at flat slot f
+        Seg t;
+        t.r = f / p.topk;
+        t.s0 = f - t.r * p.topk;
+        t.s1 = min(p.topk, t.s0 + (f_end - f));
+        return t;
+    };
+    // this warp's first item at or after flat position f: slot s0 + w of the first segment long enough to have one
+    auto first_item = [&](int f, int& r_out, int& s_out) -> bool {
+        while (f < f_end) {
+            const Seg t = seg_at(f);
+            if (t.s0 + w < t.s1) { r_out = t.r; s_out = t.s0 + w; return true; }
+            f += t.s1 - t.s0;
+        }
+        return false;
+    };
+    // Tiles are staged whether or not the slot is valid (id -1 = padding, rare: fewer candidates than k); an invalid
+    // slot is skipped after its tiles land.  This keeps the ids load off the path to the first TMA issue.
+    auto tile_row = [&](int r, int slot, int plane) -> int {
+        int idx = slot;
+        if (p.indexed) idx = max(__ldg(p.ids + (size_t)r * p.topk + slot), 0);
+        return (((r * p.n_slots + idx) * 2 + plane) * S_BLK);
+    };
+    auto issue_k = [&](int r, int slot) {
+        mbar_arrive_expect_tx(&bar_k[w], SM::TILE_BYTES);
 #pragma unroll
-        for (int nt = 0; nt < 8; ++nt) {
-            s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f;
-            const uint32_t row_addr = k_base + (nt * 8 + ri) * 128;
+        for (int h = 0; h < HALVES; ++h) tma_load_2d(stage + h * 8192, &tmap, h * 64, tile_row(r, slot, 0), &bar_k[w]);
+    };
+    auto issue_v = [&](int r, int slot) {
+        mbar_arrive_expect_tx(&bar_v[w], SM::TILE_BYTES);
 #pragma unroll
-            for (int kp = 0; kp < KSTEPS / 2; ++kp) {
-                const int c = kp * 4 + mi;  // 16-byte chunk of the D-row
-                uint32_t b0, b1, b2, b3;
-                ldmatrix_x4(row_addr + (c >> 3) * 8192 + (((c & 7) ^ ri) << 4), b0, b1, b2, b3);
-                mma_bf16_16816(s[nt], qa[2 * kp], b0, b1);
-                mma_bf16_16816(s[nt], qa[2 * kp + 1], b2, b3);
+        for (int h = 0; h < HALVES; ++h)
+            tma_load_2d(stage + SM::TILE_BYTES + h * 8192, &tmap, h * 64, tile_row(r, slot, 1), &bar_v[w]);
+    };
+
+    // ---- CTA merge of the warp partials in exchange buffer `buf` (all threads; a CTA barrier precedes it): a whole-row
+    // segment is normalised and stored, a partial-row segment goes to the row's slot `part` of the L2-resident workspace
+    constexpr int C4 = D / 4;
+    auto cta_merge = [&](int buf, int r, int part, int n_parts) {
+        const int b = r / p.Hkv, g = r % p.Hkv;
+        __nv_bfloat16* obase = p.O + (size_t)(b * p.Hq + g * p.G) * D;
+        float* po = p.part_O + ((size_t)r * p.max_splits + part) * 16 * D;
+        float* pml = p.part_ml + ((size_t)r * p.max_splits + part) * 32;
+        for (int it = tid; it < 16 * C4; it += NT) {   // items = (head row, float4 column); rows >= G carry zeros
+            const int row = it / C4, c4 = it % C4;
+            float M = -INFINITY;
+#pragma unroll
+            for (int i = 0; i < NW; ++i) M = fmaxf(M, s_ml[buf][i][0][row]);
+            float L = 0.f;
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < NW; ++i) {
+                const float wg = (M == -INFINITY) ? 0.f : exp2f(s_ml[buf][i][0][row] - M);
+                L += wg * s_ml[buf][i][1][row];
+                const float4 v = *reinterpret_cast<const float4*>(
+                    reinterpret_cast<const float*>(smem + SM::OFF_XCHG + (size_t)(buf * NW + i) * SM::XCHG_WARP) + row * SM::OROW + c4 * 4);
+                acc.x += wg * v.x; acc.y += wg * v.y; acc.z += wg * v.z; acc.w += wg * v.w;
             }
-        }
-        __syncwarp();
-        if (lane == 0 && nxt < slot_end) { fence_proxy_async_smem(); issue_k(nxt); }
-
-        // ---- online softmax (exp2 domain), P rounded to bf16 feeds both the row sum and P V
-        float mx0 = s[0][0], mx1 = s[0][2];
-#pragma unroll
-        for (int nt = 0; nt < 8; ++nt) {
-            mx0 = fmaxf(mx0, fmaxf(s[nt][0], s[nt][1]));
-            mx1 = fmaxf(mx1, fmaxf(s[nt][2], s[nt][3]));
-        }
-        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
-        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
-        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
-        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
-        const float mn0 = fmaxf(m0, mx0 * p.scale_log2), mn1 = fmaxf(m1, mx1 * p.scale_log2);
-        const float al0 = exp2f(m0 - mn0), al1 = exp2f(m1 - mn1);
-        m0 = mn0; m1 = mn1;
-        uint32_t pa[4][4];
-        float rs0 = 0.f, rs1 = 0.f;
-#pragma unroll
-        for (int nt = 0; nt < 8; ++nt) {
-            uint32_t u0 = pack_bf16(exp2f(fmaf(s[nt][0], p.scale_log2, -mn0)), exp2f(fmaf(s[nt][1], p.scale_log2, -mn0)));
-            uint32_t u1 = pack_bf16(exp2f(fmaf(s[nt][2], p.scale_log2, -mn1)), exp2f(fmaf(s[nt][3], p.scale_log2, -mn1)));
-            rs0 += bf16_lo(u0) + bf16_hi(u0);
-            rs1 += bf16_lo(u1) + bf16_hi(u1);
-            pa[nt >> 1][(nt & 1) * 2 + 0] = u0;
-            pa[nt >> 1][(nt & 1) * 2 + 1] = u1;
-        }
-        l0 = l0 * al0 + rs0;
-        l1 = l1 * al1 + rs1;
-#pragma unroll
-        for (int i = 0; i < DT; ++i) { o[i][0] *= al0; o[i][1] *= al0; o[i][2] *= al1; o[i][3] *= al1; }
-
-        // ---- O += P V
-        mbar_wait(&bar_v[w], phase);
-#pragma unroll
-        for (int kt = 0; kt < 4; ++kt) {
-            const uint32_t row_addr = v_base + (kt * 16 + (mi & 1) * 8 + ri) * 128;
-#pragma unroll
-            for (int dp = 0; dp < DT / 2; ++dp) {
-                const int c = dp * 2 + (mi >> 1);
-                uint32_t b0, b1, b2, b3;
-                ldmatrix_x4_trans(row_addr + (c >> 3) * 8192 + (((c & 7) ^ ri) << 4), b0, b1, b2, b3);
-                mma_bf16_16816(o[2 * dp], pa[kt], b0, b1);
-                mma_bf16_16816(o[2 * dp + 1], pa[kt], b2, b3);
+            if (n_parts == 1) {
+                if (row < p.G) {
+                    const float inv = L > 0.f ? 1.f / L : 0.f;
+                    uint2 u;
+                    u.x = pack_bf16(acc.x * inv, acc.y * inv);
+                    u.y = pack_bf16(acc.z * inv, acc.w * inv);
+                    *reinterpret_cast<uint2*>(obase + (size_t)row * D + c4 * 4) = u;
+                }
+            } else {
+                __stcg(reinterpret_cast<float4*>(po + (size_t)row * D + c4 * 4), acc);
+                if (c4 == 0) { __stcg(pml + row, M); __stcg(pml + 16 + row, L); }
             }
-        }
-        __syncwarp();
-        if (lane == 0 && nxt < slot_end) { fence_proxy_async_smem(); issue_v(nxt); }
-        phase ^= 1;
-        cur = nxt;
-    }
-
-    // ---- warp partial -> this warp's own (now idle) stage
-    l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
-    l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
-    l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
-    l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
-    float* wo = reinterpret_cast<float*>(stage);
-#pragma unroll
-    for (int i = 0; i < DT; ++i) {
-        *reinterpret_cast<float2*>(wo + gid * SM::OROW + i * 8 + tig * 2) = make_float2(o[i][0], o[i][1]);
-        *reinterpret_cast<float2*>(wo + (gid + 8) * SM::OROW + i * 8 + tig * 2) = make_float2(o[i][2], o[i][3]);
-    }
-    if (tig == 0) {
-        s_ml[w][0][gid] = m0; s_ml[w][1][gid] = l0;
-        s_ml[w][0][gid + 8] = m1; s_ml[w][1][gid + 8] = l1;
-    }
-    __syncthreads();
-
-    // ---- CTA merge: thread -> (row, 4-column groups); 8 threads per row
-    const int row = tid >> 3, cg = tid & 7;
-    constexpr int NCG = D / 32;  // float4 groups per thread
-    float M = -INFINITY;
-#pragma unroll
-    for (int i = 0; i < NW; ++i) M = fmaxf(M, s_ml[i][0][row]);
-    float wgt[NW], L = 0.f;
-#pragma unroll
-    for (int i = 0; i < NW; ++i) {
-        wgt[i] = (M == -INFINITY) ? 0.f : exp2f(s_ml[i][0][row] - M);
-        L += wgt[i] * s_ml[i][1][row];
-    }
-    float4 acc[NCG];
-#pragma unroll
-    for (int j = 0; j < NCG; ++j) {
-        acc[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-        for (int i = 0; i < NW; ++i) {
-            const float4 v = *reinterpret_cast<const float4*>(reinterpret_cast<const float*>(smem + (size_t)i * SM::STAGE_BYTES) +
-                                                               row * SM::OROW + cg * 4 + j * 32);
-            acc[j].x += wgt[i] * v.x; acc[j].y += wgt[i] * v.y; acc[j].z += wgt[i] * v.z; acc[j].w += wgt[i] * v.w;
-        }
-    }
-    __nv_bfloat16* orow = p.O + (size_t)(b * p.Hq + g * p.G + row) * D;
-    auto store_out = [&](const float4 (&a)[NCG], float Lsum) {
-        const float inv = Lsum > 0.f ? 1.f / Lsum : 0.f;
-#pragma unroll
-        for (int j = 0; j < NCG; ++j) {
-            uint2 u;
-            u.x = pack_bf16(a[j].x * inv, a[j].y * inv);
-            u.y = pack_bf16(a[j].z * inv, a[j].w * inv);
-            *reinterpret_cast<uint2*>(orow + cg * 4 + j * 32) = u;
         }
     };
-    if (p.splits == 1) {
-        if (row < p.G) store_out(acc, L);
-        return;
-    }
-    if (row < p.G) {
-        float* po = p.part_O + ((size_t)(r * p.max_splits + split) * 16 + row) * D;
+    // ---- row merge by the CTA that finished row r last: the row's n_parts partials (contiguous in the workspace) are
+    // pulled into shared memory by bulk copies (TMA), mch at a time, and folded with a running (M, L, acc).  Landing area:
+    // the idle K/V stages (16 partials per chunk) after the CTA's last segment, the second exchange buffer (4 per chunk)
+    // for an earlier segment, whose successor's tiles are already in flight into the stages
+    constexpr int MCH_STAGES = NW * SM::STAGE_BYTES / (16 * D * 4) > 16 ? 16 : NW * SM::STAGE_BYTES / (16 * D * 4);
+    constexpr int MCH_XCHG = NW * SM::XCHG_WARP / (16 * D * 4);
+    uint32_t phase_m = 0;
+    auto row_merge = [&](int r, int n_parts, uint8_t* land_bytes, int mch) {
+        float* land = reinterpret_cast<float*>(land_bytes);
+        const int b = r / p.Hkv, g = r % p.Hkv;
+        __nv_bfloat16* obase = p.O + (size_t)(b * p.Hq + g * p.G) * D;
+        const float* rpo = p.part_O + (size_t)r * p.max_splits * 16 * D;
+        const float* rml = p.part_ml + (size_t)r * p.max_splits * 32;
+        constexpr int IPT = (16 * C4 + NT - 1) / NT;
+        float LL[IPT];
+        float4 acc[IPT];
 #pragma unroll
-        for (int j = 0; j < NCG; ++j) __stcg(reinterpret_cast<float4*>(po + cg * 4 + j * 32), acc[j]);
-        if (cg == 0) {
-            float* pml = p.part_ml + (size_t)(r * p.max_splits + split) * 32;
-            __stcg(pml + row, M);
-            __stcg(pml + 16 + row, L);
+        for (int j = 0; j < IPT; ++j) { LL[j] = 0.f; acc[j] = make_float4(0.f, 0.f, 0.f, 0.f); }
+        if (tid < 16) s_run[tid] = -INFINITY;   // running row max
+        __syncthreads();
+        for (int i0 = 0; i0 < n_parts; i0 += mch) {
+            const int n = min(mch, n_parts - i0);
+            if (tid == 0) {
+                fence_proxy_async_all();   // partials were written through the generic proxy (st.cg), read through the async proxy
+                mbar_arrive_expect_tx(&bar_m, (uint32_t)n * (16 * D * 4 + 128));
+                bulk_g2s(land, rpo + (size_t)i0 * 16 * D, (uint32_t)n * 16 * D * 4, &bar_m);
+                bulk_g2s(s_pm, rml + (size_t)i0 * 32, (uint32_t)n * 128, &bar_m);
+            }
+            mbar_wait(&bar_m, phase_m);
+            phase_m ^= 1;
+            TRACE(7);
+            // weights of the chunk, once per (partial, head row): s_w[i][row] = exp2(m_i - M_row), M_row the running max
+            for (int e = tid; e < n * 16; e += NT) {
+                const int row = e & 15;
+                float mm = s_run[row];
+                for (int i = 0; i < n; ++i) mm = fmaxf(mm, s_pm[i * 32 + row]);
+                s_w[e] = (mm == -INFINITY) ? 0.f : exp2f(s_pm[(e >> 4) * 32 + row] - mm);
+                if (e < 16) s_resc[row] = (mm == -INFINITY) ? 0.f : exp2f(s_run[row] - mm), s_newmax[row] = mm;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < IPT; ++j) {
+                const int it = tid + j * NT;
+                if (it >= 16 * C4) continue;
+                const int row = it / C4, c4 = it % C4;
+                const float resc = s_resc[row];
+                LL[j] *= resc;
+                acc[j].x *= resc; acc[j].y *= resc; acc[j].z *= resc; acc[j].w *= resc;
+                const float* src = land + row * D + c4 * 4;
+#pragma unroll 8
+                for (int i = 0; i < n; ++i) {
+                    const float wg = s_w[i * 16 + row];
+                    LL[j] += wg * s_pm[i * 32 + 16 + row];
+                    const float4 v = *reinterpret_cast<const float4*>(src + (size_t)i * 16 * D);
+                    acc[j].x += wg * v.x; acc[j].y += wg * v.y; acc[j].z += wg * v.z; acc[j].w += wg * v.w;
+                }
+            }
+            __syncthreads();
+            if (tid < 16) s_run[tid] = s_newmax[tid];
+            __syncthreads();   // the landing area may be overwritten by the next chunk
         }
-    }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) s_ticket = atomicAdd(&p.tickets[r], 1u);
-    __syncthreads();
-    if (s_ticket != (unsigned)p.splits - 1) return;
-    __threadfence();
-    if (tid == 0) p.tickets[r] = 0;  // re-arm
-    if (row >= p.G) return;
-    // ---- row merge over the split partials (L2-resident)
-    const float* pml = p.part_ml + (size_t)r * p.max_splits * 32;
-    float MM = -INFINITY;
-    for (int i = 0; i < p.splits; ++i) MM = fmaxf(MM, __ldcg(pml + i * 32 + row));
-    float LL = 0.f;
 #pragma unroll
-    for (int j = 0; j < NCG; ++j) acc[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int i = 0; i < p.splits; ++i) {
-        const float mi_ = __ldcg(pml + i * 32 + row);
-        const float wg = (MM == -INFINITY) ? 0.f : exp2f(mi_ - MM);
-        LL += wg * __ldcg(pml + i * 32 + 16 + row);
-        const float* po = p.part_O + ((size_t)(r * p.max_splits + i) * 16 + row) * D;
-#pragma unroll
-        for (int j = 0; j < NCG; ++j) {
-            const float4 v = __ldcg(reinterpret_cast<const float4*>(po + cg * 4 + j * 32));
-            acc[j].x += wg * v.x; acc[j].y += wg * v.y; acc[j].z += wg * v.z; acc[j].w += wg * v.w;
+        for (int j = 0; j < IPT; ++j) {
+            const int it = tid + j * NT;
+            if (it >= p.G * C4) continue;
+            const int row = it / C4, c4 = it % C4;
+            const float inv = LL[j] > 0.f ? 1.f / LL[j] : 0.f;
+            uint2 u;
+            u.x = pack_bf16(acc[j].x * inv, acc[j].y * inv);
+            u.y = pack_bf16(acc[j].z * inv, acc[j].w * inv);
+            *reinterpret_cast<uint2*>(obase + (size_t)row * D + c4 * 4) = u;
         }
+    };
+    // ---- publish this CTA's partial of row r and learn whether it finished the row last: CTA barrier, then one acq_rel
+    // ticket at gpu scope (the release is cumulative over the CTA's st.cg partial writes ordered before it by the barrier;
+    // the merging CTA acquires through the same atomic)
+    auto publish = [&](int r, int n_parts) -> bool {
+        __syncthreads();
+        if (tid == 0) {
+            unsigned int t;
+            fence_proxy_async_all();
+            asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(t) : "l"(p.tickets + r) : "memory");
+            const bool last = t == (unsigned)n_parts - 1;
+            if (last) p.tickets[r] = 0;   // re-arm
+            s_last = last ? 1u : 0u;
+        }
+        __syncthreads();
+        return s_last != 0;
+    };
+    int park_r = -1, park_part = 0, park_n = 1;
+
+    int cur_r = -1, cur_s = 0;
+    bool have = first_item(f_begin, cur_r, cur_s);
+    if (lane == 0 && have) { issue_k(cur_r, cur_s); issue_v(cur_r, cur_s); }
+    TRACE(1);
+
+    for (int f = f_begin; f < f_end;) {
+        const Seg sg = seg_at(f);
+        const int r = sg.r;
+        f += sg.s1 - sg.s0;
+        const int first_cta = flat_owner(r * p.topk, p.quota, p.rem);
+        const int n_parts = flat_owner((r + 1) * p.topk - 1, p.quota, p.rem) - first_cta + 1;
+        const int part = blockIdx.x - first_cta;
+        const int b = r / p.Hkv, g = r % p.Hkv;
+        const int32_t* ids_row = p.ids + (size_t)r * p.topk;
+
+        // Q fragments (A operand, 16 heads x D): rows gid and gid+8, zero beyond G
+        uint32_t qa[KSTEPS][4];
+        {
+            const uint32_t* q0 = p.Q + ((size_t)(b * p.Hq + g * p.G + gid) * D) / 2;
+            const uint32_t* q1 = q0 + (size_t)8 * D / 2;
+            const bool v0 = gid < p.G, v1 = gid + 8 < p.G;
+#pragma unroll
+            for (int ks = 0; ks < KSTEPS; ++ks) {
+                int c = ks * 8 + tig;  // uint32 index of columns ks*16 + tig*2
+                qa[ks][0] = v0 ? __ldg(q0 + c) : 0u;
+                qa[ks][1] = v1 ? __ldg(q1 + c) : 0u;
+                qa[ks][2] = v0 ? __ldg(q0 + c + 4) : 0u;
+                qa[ks][3] = v1 ? __ldg(q1 + c + 4) : 0u;
+            }
+        }
+
+        float o[DT][4];
+#pragma unroll
+        for (int i = 0; i < DT; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+        float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+        bool first__ = true;
+        (void)first__;
+
+        while (have && cur_r == r) {   // this warp's items of the segment (a CTA's range meets a row in one segment only)
+            // the item after this one: same segment, or the warp's first item of a later segment (staged across the merge)
+            int nxt_r = r, nxt_s = cur_s + NW;
+            bool have_n = true;
+            if (nxt_s >= sg.s1) have_n = first_item(f, nxt_r, nxt_s);
+            const bool valid = __ldg(ids_row + cur_s) >= 0;
+            // ---- S = Q K^T
+            mbar_wait(&bar_k[w], phase);
+            if (first__) { TRACE(2); first__ = false; }
+            float s[8][4];
+            if (valid) {
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f;
+                    const uint32_t row_addr = k_base + (nt * 8 + ri) * 128;
+#pragma unroll
+                    for (int kp = 0; kp < KSTEPS / 2; ++kp) {
+                        const int c = kp * 4 + mi;  // 16-byte chunk of the D-row
+                        uint32_t b0, b1, b2, b3;
+                        ldmatrix_x4(row_addr + (c >> 3) * 8192 + (((c & 7) ^ ri) << 4), b0, b1, b2, b3);
+                        mma_bf16_16816(s[nt], qa[2 * kp], b0, b1);
+                        mma_bf16_16816(s[nt], qa[2 * kp + 1], b2, b3);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0 && have_n) { fence_proxy_async_smem(); issue_k(nxt_r, nxt_s); }
+
+            uint32_t pa[4][4];
+            if (valid) {
+                // ---- online softmax (exp2 domain), P rounded to bf16 feeds both the row sum and P V
+                float mx0 = s[0][0], mx1 = s[0][2];
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    mx0 = fmaxf(mx0, fmaxf(s[nt][0], s[nt][1]));
+                    mx1 = fmaxf(mx1, fmaxf(s[nt][2], s[nt][3]));
+                }
+                mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+                mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+                mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+                mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+                const float mn0 = fmaxf(m0, mx0 * p.scale_log2), mn1 = fmaxf(m1, mx1 * p.scale_log2);
+                const float al0 = exp2f(m0 - mn0), al1 = exp2f(m1 - mn1);
+                m0 = mn0; m1 = mn1;
+                float rs0 = 0.f, rs1 = 0.f;
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    uint32_t u0 = pack_bf16(exp2f(fmaf(s[nt][0], p.scale_log2, -mn0)), exp2f(fmaf(s[nt][1], p.scale_log2, -mn0)));
+                    uint32_t u1 = pack_bf16(exp2f(fmaf(s[nt][2], p.scale_log2, -mn1)), exp2f(fmaf(s[nt][3], p.scale_log2, -mn1)));
+                    rs0 += bf16_lo(u0) + bf16_hi(u0);
+                    rs1 += bf16_lo(u1) + bf16_hi(u1);
+                    pa[nt >> 1][(nt & 1) * 2 + 0] = u0;
+                    pa[nt >> 1][(nt & 1) * 2 + 1] = u1;
+                }
+                l0 = l0 * al0 + rs0;
+                l1 = l1 * al1 + rs1;
+#pragma unroll
+                for (int i = 0; i < DT; ++i) { o[i][0] *= al0; o[i][1] *= al0; o[i][2] *= al1; o[i][3] *= al1; }
+            }
+
+            // ---- O += P V
+            mbar_wait(&bar_v[w], phase);
+            if (valid) {
+#pragma unroll
+                for (int kt = 0; kt < 4; ++kt) {
+                    const uint32_t row_addr = v_base + (kt * 16 + (mi & 1) * 8 + ri) * 128;
+#pragma unroll
+                    for (int dp = 0; dp < DT / 2; ++dp) {
+                        const int c = dp * 2 + (mi >> 1);
+                        uint32_t b0, b1, b2, b3;
+                        ldmatrix_x4_trans(row_addr + (c >> 3) * 8192 + (((c & 7) ^ ri) << 4), b0, b1, b2, b3);
+                        mma_bf16_16816(o[2 * dp], pa[kt], b0, b1);
+                        mma_bf16_16816(o[2 * dp + 1], pa[kt], b2, b3);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0 && have_n) { fence_proxy_async_smem(); issue_v(nxt_r, nxt_s); }
+            phase ^= 1;
+            cur_r = nxt_r;
+            cur_s = nxt_s;
+            have = have_n;
+        }
+        TRACE(3);
+        // ---- warp partial -> exchange buffer 0
+        l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
+        l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+        l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
+        l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+        float* wo = reinterpret_cast<float*>(smem + SM::OFF_XCHG + (size_t)w * SM::XCHG_WARP);
+#pragma unroll
+        for (int i = 0; i < DT; ++i) {
+            *reinterpret_cast<float2*>(wo + gid * SM::OROW + i * 8 + tig * 2) = make_float2(o[i][0], o[i][1]);
+            *reinterpret_cast<float2*>(wo + (gid + 8) * SM::OROW + i * 8 + tig * 2) = make_float2(o[i][2], o[i][3]);
+        }
+        if (tig == 0) {
+            s_ml[0][w][0][gid] = m0; s_ml[0][w][1][gid] = l0;
+            s_ml[0][w][0][gid + 8] = m1; s_ml[0][w][1][gid + 8] = l1;
+        }
+        if (f >= f_end && n_parts > 1) {   // the CTA's last segment: finished below, when the stages are idle
+            park_r = r; park_part = part; park_n = n_parts;
+            break;
+        }
+        __syncthreads();
+        cta_merge(0, r, part, n_parts);
+        if (n_parts > 1 && publish(r, n_parts))
+            row_merge(r, n_parts, smem + SM::OFF_XCHG + (size_t)NW * SM::XCHG_WARP, MCH_XCHG);
+        __syncthreads();   // exchange buffer 0 is free again
     }
-    store_out(acc, LL);
+    if (park_r < 0) return;
+    __syncthreads();
+    TRACE(3);
+    cta_merge(0, park_r, park_part, park_n);
+    TRACE(4);
+    const bool owes_merge = publish(park_r, park_n);
+    TRACE(5);
+    if (owes_merge) row_merge(park_r, park_n, smem, MCH_STAGES);
+    TRACE(6);
+}
+
+// Launch shape: 4 consumer warps (= 4 x 32 KiB K/V stages at D = 128), one CTA per SM (128 KiB of tiles in flight per SM).
+constexpr int ATT_NW = 4;
+
+template <int D>
+int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, cudaStream_t st) {
+    auto kern = sparse_decode_kernel<D, ATT_NW, 1>;
+    constexpr int smem = AttnSmem<D, ATT_NW>::TOTAL;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
+    kern<<<C, ATT_NW * 32, smem, st>>>(*map, p);
+    return SPARDA_OK;
 }
 
 }  // namespace
+
+// Grid size of the flat split.  attn_splits = s > 0: s CTAs per row.  attn_splits = 0 (measured on B200, 128K shapes,
+// batch 4..32): a row-aligned split wins whenever one exists -- s CTAs per row with s a divisor of topk, s <= 8 (few
+// partials per row keep the row merge short) and s*R <= SM count, the largest such grid (batch 32: 2 x 64 = 128 CTAs,
+// 0.73 of the HBM peak against 0.64 for 148 row-spanning CTAs).  Otherwise (R > SM count, or topk without a useful
+// divisor) one CTA per SM over the flat list, at least one slot per consumer warp.  Always <= W and within the workspace.
+int sparda_resolve_attn_ctas(const sparda_ctx* ctx, int topk) {
+    const long long W = (long long)ctx->R * topk;
+    long long C;
+    if (ctx->cfg.attn_splits > 0) {
+        C = (long long)ctx->cfg.attn_splits * ctx->R;
+    } else {
+        long long flat = ctx->sm_count;
+        if (flat > 8LL * ctx->R) flat = 8LL * ctx->R;
+        const long long cap = (W + ATT_NW - 1) / ATT_NW;
+        if (flat > cap) flat = cap;
+        long long aligned = 0;
+        for (int s = 1; s <= 8 && s <= topk; ++s)
+            if (topk % s == 0 && (long long)s * ctx->R <= ctx->sm_count) aligned = (long long)s * ctx->R;
+        C = (aligned * 5 >= flat * 3) ? aligned : flat;
+    }
+    // workspace: a row meets at most ceil(topk / quota) + 1 CTAs, quota = floor(W / C); keep that <= max_splits
+    const long long quota_min = (topk + ctx->max_splits - 2) / (ctx->max_splits - 1);
+    if (C > W / quota_min) C = W / quota_min;
+    if (C > W) C = W;
+    if (C < 1) C = 1;
+    return (int)C;
+}
+
+int sparda_resolve_splits(const sparda_ctx* ctx, int topk) {
+    return (sparda_resolve_attn_ctas(ctx, topk) + ctx->R - 1) / ctx->R;
+}
 
 int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
                        int n_slots, void* O, cudaStream_t st) {
@@ -311,24 +493,14 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     p.Hq = ctx->cfg.n_q_heads;
     p.Hkv = ctx->cfg.n_kv_heads;
     p.G = ctx->G;
-    p.splits = sparda_resolve_splits(ctx, topk);
     p.max_splits = ctx->max_splits;
+    p.W = ctx->R * topk;
     p.scale_log2 = 1.4426950408889634f / sqrtf((float)D);
-    dim3 grid(p.splits, ctx->R);
-    static bool attr_set[2] = {false, false};
-    if (D == 128) {
-        if (!attr_set[0]) {
-            SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(sparse_decode_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::TOTAL));
-            attr_set[0] = true;
-        }
-        sparse_decode_kernel<128><<<grid, ATT_THREADS, AttnSmem<128>::TOTAL, st>>>(*map, p);
-    } else {
-        if (!attr_set[1]) {
-            SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(sparse_decode_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::TOTAL));
-            attr_set[1] = true;
-        }
-        sparse_decode_kernel<64><<<grid, ATT_THREADS, AttnSmem<64>::TOTAL, st>>>(*map, p);
-    }
+    const int C = sparda_resolve_attn_ctas(ctx, topk);
+    p.quota = p.W / C;
+    p.rem = p.W % C;
+    rc = D == 128 ? launch<128>(ctx, map, p, C, st) : launch<64>(ctx, map, p, C, st);
+    if (rc) return rc;
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;
     return SPARDA_OK;

@@ -28,7 +28,7 @@
  *    Q, O               : [B][Hq][D] bf16; head h belongs to group h / G.
  *    ids                : [R][k] int32, ascending block ids, -1 padded.
  *  - Ownership: the caller owns every tensor and every stream; the library owns only the workspace
- *    allocated by sparda_create (split-K partials, score scratch, tickets, events).  No call
+ *    allocated by sparda_create (split-K partials, tickets, events).  No call
  *    allocates after sparda_create, synchronises the host, or copies results to the host.
  *  - `stream` arguments are cudaStream_t values passed as void* (torch: stream.cuda_stream).  Calls on
  *    one context must be issued from one host thread at a time.  Work is enqueued asynchronously; a
@@ -88,7 +88,7 @@ typedef struct {
 #define SPARDA_STEP_SERIAL 1     /* same kernels, everything on compute_stream in Algorithm-2 order (no overlap) */
 
 /* Create a context for one shape family on the current device.  Allocates the workspace (split-K partials
- * R*max_splits*16*(D+2) floats, score scratch R*max_blocks floats, tickets, 2*max_layers events, host-step
+ * R*max_splits*16*(D+2) floats, R tickets, 2*max_layers events, host-step
  * staging, a 256 KiB-per-SM score tile for the comparison selector).
  * Returns SPARDA_OK, SPARDA_EINVAL, SPARDA_EUNSUPPORTED, SPARDA_ENOMEM or SPARDA_ECUDA; *out is set only on
  * success.  Destroy with sparda_destroy (synchronises the device first).                                     */
@@ -105,7 +105,8 @@ int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_bloc
  * accumulate, no softmax, no scale) for candidate blocks j in [0, n_cand); ids_out[r] = the min(topk, n_cand)
  * best blocks, ties to the lowest block id, emitted in ascending block id and padded with -1.
  * F [R][D], Kpool [R][n_blocks][D], ids_out [R][topk]: device.  0 <= n_cand <= n_blocks <= max_blocks,
- * 1 <= topk <= cfg.topk.  One kernel launch on `stream`.                                                      */
+ * 1 <= topk <= cfg.topk.  One kernel launch on `stream` (one thread-block cluster per row; the scores stay in
+ * shared memory).                                                                                              */
 int sparda_forecast_select(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
                            int32_t* ids_out, void* stream);
 

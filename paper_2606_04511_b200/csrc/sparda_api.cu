@@ -82,13 +82,11 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     const size_t D = cfg->head_dim;
     size_t n_po = (size_t)ctx->R * ctx->max_splits * SPARDA_MAX_G * D;
     size_t n_ml = (size_t)ctx->R * ctx->max_splits * 2 * SPARDA_MAX_G;
-    size_t n_sc = (size_t)ctx->R * cfg->max_blocks;
     bool ok = cudaMalloc(&ctx->part_O, n_po * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->part_ml, n_ml * sizeof(float)) == cudaSuccess &&
-              cudaMalloc(&ctx->scores, n_sc * sizeof(float)) == cudaSuccess &&
-              cudaMalloc(&ctx->tickets, 2 * (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
+              cudaMalloc(&ctx->tickets, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&ctx->pf_scratch, (size_t)ctx->sm_count * 512 * 128 * sizeof(float)) == cudaSuccess &&
-              cudaMemset(ctx->tickets, 0, 2 * (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
+              cudaMemset(ctx->tickets, 0, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
     ctx->ev_gather = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
     ctx->ev_prof = (cudaEvent_t*)calloc((size_t)3 * (ctx->max_layers + 1) * 2, sizeof(cudaEvent_t));
@@ -120,7 +118,6 @@ int sparda_destroy(sparda_ctx* ctx) {
     (void)cudaDeviceSynchronize();
     cudaFree(ctx->part_O);
     cudaFree(ctx->part_ml);
-    cudaFree(ctx->scores);
     cudaFree(ctx->tickets);
     cudaFree(ctx->pf_scratch);
     for (int i = 0; i <= ctx->max_layers; ++i) {

@@ -27,8 +27,7 @@ struct sparda_ctx {
     // workspace (device)
     float* part_O;     // [R][max_splits][16][D]
     float* part_ml;    // [R][max_splits][2][16]  (m in log2 domain, l)
-    float* scores;     // [R][max_blocks] select scratch (orderable keys as uint32)
-    unsigned int* tickets;  // [2][R]: [0] = select, [1] = attention
+    unsigned int* tickets;  // [R]: split-K attention, one per row (the select keeps its scores on chip)
     float* pf_scratch;      // prefill comparison selector: [sm_count][512][128] fp32 group-summed scores (lazy)
     cudaEvent_t* ev_sel;    // [max_layers + 1]
     cudaEvent_t* ev_gather; // [max_layers + 1]

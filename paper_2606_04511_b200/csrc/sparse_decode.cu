@@ -486,7 +486,7 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     p.O = (__nv_bfloat16*)O;
     p.part_O = ctx->part_O;
     p.part_ml = ctx->part_ml;
-    p.tickets = ctx->tickets + ctx->R;
+    p.tickets = ctx->tickets;
     p.topk = topk;
     p.indexed = indexed;
     p.n_slots = n_slots;

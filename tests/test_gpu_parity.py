@@ -94,6 +94,24 @@ def test_select_ties_and_planted_scores(sp, oracle):
     parity.check_ids(got, want, s)
 
 
+@pytest.mark.parametrize("batch,n_blocks,n_cand", [(4, 2048, 2048), (4, 2048, 1999), (32, 2048, 2048), (100, 700, 650), (1, 8192, 8190)])
+def test_forecast_select_cluster_shapes(batch, n_blocks, n_cand, sp, oracle):
+    """Every cluster shape of the select launch at the [BJ] 128K sizes: 16 CTAs per row (batch 4, configs[2]), 2 per
+    row (batch 32, configs[3]), one CTA per row in several waves (R = 200 > SM count), the largest row (8192 blocks), and
+    ragged per-CTA key ranges (n_cand not a multiple of the cluster size or of a stage)."""
+    cfg = synth.DecodeConfig("sel", batch=batch, n_q_heads=32, n_kv_heads=2, head_dim=128, n_blocks=n_blocks, topk=64, seed=61)
+    ctx = sp.Sparda.from_config(cfg)
+    g = torch.Generator(device="cuda").manual_seed(61 + batch)
+    bias = torch.randn((cfg.rows, n_blocks, 1), generator=g, device="cuda") * 1.5
+    kpool = (torch.randn((cfg.rows, n_blocks, 128), generator=g, device="cuda") * 0.125 + bias).to(torch.bfloat16)
+    F = torch.randn((cfg.rows, 128), generator=g, device="cuda").to(torch.bfloat16)
+    ids = torch.full((cfg.rows, 64), -7, dtype=torch.int32, device="cuda")
+    ctx.forecast_select(F, kpool, n_blocks, 64, ids, n_cand=n_cand)
+    torch.cuda.synchronize()
+    want, s = oracle.forecast_select(_bits(F), _bits(kpool), 64, n_cand)
+    parity.check_ids(ids.cpu().numpy(), want, s, n_cand)
+
+
 @pytest.mark.parametrize("mode", ["tma", "ldg"])
 @pytest.mark.parametrize("cfg", CASES, ids=lambda c: c.name)
 def test_gather_exact_bytes(cfg, mode, sp, oracle):
@@ -265,6 +283,46 @@ def test_decode_step_host_buffers_and_profile(sp):
     torch.cuda.synchronize()
     for d, h in zip(dev, host):
         assert torch.equal(d["O"].cpu().view(torch.int16), h["O"].view(torch.int16))
+
+
+def test_decode_step_replays_from_a_cuda_graph(sp):
+    """sparda_decode_step makes no host synchronisation and uses pre-created events, so the whole two-stream step can
+    be captured once and replayed; a replay on fresh (poisoned) pools gives bit-identical O and ids."""
+    cfg = G16.with_(n_layers=4)
+    ctx = sp.Sparda.from_config(cfg, max_layers=4)
+    R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim
+    dev = []
+    for l in range(cfg.n_layers):
+        L = synth.decode_layer(cfg, l, device="cuda")
+        kpool = torch.empty((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+        ctx.pool_keys(L["kv"], R, Nb, kpool)
+        dev.append({"F": L["F"], "Q": L["Q"], "Kpool": kpool, "kv": L["kv"] if l == 0 else L["kv"].cpu().pin_memory(),
+                    "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda"),
+                    "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda")})
+        if l == 0:
+            F0 = L["F0cur"]
+    pools = [torch.zeros((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    arr = ctx.make_layers(dev)
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    ctx.decode_step(arr, F0, Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)      # eager: reference + warm-up
+    torch.cuda.synchronize()
+    want = [(d["O"].clone(), d["ids"].clone()) for d in dev]
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=cs):
+        ctx.decode_step(arr, F0, Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)
+    for rep in range(2):
+        for d in dev:
+            d["O"].zero_()
+            d["ids"].fill_(-9)
+        for p in pools:
+            p.fill_(float("nan"))
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        for d, (o, i) in zip(dev, want):
+            assert torch.equal(d["ids"], i)
+            assert torch.equal(d["O"].view(torch.int16), o.view(torch.int16))
 
 
 def test_cfg2_full_size_layer(sp, oracle):

@@ -243,3 +243,76 @@ def decode_pipeline(layers, k: int):
             O, O64 = sparse_attn(lay["Q"], pool, ids, pool_is_indexed=False)
         out.append({"ids": ids, "scores": s, "pool": pool, "O": O, "O64": O64})
     return out
+
+
+# ---- o11 / o12: step-to-step block reuse ----------------------------------
+def reuse_plan(ids_new: np.ndarray, slot_ids: np.ndarray):
+    """o11: which pool slot holds which block after a step, and what must be fetched.
+
+    The paper's engine keeps, per layer, the blocks selected at the previous decode step and fetches
+    "only newly selected blocks"; it gives no slot policy.  Reading q18: a slot
+    whose block is selected again keeps it; the j-th smallest newly selected block id that is not
+    resident goes to the j-th lowest-numbered slot whose block was not selected again; slots left
+    over (fewer selected blocks than slots) become empty (-1).  Plain loops over Python sets, one
+    row at a time.
+
+    ids_new [R][k] (ascending, -1 padded), slot_ids [R][k] (block held by each slot, -1 = empty)
+    -> (slot_ids_after [R][k], fetch [R][k]): fetch[r][s] = block to copy into slot s, or -1.
+    """
+    ids_new = np.asarray(ids_new, dtype=np.int32)
+    slot_ids = np.asarray(slot_ids, dtype=np.int32)
+    assert ids_new.shape == slot_ids.shape
+    R, k = ids_new.shape
+    after = np.full((R, k), -1, dtype=np.int32)
+    fetch = np.full((R, k), -1, dtype=np.int32)
+    for r in range(R):
+        wanted = [int(b) for b in ids_new[r] if b >= 0]
+        wanted_set = set(wanted)
+        resident = set()
+        free = []
+        for s in range(k):
+            b = int(slot_ids[r, s])
+            if b >= 0 and b in wanted_set and b not in resident:
+                after[r, s] = b
+                resident.add(b)
+            else:
+                free.append(s)
+        misses = sorted(b for b in wanted_set if b not in resident)
+        assert len(misses) <= len(free)
+        for j, b in enumerate(misses):
+            after[r, free[j]] = b
+            fetch[r, free[j]] = b
+    return after, fetch
+
+
+def decode_pipeline_cached(steps, k: int, state=None):
+    """o12: Algorithm 2 lines 4-7 over several decode steps with the per-layer block cache of the
+    previous step.  ``steps`` is a list (one entry per decode step) of layer lists as in
+    ``decode_pipeline``; the KV caches and pooled keys may be shared between steps.  Per layer l >= 1 the pool
+    persists between steps: o11 decides the slots, o5 copies only the fetched blocks, o6 attends over the pool
+    in slot order.  Returns (per-step list of per-layer dicts {ids, slot_ids, fetch, pool, O, O64}, state)."""
+    n_layers = len(steps[0])
+    if state is None:
+        state = {"slot_ids": [None] * n_layers, "pool": [None] * n_layers}
+    out = []
+    for layers in steps:
+        res = []
+        for l, lay in enumerate(layers):
+            f = lay["F0cur"] if l == 0 else layers[l - 1]["F"]
+            ids, s = forecast_select(f, lay["kpool"], k)
+            if l == 0:
+                O, O64 = sparse_attn(lay["Q"], lay["kv"], ids, pool_is_indexed=True)
+                res.append({"ids": ids, "scores": s, "slot_ids": None, "fetch": None, "pool": None, "O": O, "O64": O64})
+                continue
+            if state["slot_ids"][l] is None:
+                R, _, _, S, D = lay["kv"].shape
+                state["slot_ids"][l] = np.full((R, k), -1, dtype=np.int32)
+                state["pool"][l] = np.zeros((R, k, 2, S, D), dtype=np.uint16)
+            after, fetch = reuse_plan(ids, state["slot_ids"][l])
+            gather(lay["kv"], fetch, state["pool"][l])       # copies fetch >= 0 slots only
+            state["slot_ids"][l] = after
+            O, O64 = sparse_attn(lay["Q"], state["pool"][l], after, pool_is_indexed=False)
+            res.append({"ids": ids, "scores": s, "slot_ids": after.copy(), "fetch": fetch, "pool": state["pool"][l].copy(),
+                        "O": O, "O64": O64})
+        out.append(res)
+    return out, state

@@ -347,6 +347,101 @@ def test_pipeline_wiring_with_planted_needles(oracle):
                 assert out[l]["pool"][r, i].tobytes() == layers[l]["kv"][r, j].tobytes()
 
 
+# ---------------------------------------------------------------- o11 / o12 block reuse between decode steps
+def test_reuse_plan_set_invariants_random(oracle):
+    """o11 against what 'only newly selected blocks are fetched' fixes, checked with Python sets written
+    here: after the step the pool holds exactly the new selection, re-selected blocks did not move, the fetched
+    blocks are exactly new \\ old, nothing else is touched."""
+    rng = np.random.default_rng(7)
+    for trial in range(200):
+        k = int(rng.integers(1, 20))
+        nb = int(rng.integers(k, 3 * k + 2))
+        R = 3
+        old = np.full((R, k), -1, dtype=np.int32)
+        new = np.full((R, k), -1, dtype=np.int32)
+        for r in range(R):
+            m_old = int(rng.integers(0, k + 1))
+            m_new = int(rng.integers(0, k + 1))
+            old[r, rng.permutation(k)[:m_old]] = rng.permutation(nb)[:m_old]      # unordered slots, some empty
+            new[r, :m_new] = np.sort(rng.permutation(nb)[:m_new])                    # ascending, -1 padded
+        after, fetch = oracle.reuse_plan(new, old)
+        for r in range(R):
+            so, sn = set(old[r][old[r] >= 0].tolist()), set(new[r][new[r] >= 0].tolist())
+            assert set(after[r][after[r] >= 0].tolist()) == sn
+            assert len(after[r][after[r] >= 0]) == len(sn)                           # no duplicates
+            assert set(fetch[r][fetch[r] >= 0].tolist()) == sn - so
+            for s_ in range(k):
+                if old[r, s_] >= 0 and int(old[r, s_]) in sn:
+                    assert after[r, s_] == old[r, s_] and fetch[r, s_] == -1          # a hit stays where it is
+                if fetch[r, s_] >= 0:
+                    assert after[r, s_] == fetch[r, s_]
+            # ascending misses meet ascending freed slots
+            f = fetch[r][fetch[r] >= 0]
+            assert np.all(np.diff(f) > 0)
+
+
+def test_reuse_plan_special_cases(oracle):
+    new = np.array([[2, 5, 9, 11]], dtype=np.int32)
+    empty = np.full((1, 4), -1, dtype=np.int32)
+    after, fetch = oracle.reuse_plan(new, empty)                 # first step: a plain gather in id order
+    np.testing.assert_array_equal(after, new)
+    np.testing.assert_array_equal(fetch, new)
+    after2, fetch2 = oracle.reuse_plan(new, after)               # same selection again: nothing to fetch
+    np.testing.assert_array_equal(after2, after)
+    assert np.all(fetch2 == -1)
+    after3, fetch3 = oracle.reuse_plan(np.array([[1, 5, 11, 30]], dtype=np.int32), after)
+    np.testing.assert_array_equal(after3, [[1, 5, 30, 11]])      # 2 -> 1 (slot 0), 9 -> 30 (slot 2); 5 and 11 stay
+    np.testing.assert_array_equal(fetch3, [[1, -1, 30, -1]])
+    after4, fetch4 = oracle.reuse_plan(np.array([[5, -1, -1, -1]], dtype=np.int32), after3)
+    np.testing.assert_array_equal(after4, [[-1, 5, -1, -1]])     # fewer selected than slots: the rest become empty
+    assert np.all(fetch4 == -1)
+
+
+def test_cached_pipeline_equals_plain_pipeline_step_by_step(oracle):
+    """o12: with the block cache the pool holds the same blocks in another slot order, so every step's attention
+    equals the cache-free pipeline o10 up to the order of a double-precision sum, the pool slots hold exactly the
+    bytes of the blocks slot_ids names, and only new blocks are copied."""
+    cfg = SMALL.with_(n_layers=3, topk=4)
+    base = []
+    for l in range(cfg.n_layers):
+        L = _layer(cfg, l)
+        L["kpool"] = oracle.pool_keys(L["kv"])
+        base.append(L)
+    rng = np.random.default_rng(3)
+    steps = []
+    for t in range(4):
+        layers = []
+        for l, L in enumerate(base):
+            d = dict(L)
+            if t > 0:                                             # drift the Forecast a little: selections overlap
+                f = bf.bits_to_f64(L["F"]) + 0.6 * t * rng.standard_normal(L["F"].shape)
+                d["F"] = bf.f64_to_bf16_bits(f)
+            layers.append(d)
+        steps.append(layers)
+    out, _ = oracle.decode_pipeline_cached(steps, cfg.topk)
+    fetched_total = 0
+    for t, layers in enumerate(steps):
+        plain = oracle.decode_pipeline(layers, cfg.topk)
+        for l in range(cfg.n_layers):
+            np.testing.assert_array_equal(out[t][l]["ids"], plain[l]["ids"])
+            np.testing.assert_allclose(out[t][l]["O64"], plain[l]["O64"], rtol=0, atol=1e-9)
+            if l == 0:
+                continue
+            for r in range(cfg.rows):
+                assert sorted(out[t][l]["slot_ids"][r].tolist()) == sorted(plain[l]["ids"][r].tolist())
+                for s_, j in enumerate(out[t][l]["slot_ids"][r]):
+                    assert out[t][l]["pool"][r, s_].tobytes() == layers[l]["kv"][r, j].tobytes()
+            n_f = int((out[t][l]["fetch"] >= 0).sum())
+            if t == 0:
+                assert n_f == cfg.rows * cfg.topk
+            else:
+                new_blocks = sum(len(set(out[t][l]["ids"][r].tolist()) - set(out[t - 1][l]["ids"][r].tolist()))
+                                 for r in range(cfg.rows))
+                assert n_f == new_blocks
+                fetched_total += n_f
+    assert 0 < fetched_total < 3 * 2 * cfg.rows * cfg.topk       # the drift really produced partial reuse
+
+
 # ---------------------------------------------------------------- closed forms the paper prints
 def test_paper_closed_forms_golden():
     """tests/golden/paper_closed_forms.txt: P:L95 (33.5M Forecast parameters, 0.41% of 8B) and the

@@ -152,6 +152,38 @@ int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_l
                             int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
                             int mode);
 
+/* (f1) Step-to-step block reuse.  The paper's engine keeps, per layer, the blocks selected at the previous decode
+ * step and fetches "only newly selected blocks" (App. C); it states no slot policy, so this library fixes one
+ * (reading q18): a pool slot whose block is selected again keeps it; the j-th smallest newly selected block
+ * that is not resident goes to the j-th lowest-numbered slot whose block was not selected again; slots left over
+ * become empty (-1).
+ *   ids_new  [R][topk] device, this step's selection as written by sparda_forecast_select (ascending, -1 padded);
+ *   slot_ids [R][topk] device, in/out: the block each slot of the layer's persistent pool holds (-1 = empty; the
+ *            caller initialises it to -1 once);
+ *   fetch    [R][topk] device, out: fetch[r][s] = block to copy into slot s, or -1 -- pass it as `ids` to
+ *            sparda_prefetch_launch; pass slot_ids as `ids` to sparda_sparse_decode (pool_is_indexed = 0);
+ *   n_fetch  [R] device, out (may be NULL): blocks to fetch per row.
+ * One small kernel on `stream`; topk <= 256.                                                                  */
+int sparda_reuse_plan(sparda_ctx* ctx, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch,
+                      int32_t* n_fetch, void* stream);
+
+/* One decoder layer of sparda_decode_step_cached: sparda_layer plus the layer's persistent pool and slot table.   */
+typedef struct {
+    sparda_layer base;   /* as in sparda_decode_step                                                             */
+    void* pool;          /* [R][topk][2][S][D] device, owned by the caller, persistent across steps (layer 0: unused) */
+    int32_t* slot_ids;   /* [R][topk] device, in/out (see sparda_reuse_plan); initialise to -1                   */
+    int32_t* fetch;      /* [R][topk] device, written                                                            */
+    int32_t* n_fetch;    /* [R] device, written; may be NULL                                                     */
+} sparda_cached_layer;
+
+/* sparda_decode_step with the previous step's blocks kept per layer: per layer l >= 1 the compute stream
+ * runs select B_{l+1} -> reuse_plan -> [prefetch stream: gather only the missing blocks into layer l+1's own pool] ->
+ * wait for layer l's gather -> attention over pool_l in slot order.  Layer 0 attends from its resident cache as
+ * before.  Same modes, same capture rules; with every slot_ids at -1 the step moves exactly the bytes of
+ * sparda_decode_step.                                                                                           */
+int sparda_decode_step_cached(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur,
+                              int n_blocks, int topk, void* compute_stream, void* prefetch_stream, int mode);
+
 /* Per-kernel device timing of sparda_decode_step (measurement aid).  While enabled, every kernel
  * launched by sparda_decode_step is bracketed by timing events on the stream it is launched on (after any
  * stream wait, so a wait is not counted).  sparda_profile_read synchronises on those events and returns, for

@@ -20,6 +20,7 @@ STEP_OVERLAP, STEP_SERIAL = 0, 1
 EXPORTS = [
     "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_select", "sparda_prefetch_launch",
     "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
+    "sparda_reuse_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
     "sparda_launch_count", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
     "sparda_last_cuda_error", "sparda_version",
@@ -39,6 +40,11 @@ class SpardaConfig(ctypes.Structure):
 class SpardaLayer(ctypes.Structure):
     _fields_ = [("F", ctypes.c_void_p), ("Q", ctypes.c_void_p), ("Kpool", ctypes.c_void_p), ("kv", ctypes.c_void_p),
                 ("O", ctypes.c_void_p), ("ids", ctypes.c_void_p)]
+
+
+class SpardaCachedLayer(ctypes.Structure):
+    _fields_ = [("base", SpardaLayer), ("pool", ctypes.c_void_p), ("slot_ids", ctypes.c_void_p), ("fetch", ctypes.c_void_p),
+                ("n_fetch", ctypes.c_void_p)]
 
 
 _lib = None
@@ -61,6 +67,8 @@ def lib() -> ctypes.CDLL:
         L.sparda_sparse_decode.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_decode_step.argtypes = [vp, ctypes.POINTER(SpardaLayer), i32, vp, i32, i32, vp, vp, vp, vp, i32]
         L.sparda_decode_step_host.argtypes = L.sparda_decode_step.argtypes
+        L.sparda_reuse_plan.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+        L.sparda_decode_step_cached.argtypes = [vp, ctypes.POINTER(SpardaCachedLayer), i32, vp, i32, i32, vp, vp, i32]
         L.sparda_profile_enable.argtypes = [vp, i32]
         L.sparda_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
         L.sparda_prefill_select.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
@@ -168,6 +176,25 @@ class Sparda:
         self._check(self._L.sparda_decode_step_host(self._h, layer_array, len(layer_array), _ptr(F0cur), n_blocks, topk,
                                                     _ptr(pool0), _ptr(pool1), _stream(compute_stream),
                                                     _stream(prefetch_stream), mode), "decode_step_host")
+
+    def reuse_plan(self, ids_new, topk, slot_ids, fetch, n_fetch=None, stream=None):
+        self._check(self._L.sparda_reuse_plan(self._h, _ptr(ids_new), topk, _ptr(slot_ids), _ptr(fetch),
+                                              _ptr(n_fetch) if n_fetch is not None else None, _stream(stream)), "reuse_plan")
+
+    def make_cached_layers(self, layers):
+        """layers: list of dicts with tensors F, Q, Kpool, kv, O, ids and (layers >= 1) pool, slot_ids, fetch, n_fetch."""
+        arr = (SpardaCachedLayer * len(layers))()
+        for i, l in enumerate(layers):
+            base = SpardaLayer(_ptr(l["F"]), _ptr(l["Q"]), _ptr(l["Kpool"]), _ptr(l["kv"]), _ptr(l["O"]), _ptr(l["ids"]))
+            opt = [(_ptr(l[n]) if l.get(n) is not None else None) for n in ("pool", "slot_ids", "fetch", "n_fetch")]
+            arr[i] = SpardaCachedLayer(base, *opt)
+        return arr
+
+    def decode_step_cached(self, layer_array, F0cur, n_blocks, topk, compute_stream=None, prefetch_stream=None,
+                           mode=STEP_OVERLAP):
+        self._check(self._L.sparda_decode_step_cached(self._h, layer_array, len(layer_array), _ptr(F0cur), n_blocks, topk,
+                                                      _stream(compute_stream), _stream(prefetch_stream), mode),
+                    "decode_step_cached")
 
     def profile_enable(self, on=True):
         self._check(self._L.sparda_profile_enable(self._h, 1 if on else 0), "profile_enable")

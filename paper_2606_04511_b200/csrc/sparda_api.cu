@@ -246,6 +246,64 @@ int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers
     return SPARDA_OK;
 }
 
+int sparda_reuse_plan(sparda_ctx* ctx, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch,
+                      void* stream) {
+    if (!ctx || !sparda_aligned(ids_new, 4) || !sparda_aligned(slot_ids, 4) || !sparda_aligned(fetch, 4)) return SPARDA_EINVAL;
+    if (n_fetch && !sparda_aligned(n_fetch, 4)) return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    return sparda_launch_reuse_plan(ctx, ids_new, topk, slot_ids, fetch, n_fetch, (cudaStream_t)stream);
+}
+
+// Algorithm 2 lines 4-7 with the per-layer block cache of the previous step.  Hand-off: gather l+1 writes
+// pool_{l+1}, last read by attention l+1 of the PREVIOUS step, which precedes this step's select on the compute stream,
+// so ev_sel[l+1] releases it; reuse_plan updates slot_ids_{l+1} in place under the same ordering.
+int sparda_decode_step_cached(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur, int n_blocks,
+                              int topk, void* compute_stream, void* prefetch_stream, int mode) {
+    if (!ctx || !layers || n_layers < 1 || n_layers > ctx->max_layers || !F0cur) return SPARDA_EINVAL;
+    if (mode != SPARDA_STEP_OVERLAP && mode != SPARDA_STEP_SERIAL) return SPARDA_EINVAL;
+    for (int l = 1; l < n_layers; ++l)
+        if (!layers[l].pool || !layers[l].slot_ids || !layers[l].fetch) return SPARDA_EINVAL;
+    cudaStream_t cs = (cudaStream_t)compute_stream;
+    cudaStream_t ps = mode == SPARDA_STEP_OVERLAP ? (cudaStream_t)prefetch_stream : cs;
+    int rc;
+    ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
+    SPARDA_PROF_BEGIN(0, cs);
+    rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_blocks, topk, layers[0].base.ids, cs);
+    if (rc) return rc;
+    SPARDA_PROF_END(0, cs);
+    for (int l = 0; l < n_layers; ++l) {
+        if (l + 1 < n_layers) {
+            const sparda_cached_layer* nx = &layers[l + 1];
+            SPARDA_PROF_BEGIN(0, cs);
+            rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, cs);
+            if (rc) return rc;
+            rc = sparda_reuse_plan(ctx, nx->base.ids, topk, nx->slot_ids, nx->fetch, nx->n_fetch, cs);
+            if (rc) return rc;
+            SPARDA_PROF_END(0, cs);
+            if (ps != cs) {
+                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], cs));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ps, ctx->ev_sel[l + 1], 0));
+            }
+            SPARDA_PROF_BEGIN(1, ps);
+            rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->fetch, topk, nx->pool, ps);
+            if (rc) return rc;
+            SPARDA_PROF_END(1, ps);
+            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], ps));
+        }
+        if (l == 0) {
+            SPARDA_PROF_BEGIN(2, cs);
+            rc = sparda_sparse_decode(ctx, layers[0].base.Q, layers[0].base.kv, layers[0].base.ids, topk, 1, n_blocks, layers[0].base.O, cs);
+        } else {
+            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
+            SPARDA_PROF_BEGIN(2, cs);
+            rc = sparda_sparse_decode(ctx, layers[l].base.Q, layers[l].pool, layers[l].slot_ids, topk, 0, topk, layers[l].base.O, cs);
+        }
+        if (rc) return rc;
+        SPARDA_PROF_END(2, cs);
+    }
+    return SPARDA_OK;
+}
+
 int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                             int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
                             int mode) {

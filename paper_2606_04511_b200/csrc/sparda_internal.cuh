@@ -63,6 +63,8 @@ int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_bl
                          int32_t* ids, cudaStream_t);
 int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
                          cudaStream_t);
+int sparda_launch_reuse_plan(sparda_ctx*, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch,
+                             cudaStream_t);
 int sparda_launch_attn(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
                        int n_slots, void* O, cudaStream_t);
 int sparda_launch_prefill_select(sparda_ctx*, const void* F, const void* Kpool, int T, int n_blocks, int row0,

@@ -325,6 +325,117 @@ def test_decode_step_replays_from_a_cuda_graph(sp):
             assert torch.equal(d["O"].view(torch.int16), o.view(torch.int16))
 
 
+def test_reuse_plan_matches_oracle(sp, oracle):
+    """f1 slot policy (o11) on the device: bit-exact slot tables, fetch lists and counts, for unordered / partly empty
+    slot tables, padded selections and k from 1 to the 256 maximum."""
+    rng = np.random.default_rng(17)
+    for k, R, nb in [(1, 3, 5), (8, 5, 40), (37, 6, 300), (64, 64, 2048), (256, 9, 700)]:
+        cfg = synth.DecodeConfig("rp", batch=R, n_q_heads=1, n_kv_heads=1, head_dim=64, n_blocks=nb, topk=k)
+        ctx = sp.Sparda.from_config(cfg)
+        old = np.full((R, k), -1, dtype=np.int32)
+        new = np.full((R, k), -1, dtype=np.int32)
+        for r in range(R):
+            m_old = k if r % 3 else int(rng.integers(0, k + 1))
+            m_new = k if r % 4 else int(rng.integers(0, k + 1))
+            base = rng.permutation(nb)
+            old[r, rng.permutation(k)[:m_old]] = base[:m_old]
+            keep = int(rng.integers(0, min(m_old, m_new) + 1))                   # force an overlap of `keep` blocks
+            pick = np.concatenate([base[:keep], base[max(m_old, keep):max(m_old, keep) + m_new - keep]])[:m_new]
+            new[r, :len(pick)] = np.sort(pick)
+        slot = torch.from_numpy(old).cuda()
+        fetch = torch.full((R, k), -5, dtype=torch.int32, device="cuda")
+        nf = torch.full((R,), -5, dtype=torch.int32, device="cuda")
+        ctx.reuse_plan(torch.from_numpy(new).cuda(), k, slot, fetch, nf)
+        torch.cuda.synchronize()
+        want_after, want_fetch = oracle.reuse_plan(new, old)
+        np.testing.assert_array_equal(slot.cpu().numpy(), want_after)
+        np.testing.assert_array_equal(fetch.cpu().numpy(), want_fetch)
+        np.testing.assert_array_equal(nf.cpu().numpy(), (want_fetch >= 0).sum(1))
+
+
+@pytest.mark.parametrize("cfg", [synth.CFG1_TINY.with_(n_layers=4), G16.with_(n_layers=3, batch=3)], ids=lambda c: c.name)
+def test_decode_step_cached_multi_step(cfg, sp, oracle):
+    """Several decode steps with the per-layer block cache (f1) while the Forecast drifts: every step the slot
+    tables and fetch lists equal o11 applied to the GPU's own selection, the pools hold exactly the bytes of the blocks
+    their slot tables name (poisoned before step 0: a missed copy shows as NaN), attention matches the oracle over the
+    pool in slot order, only new blocks move, and overlapped == serialized bit for bit."""
+    R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
+    data = _pipeline_inputs(cfg, sp)
+    g = torch.Generator(device="cuda").manual_seed(99)
+    n_steps = 4
+    Fs = [[(L["F"].float() + 0.5 * t * torch.randn(L["F"].shape, generator=g, device="cuda")).to(torch.bfloat16)
+           for (L, _) in data] for t in range(n_steps)]
+    F0s = [(data[0][0]["F0cur"].float() + 0.5 * t * torch.randn((R, D), generator=g, device="cuda")).to(torch.bfloat16)
+           for t in range(n_steps)]
+
+    def run(mode):
+        ctx = sp.Sparda.from_config(cfg, max_layers=8)
+        dev = []
+        for l, (L, kv_host) in enumerate(data):
+            kpool = torch.empty((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+            ctx.pool_keys(L["kv"], R, Nb, kpool)
+            dev.append({"F": L["F"].clone(), "Q": L["Q"], "Kpool": kpool, "kv": L["kv"] if l == 0 else kv_host,
+                        "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                        "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda"),
+                        "pool": torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") if l else None,
+                        "slot_ids": torch.full((R, k), -1, dtype=torch.int32, device="cuda") if l else None,
+                        "fetch": torch.full((R, k), -9, dtype=torch.int32, device="cuda") if l else None,
+                        "n_fetch": torch.zeros((R,), dtype=torch.int32, device="cuda") if l else None})
+        arr = ctx.make_cached_layers(dev)
+        F0 = F0s[0].clone()
+        cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+        hist = []
+        for t in range(n_steps):
+            for l in range(NL):
+                dev[l]["F"].copy_(Fs[t][l])
+            F0.copy_(F0s[t])
+            torch.cuda.synchronize()
+            ctx.decode_step_cached(arr, F0, Nb, k, cs, ps, mode)
+            torch.cuda.synchronize()
+            hist.append([{n: (d[n].clone() if d[n] is not None else None) for n in ("O", "ids", "pool", "slot_ids", "fetch", "n_fetch")}
+                         for d in dev])
+        return hist, dev
+
+    h_ser, _ = run(sp.STEP_SERIAL)
+    h_ovl, dev = run(sp.STEP_OVERLAP)
+    for t in range(n_steps):
+        for l in range(NL):
+            for n in ("O", "ids", "pool", "slot_ids", "fetch"):
+                a, b = h_ser[t][l][n], h_ovl[t][l][n]
+                if a is not None:
+                    assert torch.equal(a.view(torch.int16) if a.dtype == torch.bfloat16 else a,
+                                       b.view(torch.int16) if b.dtype == torch.bfloat16 else b), f"step {t} layer {l} {n}"
+    kv_bits = [_bits(L["kv"]) for (L, _) in data]
+    kp_bits = [_bits(d["Kpool"]) for d in dev]
+    moved = 0
+    for t in range(n_steps):
+        for l in range(NL):
+            h = h_ovl[t][l]
+            f_bits = _bits(F0s[t]) if l == 0 else _bits(Fs[t][l - 1])
+            want_ids, s = oracle.forecast_select(f_bits, kp_bits[l], k)
+            gids = h["ids"].cpu().numpy()
+            parity.check_ids(gids, want_ids, s)
+            q_bits = _bits(data[l][0]["Q"])
+            if l == 0:
+                want, _ = oracle.sparse_attn(q_bits, kv_bits[0], gids, pool_is_indexed=True)
+                parity.check_attn(_bits(h["O"]), want, f"step {t} layer 0")
+                continue
+            prev = h_ovl[t - 1][l]["slot_ids"].cpu().numpy() if t else np.full((R, k), -1, dtype=np.int32)
+            want_after, want_fetch = oracle.reuse_plan(gids, prev)
+            np.testing.assert_array_equal(h["slot_ids"].cpu().numpy(), want_after)
+            np.testing.assert_array_equal(h["fetch"].cpu().numpy(), want_fetch)
+            np.testing.assert_array_equal(h["n_fetch"].cpu().numpy(), (want_fetch >= 0).sum(1))
+            pool_ref = oracle.gather(kv_bits[l], want_after)
+            assert _bits(h["pool"]).tobytes() == pool_ref.tobytes(), f"step {t} layer {l}: pool bytes"
+            want, _ = oracle.sparse_attn(q_bits, pool_ref, want_after)
+            parity.check_attn(_bits(h["O"]), want, f"step {t} layer {l}")
+            if t:
+                moved += int((want_fetch >= 0).sum())
+            else:
+                assert int((want_fetch >= 0).sum()) == R * k
+    assert 0 < moved < (n_steps - 1) * (NL - 1) * R * k, "the drift should give partial reuse"
+
+
 def test_cfg2_full_size_layer(sp, oracle):
     """BASELINE.json configs[1] at full size: batch 8, 32/2 heads, D=128, 512 blocks, top-64, KV pinned on host."""
     cfg = synth.CFG2_32K

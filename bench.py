@@ -332,6 +332,85 @@ def bench_prefill(torch, binding, peaks_all):
     return out
 
 
+def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps):
+    """SURVEY 8(f) f1 / 8(d) "gather hidden": the same 32-layer decode step with the previous step's blocks kept per
+    layer, so only newly selected blocks cross the host link.  The Forecast alternates between F_A and
+    F_B = bf16(F_A + alpha * N(0,1)) from step to step; alpha sets how much the selection drifts, the fresh-fetch
+    fraction rho is MEASURED (blocks fetched / blocks selected, from the plan kernel's counters).  alpha = 0 gives
+    rho = 0: the compute-only floor of the step; exposed gather time = step(rho) - step(0)."""
+    R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
+    g = torch.Generator(device="cuda").manual_seed(777)
+    layers = []
+    for l, d in enumerate(dev_layers):
+        e = dict(d)
+        e["F"] = d["F"].clone()
+        if l:
+            e["pool"] = torch.zeros((R, k, 2, cfg.block_size, D), dtype=torch.bfloat16, device="cuda")
+            e["slot_ids"] = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
+            e["fetch"] = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
+            e["n_fetch"] = torch.zeros((R,), dtype=torch.int32, device="cuda")
+        layers.append(e)
+    arr = ctx.make_cached_layers(layers)
+    F0w = F0.clone()
+    FA = [d["F"].clone() for d in dev_layers]
+    noise = [torch.randn(d["F"].shape, generator=g, device="cuda") for d in dev_layers]
+    noise0 = torch.randn(F0.shape, generator=g, device="cuda")
+
+    def set_F(which, alpha):
+        for l, e in enumerate(layers):
+            e["F"].copy_(FA[l] if which == 0 else (FA[l].float() + alpha * noise[l]).to(torch.bfloat16))
+        F0w.copy_(F0 if which == 0 else (F0.float() + alpha * noise0).to(torch.bfloat16))
+
+    def one(which, alpha):
+        with torch.cuda.stream(cs):                          # the Forecast of this step is produced on the compute stream
+            set_F(which, alpha)
+        ctx.decode_step_cached(arr, F0w, Nb, k, cs, ps, binding.STEP_OVERLAP)
+
+    out = []
+    for alpha in (0.0, 0.05, 0.1, 0.2, 0.4, 0.8, 1e9):
+        for e in layers[1:]:
+            e["slot_ids"].fill_(-1)
+        for i in range(4):
+            one(i & 1, alpha)
+        torch.cuda.synchronize()
+        fetched = 0
+        for i in range(2):                                   # periodic state: count one A step and one B step
+            one(i & 1, alpha)
+            torch.cuda.synchronize()
+            fetched += sum(int(e["n_fetch"].sum().item()) for e in layers[1:])
+        rho = fetched / (2.0 * (NL - 1) * R * k)
+        n = max(4, steps - steps % 2)
+        torch.cuda.synchronize()
+        # one A step and one B step captured into a CUDA graph (two streams, events and the F copies included): the
+        # ~300 enqueue calls of a step would otherwise pace this compute-sized step from the host
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=cs):
+            for i in range(2):
+                set_F(i & 1, alpha)
+                ctx.decode_step_cached(arr, F0w, Nb, k, cs, ps, binding.STEP_OVERLAP)
+        graph.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(cs):
+            e0.record(cs)
+            for i in range(n // 2):
+                graph.replay()
+            e1.record(cs)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / n
+        del graph
+        out.append({"alpha": alpha if alpha < 1e8 else "independent", "fresh_fetch_fraction": rho, "ms_per_step": ms,
+                    "tok_s": cfg.batch / (ms * 1e-3), "host_link_mib_per_step": rho * (NL - 1) * cfg.gather_bytes_per_layer / 2**20})
+    floor = out[0]["ms_per_step"]
+    for o in out:
+        o["gather_exposed_us_per_layer"] = max(0.0, (o["ms_per_step"] - floor) * 1e3 / (NL - 1))
+    del layers, arr
+    torch.cuda.empty_cache()
+    return {"workload": f"{cfg.name}, per-layer persistent pools ({(NL - 1) * cfg.gather_bytes_per_layer / 2**20:.0f} MiB of HBM), "
+                        "Forecast alternating F_A / F_A + alpha*N(0,1) (F copied on the device each step, inside the timed region); steps replayed from a CUDA graph",
+            "compute_floor_ms_per_step": floor, "sweep": out}
+
+
 def run_sparda(args):
     import torch
     import torch.distributed as dist
@@ -443,6 +522,10 @@ def run_sparda(args):
         step(binding.STEP_SERIAL)
     ms_serial = timed_region(lambda: step(binding.STEP_SERIAL), max(3, args.steps // 3)) / max(3, args.steps // 3)
 
+    reuse = None
+    if not args.no_kernels and rank == 0:
+        reuse = bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, args.steps)
+
     # ---- per-kernel device times inside the pipeline (second pass over the same K steps, timing events on)
     ctx.profile_enable(True)
     prof = {"select": [0.0, 0], "gather": [0.0, 0], "attn": [0.0, 0]}
@@ -534,6 +617,7 @@ def run_sparda(args):
         "roofline_kernels": kernels,
         "cpu_baseline": base,
         "prefill_select": prefill,
+        "reuse_cache": reuse,
         "pipeline": {"ms_per_step_overlap": ms_per_step, "ms_per_step_serial": ms_serial,
                      "us_per_layer_step": ms_per_step * 1e3 / NL,
                      "us_select": t_sel * 1e6, "us_gather": t_gat * 1e6, "us_attn": t_att * 1e6,

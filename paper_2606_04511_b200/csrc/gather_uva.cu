@@ -7,7 +7,7 @@
 // dev_pool[(r*k + slot)].  ids are read from device memory when the kernel runs.
 //
 // Two engines, same tasks, same bytes:
-//  * SPARDA_GATHER_TMA (default, B200-native): ONE thread per CTA drives a ring of 16 KiB shared-memory
+//  * SPARDA_GATHER_TMA (default, B200-native): one warp per CTA compacts the task list and ONE of its threads drives a ring of 16 KiB shared-memory
 //    stages with bulk-copy (TMA) instructions: cp.async.bulk global(host-mapped)->smem completing on an
 //    mbarrier, then cp.async.bulk smem->global(HBM).  No registers or LSU slots are spent on payload, so a
 //    handful of CTAs saturates the host link (measured on this box: 2-4 CTAs x 1 thread reach the same
@@ -24,58 +24,92 @@ using namespace sparda;
 constexpr int GATHER_STAGE_BYTES = 16384;
 constexpr int GATHER_STAGES = 6;  // 96 KiB ring per CTA, up to 5 loads in flight while one stage drains
 
+constexpr int GATHER_WIN = 1024;  // tasks compacted per window (32 per lane, held in registers)
+
+// The task list ids[R*k] may be sparse (the reuse cache, f1, fetches only the blocks that are not resident): the warp
+// first compacts the valid tasks of a window with ballots -- every CTA scans the whole window, CTA c takes the c-th
+// equal share of the VALID tasks, so the split is balanced whatever the pattern -- then lane 0 drives the bulk-copy
+// ring over its share.  An empty list costs one scan (a few microseconds), not one dependent load per slot.
 __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__ host_kv, const int32_t* __restrict__ ids,
                                                         char* __restrict__ pool, int n_rows, int n_blocks, int topk,
                                                         uint32_t block_bytes) {
     extern __shared__ __align__(128) char ring[];
     __shared__ uint64_t full[GATHER_STAGES];
-    if (threadIdx.x != 0) return;
-    for (int s = 0; s < GATHER_STAGES; ++s) mbar_init(&full[s], 1);
-    mbar_fence_init();
-    fence_proxy_async_smem();
-
-    const uint32_t chunks_per_block = block_bytes / GATHER_STAGE_BYTES;  // 2 at D=128, 1 at D=64
-    const int64_t n_units = (int64_t)n_rows * topk * chunks_per_block;
-    // unit u -> (task = u / cpb, chunk = u % cpb); static round-robin over the persistent grid
-    int64_t load_u = blockIdx.x, store_u = blockIdx.x;
-    int load_s = 0, store_s = 0;
+    __shared__ int32_t q_task[GATHER_WIN], q_id[GATHER_WIN];
+    __shared__ char* dst_of[GATHER_STAGES];
+    const int lane = threadIdx.x;
+    if (lane == 0) {
+        for (int s = 0; s < GATHER_STAGES; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+        fence_proxy_async_smem();
+    }
+    __syncwarp();
+    const uint32_t cpb = block_bytes / GATHER_STAGE_BYTES;  // 16 KiB chunks per block: 2 at D=128, 1 at D=64
+    const int64_t n_tasks = (int64_t)n_rows * topk;
+    const unsigned lt = (1u << lane) - 1u;
+    int load_s = 0, store_s = 0, in_flight = 0;
     uint32_t store_phase = 0;
-    int in_flight = 0;
-    // a skipped (-1) unit occupies no stage: both cursors skip it identically
-    auto src_of = [&](int64_t u, const char*& src) -> bool {
-        int64_t task = u / chunks_per_block;
-        uint32_t c = (uint32_t)(u % chunks_per_block);
-        int32_t id = __ldg(ids + task);
-        if (id < 0) return false;
-        int64_t r = task / topk;
-        src = host_kv + ((r * n_blocks + id) * (int64_t)block_bytes + (int64_t)c * GATHER_STAGE_BYTES);
-        return true;
+    auto drain_one = [&]() {   // oldest stage: wait for its load, store it to HBM, free it once the store has read it
+        mbar_wait(&full[store_s], store_phase);
+        bulk_s2g(dst_of[store_s], ring + (size_t)store_s * GATHER_STAGE_BYTES, GATHER_STAGE_BYTES);
+        bulk_commit();
+        bulk_wait_read<0>();
+        if (++store_s == GATHER_STAGES) { store_s = 0; store_phase ^= 1; }
+        --in_flight;
     };
-    while (true) {
-        // fill the ring
-        while (in_flight < GATHER_STAGES && load_u < n_units) {
-            const char* src;
-            if (src_of(load_u, src)) {
+
+    // the ids of a window are loaded one window ahead, so their latency hides behind the copies of the current one
+    int32_t v[GATHER_WIN / 32], vn[GATHER_WIN / 32];
+#pragma unroll
+    for (int j = 0; j < GATHER_WIN / 32; ++j) {
+        const int64_t t = (int64_t)j * 32 + lane;
+        vn[j] = t < n_tasks ? __ldg(ids + t) : -1;
+    }
+    for (int64_t base = 0; base < n_tasks; base += GATHER_WIN) {
+        // ---- compact this window's valid tasks; keep the share [lo, hi) of this CTA
+        int nv = 0;
+#pragma unroll
+        for (int j = 0; j < GATHER_WIN / 32; ++j) {
+            v[j] = vn[j];
+            const int64_t t = base + GATHER_WIN + j * 32 + lane;
+            vn[j] = t < n_tasks ? __ldg(ids + t) : -1;
+            nv += __popc(__ballot_sync(0xffffffffu, v[j] >= 0));
+        }
+        const int lo = (int)((int64_t)nv * blockIdx.x / gridDim.x), hi = (int)((int64_t)nv * (blockIdx.x + 1) / gridDim.x);
+        int seen = 0;
+#pragma unroll
+        for (int j = 0; j < GATHER_WIN / 32; ++j) {
+            const unsigned b = __ballot_sync(0xffffffffu, v[j] >= 0);
+            const int rank = seen + __popc(b & lt);
+            if (v[j] >= 0 && rank >= lo && rank < hi) {
+                q_task[rank - lo] = (int32_t)(base + j * 32 + lane);
+                q_id[rank - lo] = v[j];
+            }
+            seen += __popc(b);
+        }
+        __syncwarp();
+        // ---- lane 0: ring of bulk copies host -> smem -> HBM over (hi - lo) * cpb units of 16 KiB.  A stage remembers
+        // its destination, so loads stay in flight across windows (no drain at a window boundary)
+        if (lane == 0) {
+            const int n_units = (hi - lo) * (int)cpb;
+            for (int u = 0; u < n_units; ++u) {
+                if (in_flight == GATHER_STAGES) { drain_one(); }
+                const int e = u / (int)cpb, c = u % (int)cpb;
+                const int64_t r = q_task[e] / topk;
+                const char* src = host_kv + ((r * n_blocks + q_id[e]) * (int64_t)block_bytes + (int64_t)c * GATHER_STAGE_BYTES);
+                dst_of[load_s] = pool + ((int64_t)q_task[e] * block_bytes + (int64_t)c * GATHER_STAGE_BYTES);
                 mbar_arrive_expect_tx(&full[load_s], GATHER_STAGE_BYTES);
                 bulk_g2s(ring + (size_t)load_s * GATHER_STAGE_BYTES, src, GATHER_STAGE_BYTES, &full[load_s]);
                 if (++load_s == GATHER_STAGES) load_s = 0;
                 ++in_flight;
             }
-            load_u += gridDim.x;
         }
-        if (in_flight == 0) break;
-        // drain the oldest stage
-        const char* dummy;
-        while (!src_of(store_u, dummy)) store_u += gridDim.x;
-        mbar_wait(&full[store_s], store_phase);
-        bulk_s2g(pool + store_u * (int64_t)GATHER_STAGE_BYTES, ring + (size_t)store_s * GATHER_STAGE_BYTES, GATHER_STAGE_BYTES);
-        bulk_commit();
-        bulk_wait_read<0>();  // the stage may be refilled once the store has read it
-        if (++store_s == GATHER_STAGES) { store_s = 0; store_phase ^= 1; }
-        store_u += gridDim.x;
-        --in_flight;
+        __syncwarp();   // the queue is rewritten by the next window
     }
-    bulk_wait<0>();  // all HBM writes complete before the kernel (and its completion event) retires
+    if (lane == 0) {
+        while (in_flight > 0) drain_one();
+    }
+    if (lane == 0) bulk_wait<0>();  // all HBM writes complete before the kernel (and its completion event) retires
 }
 
 constexpr int LDG_UNROLL = 8;                       // 8 x 16 B in flight per lane

@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--host-gib", type=float, default=0.0, help="cap on pinned host KV per rank (GiB); 0 = auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernels", action="store_true", help="skip the batch-32 per-kernel HBM roofline section")
+    ap.add_argument("--section", default="all", choices=["all", "kernels"],
+                    help="kernels: only the per-kernel sections (batch-32 select / attention, prefill selection); used for ncu captures")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
     return ap.parse_args()
 
@@ -426,6 +428,10 @@ def run_sparda(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     assert args.warmup >= 3, "timing rules: at least 3 warm-up steps"
     peaks = load_peaks()
+    if args.section == "kernels":
+        print(json.dumps({"section": "kernels", "roofline_kernels": bench_kernels_b32(torch, binding, peaks, args),
+                          "prefill_select": bench_prefill(torch, binding, peaks)}))
+        return 0
     cfg = workload_config(args)
     cfg = cfg.with_(seed=cfg.seed + 1000 * rank)             # every rank decodes its own sequences
     R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers

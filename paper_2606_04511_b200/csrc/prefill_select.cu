@@ -12,14 +12,17 @@
 // elected thread issues tcgen05.mma (M = 128, N <= 256 per instruction, K = 16 per step) into a 128 x 512 fp32
 // accumulator that fills TMEM.  Causal truncation: a tile only multiplies the N = (m0 + 128)/S columns it can see.
 //
-// The per-row top-k is the real cost (plain ALU): 4 epilogue warps own one TMEM lane quadrant each, one thread per
-// query row, and never leave registers except for a <= 24-entry boundary list:
+// The per-row top-k is the real cost (plain ALU).  4 x PF_NP epilogue warps: the PF_NP warps that share a TMEM lane
+// quadrant hold the same 32 query rows and split each row's 32-column chunks between them (chunk c -> part c % PF_NP),
+// combining per-row partial results through shared memory behind a named barrier.  Per row, all in registers except a
+// <= 24-entry boundary list:
 //   pass 0   row min / max
-//   7 passes bisection over 128 equal-width value buckets of [min, max]: count(s >= t) per pass (2 instr / element)
-//   pass 8   collect the elements of the boundary bucket (value, id); exact k-th (value desc, id asc) among them
-//   pass 9   emit ids with s > T or (s == T and id <= id_T) in ascending id order
-// A row whose boundary bucket holds more than 24 elements (heavy ties) takes an exact bitwise radix search over
-// order-preserving keys instead (33 passes; warp-uniform because tcgen05.ld is warp-collective).
+//   7 passes bisection over 128 equal-width value buckets of [min, max]: count(s >= t) per pass
+//   pass 8   collect the elements of the boundary bucket (value, id); exact k-th by (value desc, id asc) among them
+//   pass 9   selected count per chunk;  pass 10  emit ids with s > T or (s == T and id <= id_T) at the chunk's offset
+// Columns beyond a row's causal candidates read as -inf, so the passes compare values only.  A row whose boundary
+// bucket holds more than 24 elements (heavy ties) takes an exact bitwise radix search over order-preserving keys in
+// part 0 alone (33 passes; warp-uniform because tcgen05.ld is warp-collective), which hands (T, id_T) to the others.
 // Scores never leave the SM.  a7' loops the same MMA over the G heads of the group, turns each head's accumulator
 // into softmax probabilities (two TMEM passes) summed into an L2-resident per-CTA scratch tile, and runs the same
 // selection on that tile.
@@ -29,7 +32,11 @@ namespace {
 
 using namespace sparda;
 
-constexpr int PF_THREADS = 192;   // warp 0: TMA producer, warp 1: TMEM owner + MMA issuer, warps 2-5: epilogue
+#ifndef PF_NP_V
+#define PF_NP_V 4
+#endif
+constexpr int PF_NP = PF_NP_V;    // epilogue warps per TMEM lane quadrant: the threads that share a query row
+constexpr int PF_THREADS = 64 + 128 * PF_NP;   // warp 0: TMA producer, warp 1: TMEM owner + MMA issuer, then 4 * PF_NP epilogue warps
 constexpr int PF_ROWS = 128;      // UMMA M
 constexpr int PF_MAXN = 512;      // TMEM columns = max pooled keys per group
 constexpr int PF_CAP = 24;        // boundary-list capacity per row
@@ -49,7 +56,10 @@ struct PfSmem {
     static constexpr int OFF_LIST = OFF_A + KH * A_SLAB;
     static constexpr int OFF_OUT = OFF_LIST + PF_LIST_WORDS * PF_WSTRIDE * 4;
     static constexpr int OFF_STAT = OFF_OUT + PF_MAXK * PF_OPITCH;          // a7': (m, 1/l) per row, 1 KB
-    static constexpr int OFF_BAR = (OFF_STAT + PF_ROWS * 8 + 7) & ~7;
+    static constexpr int OFF_COMB = OFF_STAT + PF_ROWS * 8;                   // exchange cells: [2][PF_NP][rows] float2
+    static constexpr int OFF_NLIST = OFF_COMB + 2 * PF_NP * PF_ROWS * 8;      // boundary-list length per row
+    static constexpr int OFF_CCNT = OFF_NLIST + PF_ROWS * 4;                  // selected count per (chunk, row), u8
+    static constexpr int OFF_BAR = (OFF_CCNT + (PF_MAXN / 32) * PF_ROWS + 7) & ~7;
     static constexpr int TOTAL = OFF_BAR + 64 + 1024;            // + slack for 1024-byte alignment
 };
 
@@ -76,6 +86,20 @@ __device__ __forceinline__ void tc_commit(uint64_t* bar) {
 }
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// mbarrier wait for a role that waits long (a whole epilogue): back off between polls so the spinning warp does not
+// take issue slots from the warps that work
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity, unsigned ns) {
+    for (;;) {
+        uint32_t ok;
+        asm volatile(
+            "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+        if (ok) break;
+        __nanosleep(ns);
+    }
 }
 // D[tmem] (+)= A[smem desc] * B[smem desc], bf16 x bf16 -> fp32, issued by one thread
 __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
@@ -135,23 +159,61 @@ __device__ __forceinline__ float key_to_float(uint32_t key) {
     return __uint_as_float(key ^ ((key >> 31) ? 0x80000000u : 0xFFFFFFFFu));
 }
 
-// Exact per-row top-k of src[0 .. ncand) for one thread's row; all 32 lanes of the warp call it together
-// (loads are warp-collective), a lane with active == false only keeps the others company.
-// On return the row's k ids (ascending) are staged as u16 at out_base[pos * PF_OPITCH].
+// ---- the PF_NP epilogue warps that share a TMEM lane quadrant (same 32 query rows) split a row's 32-column chunks
+// between them (chunk c belongs to part c % PF_NP) and combine per-row partial results through shared memory:
+// write own partial, named barrier of the quadrant's PF_NP warps, read all parts.  Two buffers alternate, so one
+// barrier per exchange is enough.
+struct PartComm {
+    float2* comb;       // this row's cell of part 0, buffer 0; part stride PF_ROWS, buffer stride PF_NP * PF_ROWS
+    int part, bar_id, buf;
+    __device__ __forceinline__ void sync() const { asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(PF_NP * 32) : "memory"); }
+    __device__ __forceinline__ void put(float2 v) {
+        buf ^= 1;
+        comb[(buf * PF_NP + part) * PF_ROWS] = v;
+        sync();
+    }
+    __device__ __forceinline__ float2 get(int p) const { return comb[(buf * PF_NP + p) * PF_ROWS]; }
+    __device__ __forceinline__ int sum_int(int a) {
+        put(make_float2(__int_as_float(a), 0.f));
+        int s = 0;
+#pragma unroll
+        for (int p = 0; p < PF_NP; ++p) s += __float_as_int(get(p).x);
+        return s;
+    }
+};
+
+// Exact per-row top-k of src[0 .. ncand) for the PF_NP threads that own one query row (one per part); the whole quadrant
+// group calls it together (loads are warp-collective, exchanges are group barriers); a thread with active == false
+// only keeps the others company.  On return the row's k ids (ascending) are staged as u16 at out_base[pos * PF_OPITCH].
 template <class Src>
-__device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int k, bool active, uint32_t* list /* private, stride PF_WSTRIDE */,
-                                         uint8_t* out_base) {
+__device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int k, bool active, PartComm& pc,
+                                         uint32_t* list /* row's list, stride PF_WSTRIDE */, uint32_t* n_list /* row's counter */,
+                                         uint8_t* chunk_cnt /* row's [16] chunk counts, stride PF_ROWS */, uint8_t* out_base) {
     float v[32];
     const float NEG = -INFINITY;
+    const int part = pc.part;
     if (!active) ncand = 0;
+    if (part == 0) *n_list = 0;                       // ordered before the collection by the exchanges below
+    // columns beyond the row's candidates read as -inf (only the last chunk of a warp's rows can hold any), so the
+    // passes below compare values only: no index test per element
+    auto load = [&](int c, float (&x)[32]) {
+        src.load(c, x);
+        if (__any_sync(0xffffffffu, c * 32 + 32 > ncand)) {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) x[e] = c * 32 + e < ncand ? x[e] : NEG;
+        }
+    };
     // ---- pass 0: min / max over the candidates
     float lo = INFINITY, hi = -INFINITY;
-    for (int c = 0; c < nch; ++c) {
+    for (int c = part; c < nch; c += PF_NP) {
         src.load(c, v);
 #pragma unroll
         for (int e = 0; e < 32; ++e)
             if (c * 32 + e < ncand) { lo = fminf(lo, v[e]); hi = fmaxf(hi, v[e]); }
     }
+    pc.put(make_float2(lo, hi));
+#pragma unroll
+    for (int p = 0; p < PF_NP; ++p) { const float2 o = pc.get(p); lo = fminf(lo, o.x); hi = fmaxf(hi, o.y); }
     // ---- bisection over 2^7 equal-width buckets: largest bucket edge t_b with count(s >= t_b) >= k
     const float w = (hi - lo) * (1.0f / (1 << PF_BUCKET_BITS));
     int blo = 0, bhi = 1 << PF_BUCKET_BITS;          // count(s >= t_blo) >= k > count(s >= t_bhi);  t_128 = +inf
@@ -161,109 +223,116 @@ __device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int
         const int mid = (blo + bhi) >> 1;
         const float t = fmaf((float)mid, w, lo);
         int cnt0 = 0, cnt1 = 0;
-        for (int c = 0; c < nch; ++c) {
-            src.load(c, v);
+        for (int c = part; c < nch; c += PF_NP) {
+            load(c, v);
 #pragma unroll
             for (int e = 0; e < 32; e += 2) {
-                cnt0 += (c * 32 + e < ncand && v[e] >= t) ? 1 : 0;
-                cnt1 += (c * 32 + e + 1 < ncand && v[e + 1] >= t) ? 1 : 0;
+                cnt0 += v[e] >= t ? 1 : 0;
+                cnt1 += v[e + 1] >= t ? 1 : 0;
             }
         }
-        const int cnt = cnt0 + cnt1;
+        const int cnt = pc.sum_int(cnt0 + cnt1);
         if (cnt >= k) { blo = mid; c_lo = cnt; } else { bhi = mid; c_hi = cnt; }
     }
     const float tlo = fmaf((float)blo, w, lo);
     const float thi = bhi == (1 << PF_BUCKET_BITS) ? INFINITY : fmaf((float)bhi, w, lo);
     const int need = k - c_hi;                        // how many of the boundary bucket are selected (>= 1)
-    const bool slow = active && (c_lo - c_hi > PF_CAP);
+    const int n_b = c_lo - c_hi;                      // population of the boundary bucket
+    const bool slow = active && (n_b > PF_CAP);
     float T = NEG;                                    // k-th largest value
     int jT = -1;                                      // selected among s == T: ids <= jT
-    bool general = false;                             // needs the tie-aware emission
-    // ---- collect the boundary bucket and resolve it exactly
-    {
-        int n = 0;
-        for (int c = 0; c < nch; ++c) {
-            src.load(c, v);
+    // ---- collect the boundary bucket (any order; entries carry their id) and resolve it exactly
+    for (int c = part; c < nch; c += PF_NP) {
+        load(c, v);
 #pragma unroll
-            for (int e = 0; e < 32; ++e) {
-                const int j = c * 32 + e;
-                if (j < ncand && v[e] >= tlo && v[e] < thi && n < PF_CAP) {
+        for (int e = 0; e < 32; ++e) {
+            const int j = c * 32 + e;
+            if (v[e] >= tlo && v[e] < thi && !slow) {
+                const uint32_t n = atomicAdd(n_list, 1u);
+                if (n < PF_CAP) {
                     list[(2 * n) * PF_WSTRIDE] = __float_as_uint(v[e]);
                     list[(2 * n + 1) * PF_WSTRIDE] = (uint32_t)j;
-                    ++n;
-                }
-            }
-        }
-        if (active && !slow) {
-            // the need-th largest of the list by (value desc, position asc); the list is in ascending id order
-            for (int e = 0; e < n; ++e) {
-                const float se = __uint_as_float(list[(2 * e) * PF_WSTRIDE]);
-                int rank = 0, later_eq = 0;
-                for (int f = 0; f < n; ++f) {
-                    const float sf = __uint_as_float(list[(2 * f) * PF_WSTRIDE]);
-                    rank += (sf > se || (sf == se && f < e)) ? 1 : 0;
-                    later_eq += (sf == se && f > e) ? 1 : 0;
-                }
-                if (rank == need - 1) {
-                    T = se;
-                    jT = (int)list[(2 * e + 1) * PF_WSTRIDE];
-                    general = later_eq > 0;           // an equal element with a larger id stays out
                 }
             }
         }
     }
-    // ---- heavy ties: exact bitwise search of the k-th largest order-preserving key (warp-uniform)
-    int need_eq = 0;
+    pc.sync();
+    if (active && !slow) {
+        // the need-th largest of the list by (value desc, id asc), redundantly in every part
+        for (int e = 0; e < n_b; ++e) {
+            const float se = __uint_as_float(list[(2 * e) * PF_WSTRIDE]);
+            const int je = (int)list[(2 * e + 1) * PF_WSTRIDE];
+            int rank = 0;
+            for (int f = 0; f < n_b; ++f) {
+                const float sf = __uint_as_float(list[(2 * f) * PF_WSTRIDE]);
+                const int jf = (int)list[(2 * f + 1) * PF_WSTRIDE];
+                rank += (sf > se || (sf == se && jf < je)) ? 1 : 0;
+            }
+            if (rank == need - 1) { T = se; jT = je; }
+        }
+    }
+    // ---- heavy ties (rare): part 0 alone searches the k-th largest order-preserving key bit by bit over all chunks, finds
+    // the id of the last equal it takes, and hands (T, jT) to the other parts.  Warp-uniform, and the same in every warp
+    // of the quadrant (they hold the same rows).
     if (__any_sync(0xffffffffu, slow)) {
-        uint32_t tk = 0;
+        if (part == 0) {
+            uint32_t tk = 0;
 #pragma unroll 1
-        for (int bit = 31; bit >= 0; --bit) {
-            const uint32_t cand = tk | (1u << bit);
-            int cnt = 0;
-            for (int c = 0; c < nch; ++c) {
-                src.load(c, v);
+            for (int bit = 31; bit >= 0; --bit) {
+                const uint32_t cand = tk | (1u << bit);
+                int cnt = 0;
+                for (int c = 0; c < nch; ++c) {
+                    load(c, v);
 #pragma unroll
-                for (int e = 0; e < 32; ++e) cnt += (c * 32 + e < ncand && orderable(v[e] + 0.0f) >= cand) ? 1 : 0;
-            }
-            if (cnt >= k) tk = cand;
-        }
-        int cgt = 0;
-        for (int c = 0; c < nch; ++c) {
-            src.load(c, v);
-#pragma unroll
-            for (int e = 0; e < 32; ++e) cgt += (c * 32 + e < ncand && orderable(v[e] + 0.0f) > tk) ? 1 : 0;
-        }
-        if (slow) { T = key_to_float(tk); need_eq = k - cgt; general = true; }
-    }
-    // ---- emit ascending ids
-    int pos = 0;
-    if (__any_sync(0xffffffffu, general)) {
-        int eq_seen = 0;
-        for (int c = 0; c < nch; ++c) {
-            src.load(c, v);
-#pragma unroll
-            for (int e = 0; e < 32; ++e) {
-                const int j = c * 32 + e;
-                if (j < ncand) {
-                    bool sel = v[e] > T;
-                    if (v[e] == T) {
-                        sel = slow ? (eq_seen < need_eq) : (j <= jT);
-                        ++eq_seen;
-                    }
-                    if (sel && pos < PF_MAXK) { *reinterpret_cast<uint16_t*>(out_base + pos * PF_OPITCH) = (uint16_t)j; ++pos; }
+                    for (int e = 0; e < 32; ++e) cnt += (c * 32 + e < ncand && orderable(v[e] + 0.0f) >= cand) ? 1 : 0;
                 }
+                if (cnt >= k) tk = cand;
             }
-        }
-    } else {
-        for (int c = 0; c < nch; ++c) {
-            src.load(c, v);
+            int cgt = 0;
+            for (int c = 0; c < nch; ++c) {
+                load(c, v);
 #pragma unroll
-            for (int e = 0; e < 32; ++e) {
-                const int j = c * 32 + e;
-                if (j < ncand && v[e] >= T && pos < PF_MAXK) { *reinterpret_cast<uint16_t*>(out_base + pos * PF_OPITCH) = (uint16_t)j; ++pos; }
+                for (int e = 0; e < 32; ++e) cgt += (c * 32 + e < ncand && orderable(v[e] + 0.0f) > tk) ? 1 : 0;
+            }
+            int eq_left = k - cgt, j_last = -1;       // take the first k - cgt equals in ascending id
+            for (int c = 0; c < nch; ++c) {
+                load(c, v);
+#pragma unroll
+                for (int e = 0; e < 32; ++e)
+                    if (c * 32 + e < ncand && orderable(v[e] + 0.0f) == tk && eq_left > 0) { j_last = c * 32 + e; --eq_left; }
+            }
+            if (slow) { T = key_to_float(tk); jT = j_last; }
+        }
+        pc.put(make_float2(T, __int_as_float(jT)));
+        if (slow) { const float2 o = pc.get(0); T = o.x; jT = __float_as_int(o.y); }
+    }
+    // ---- selected element: s > T, or s == T with id <= jT (+-0 compare equal, as in the oracle's ordering).  Count per
+    // chunk, exchange, then emit every chunk at its offset: ascending ids.
+    for (int c = part; c < nch; c += PF_NP) {
+        load(c, v);
+        int n = 0;
+#pragma unroll
+        for (int e = 0; e < 32; ++e) {
+            const int j = c * 32 + e;
+            n += (v[e] > T || (v[e] == T && j <= jT)) ? 1 : 0;
+        }
+        chunk_cnt[c * PF_ROWS] = (uint8_t)n;
+    }
+    pc.sync();
+    for (int c = part; c < nch; c += PF_NP) {
+        int pos = 0;
+        for (int cc = 0; cc < c; ++cc) pos += chunk_cnt[cc * PF_ROWS];
+        load(c, v);
+#pragma unroll
+        for (int e = 0; e < 32; ++e) {
+            const int j = c * 32 + e;
+            if ((v[e] > T || (v[e] == T && j <= jT)) && pos < PF_MAXK) {
+                *reinterpret_cast<uint16_t*>(out_base + pos * PF_OPITCH) = (uint16_t)j;
+                ++pos;
             }
         }
     }
+    pc.sync();   // the staged ids of the row are complete
 }
 
 template <int D, bool BASELINE>
@@ -292,7 +361,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
         mbar_init(a_full, 1);
         mbar_init(a_empty, 1);
         mbar_init(mma_done, 1);
-        mbar_init(tmem_empty, 4);
+        mbar_init(tmem_empty, 4 * PF_NP);
         mbar_fence_init();
         fence_proxy_async_smem();
         tma_prefetch_desc(&tmapA);
@@ -326,7 +395,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 const int mt = tile_of_round(r);
                 if (mt < 0 || tile_ncols(mt) <= p.topk) continue;   // nothing to rank: every candidate is selected
                 for (int h = 0; h < NH; ++h, ++it) {
-                    mbar_wait(a_empty, (it & 1) ^ 1);
+                    mbar_wait_backoff(a_empty, (it & 1) ^ 1, 400);
                     mbar_arrive_expect_tx(a_full, (uint32_t)(KH * SM::A_SLAB));
                     const int arow = (BASELINE ? (g * p.G + h) : g) * p.T + mt * PF_ROWS;
                     for (int kh = 0; kh < KH; ++kh) tma_load_2d(smem + SM::OFF_A + kh * SM::A_SLAB, &tmapA, kh * 64, arow, a_full);
@@ -344,8 +413,8 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 if (mt < 0 || tile_ncols(mt) <= p.topk) continue;
                 const int ncols = (tile_ncols(mt) + 15) & ~15;
                 for (int h = 0; h < NH; ++h, ++it) {
-                    mbar_wait(a_full, it & 1);
-                    mbar_wait(tmem_empty, (it & 1) ^ 1);
+                    mbar_wait_backoff(a_full, it & 1, 100);
+                    mbar_wait_backoff(tmem_empty, (it & 1) ^ 1, 200);
                     tc_fence_after();
                     for (int nh = 0; nh * 256 < ncols; ++nh) {
                         const int n = min(256, ncols - nh * 256);
@@ -363,12 +432,15 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
             }
         }
     } else {
-        // =============================== epilogue: one thread per query row ===============================
+        // =============================== epilogue: PF_NP threads per query row ===============================
         const int q = warp & 3;                                  // TMEM lane quadrant this warp may access
+        const int part = (warp - 2) >> 2;                        // which share of the row's chunks this warp takes
         const int trow = q * 32 + lane;                          // row within the tile
         uint32_t* list = reinterpret_cast<uint32_t*>(smem + SM::OFF_LIST) + trow;
         uint8_t* out_base = smem + SM::OFF_OUT + trow * 2;
-        float2* stat = reinterpret_cast<float2*>(smem + SM::OFF_STAT) + trow;
+        uint32_t* n_list = reinterpret_cast<uint32_t*>(smem + SM::OFF_NLIST) + trow;
+        uint8_t* chunk_cnt = smem + SM::OFF_CCNT + trow;
+        PartComm pc{reinterpret_cast<float2*>(smem + SM::OFF_COMB) + trow, part, 1 + q, 0};
         float* scr = BASELINE ? p.scratch + (size_t)blockIdx.x * PF_MAXN * PF_ROWS + trow : nullptr;
         const TmemRow trsrc{tmem_base + ((uint32_t)(q * 32) << 16)};
         uint32_t it = 0;
@@ -380,9 +452,11 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
             const int ncand = min(p.n_blocks, (i + 1) / 64);
             int32_t* dst = p.ids + ((size_t)g * p.n_rows + (i - p.row0)) * p.topk;
             const int ncols = tile_ncols(mt);
+            // this part's share of the row's k output positions
+            const int s_lo = part * ((p.topk + PF_NP - 1) / PF_NP), s_hi = min(p.topk, s_lo + (p.topk + PF_NP - 1) / PF_NP);
             if (ncols <= p.topk) {                               // whole tile: every candidate is selected (reading q5)
                 if (in_chunk)
-                    for (int s = 0; s < p.topk; ++s) dst[s] = s < ncand ? s : -1;
+                    for (int s = s_lo; s < s_hi; ++s) dst[s] = s < ncand ? s : -1;
                 continue;
             }
             const int wmax = min(p.n_blocks, (mt * PF_ROWS + q * 32 + 32) / 64);   // candidates of the warp's last row
@@ -392,25 +466,32 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 // a7': per head, softmax over the causal candidates of the row, summed into the scratch tile
                 float v[32];
                 for (int h = 0; h < NH; ++h, ++it) {
-                    mbar_wait(mma_done, it & 1);
+                    mbar_wait_backoff(mma_done, it & 1, 100);
                     tc_fence_after();
                     float m = -INFINITY;
-                    for (int c = 0; c < nch; ++c) {
+                    for (int c = part; c < nch; c += PF_NP) {
                         trsrc.load(c, v);
 #pragma unroll
                         for (int e = 0; e < 32; ++e)
                             if (c * 32 + e < ncand) m = fmaxf(m, v[e]);
                     }
+                    pc.put(make_float2(m, 0.f));
+#pragma unroll
+                    for (int pp = 0; pp < PF_NP; ++pp) m = fmaxf(m, pc.get(pp).x);
                     const float ms = m * p.scale_log2;
                     float l = 0.f;
-                    for (int c = 0; c < nch; ++c) {
+                    for (int c = part; c < nch; c += PF_NP) {
                         trsrc.load(c, v);
 #pragma unroll
                         for (int e = 0; e < 32; ++e)
                             if (c * 32 + e < ncand) l += exp2f(fmaf(v[e], p.scale_log2, -ms));
                     }
+                    pc.put(make_float2(l, 0.f));
+                    l = 0.f;
+#pragma unroll
+                    for (int pp = 0; pp < PF_NP; ++pp) l += pc.get(pp).x;   // same order in every part
                     const float inv = ncand > 0 ? 1.0f / l : 0.f;
-                    for (int c = 0; c < nch; ++c) {
+                    for (int c = part; c < nch; c += PF_NP) {
                         trsrc.load(c, v);
 #pragma unroll
                         for (int e = 0; e < 32; ++e) {
@@ -426,32 +507,22 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     __syncwarp();
                     if (lane == 0) mbar_arrive(tmem_empty);
                 }
-                (void)stat;
-                if (__any_sync(0xffffffffu, ranked)) row_topk(ScratchRow{scr}, ncand, nch, p.topk, ranked, list, out_base);
+                if (__any_sync(0xffffffffu, ranked))
+                    row_topk(ScratchRow{scr}, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, out_base);
             } else {
-                mbar_wait(mma_done, it & 1);
+                mbar_wait_backoff(mma_done, it & 1, 100);
                 ++it;
                 tc_fence_after();
-                if (__any_sync(0xffffffffu, ranked)) row_topk(trsrc, ncand, nch, p.topk, ranked, list, out_base);
+                if (__any_sync(0xffffffffu, ranked))
+                    row_topk(trsrc, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, out_base);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(tmem_empty);
             }
             if (ranked) {
-                if ((p.topk & 3) == 0) {
-                    for (int s = 0; s < p.topk; s += 4) {
-                        int4 o;
-                        o.x = *reinterpret_cast<const uint16_t*>(out_base + (s + 0) * PF_OPITCH);
-                        o.y = *reinterpret_cast<const uint16_t*>(out_base + (s + 1) * PF_OPITCH);
-                        o.z = *reinterpret_cast<const uint16_t*>(out_base + (s + 2) * PF_OPITCH);
-                        o.w = *reinterpret_cast<const uint16_t*>(out_base + (s + 3) * PF_OPITCH);
-                        *reinterpret_cast<int4*>(dst + s) = o;
-                    }
-                } else {
-                    for (int s = 0; s < p.topk; ++s) dst[s] = *reinterpret_cast<const uint16_t*>(out_base + s * PF_OPITCH);
-                }
+                for (int s = s_lo; s < s_hi; ++s) dst[s] = *reinterpret_cast<const uint16_t*>(out_base + s * PF_OPITCH);
             } else if (in_chunk) {
-                for (int s = 0; s < p.topk; ++s) dst[s] = s < ncand ? s : -1;
+                for (int s = s_lo; s < s_hi; ++s) dst[s] = s < ncand ? s : -1;
             }
         }
     }

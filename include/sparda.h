@@ -167,6 +167,12 @@ int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_l
 int sparda_reuse_plan(sparda_ctx* ctx, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch,
                       int32_t* n_fetch, void* stream);
 
+/* sparda_forecast_select followed by sparda_reuse_plan on its result, in ONE launch: the CTA that selects a row also
+ * updates the row's slot table and fetch list (same results as the two calls; saves a launch per layer of the cached
+ * decode step).  Arguments as in the two calls.                                                                   */
+int sparda_forecast_select_plan(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
+                                int32_t* ids_out, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch, void* stream);
+
 /* One decoder layer of sparda_decode_step_cached: sparda_layer plus the layer's persistent pool and slot table.   */
 typedef struct {
     sparda_layer base;   /* as in sparda_decode_step                                                             */
@@ -177,7 +183,7 @@ typedef struct {
 } sparda_cached_layer;
 
 /* sparda_decode_step with the previous step's blocks kept per layer: per layer l >= 1 the compute stream
- * runs select B_{l+1} -> reuse_plan -> [prefetch stream: gather only the missing blocks into layer l+1's own pool] ->
+ * runs select B_{l+1} + reuse plan (one launch) -> [prefetch stream: gather only the missing blocks into layer l+1's own pool] ->
  * wait for layer l's gather -> attention over pool_l in slot order.  Layer 0 attends from its resident cache as
  * before.  Same modes, same capture rules; with every slot_ids at -1 the step moves exactly the bytes of
  * sparda_decode_step.                                                                                           */

@@ -20,7 +20,7 @@ STEP_OVERLAP, STEP_SERIAL = 0, 1
 EXPORTS = [
     "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_select", "sparda_prefetch_launch",
     "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
-    "sparda_reuse_plan", "sparda_decode_step_cached",
+    "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
     "sparda_launch_count", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
     "sparda_last_cuda_error", "sparda_version",
@@ -68,6 +68,7 @@ def lib() -> ctypes.CDLL:
         L.sparda_decode_step.argtypes = [vp, ctypes.POINTER(SpardaLayer), i32, vp, i32, i32, vp, vp, vp, vp, i32]
         L.sparda_decode_step_host.argtypes = L.sparda_decode_step.argtypes
         L.sparda_reuse_plan.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+        L.sparda_forecast_select_plan.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp]
         L.sparda_decode_step_cached.argtypes = [vp, ctypes.POINTER(SpardaCachedLayer), i32, vp, i32, i32, vp, vp, i32]
         L.sparda_profile_enable.argtypes = [vp, i32]
         L.sparda_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
@@ -180,6 +181,12 @@ class Sparda:
     def reuse_plan(self, ids_new, topk, slot_ids, fetch, n_fetch=None, stream=None):
         self._check(self._L.sparda_reuse_plan(self._h, _ptr(ids_new), topk, _ptr(slot_ids), _ptr(fetch),
                                               _ptr(n_fetch) if n_fetch is not None else None, _stream(stream)), "reuse_plan")
+
+    def forecast_select_plan(self, F, Kpool, n_blocks, topk, ids_out, slot_ids, fetch, n_fetch=None, n_cand=None, stream=None):
+        n_cand = n_blocks if n_cand is None else n_cand
+        self._check(self._L.sparda_forecast_select_plan(self._h, _ptr(F), _ptr(Kpool), n_blocks, n_cand, topk, _ptr(ids_out),
+                                                        _ptr(slot_ids), _ptr(fetch), _ptr(n_fetch) if n_fetch is not None else None,
+                                                        _stream(stream)), "forecast_select_plan")
 
     def make_cached_layers(self, layers):
         """layers: list of dicts with tensors F, Q, Kpool, kv, O, ids and (layers >= 1) pool, slot_ids, fetch, n_fetch."""

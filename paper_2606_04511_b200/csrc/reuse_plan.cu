@@ -16,87 +16,26 @@
 // lowest slot as its owner (so a duplicated resident block, which this kernel never produces, is still resolved as
 // the oracle does), two ballot compactions list the freed slots and the missing blocks in ascending order.
 #include "sparda_internal.cuh"
+#include "reuse_plan.cuh"
 
 namespace {
 
+using namespace sparda;
+
 constexpr int RP_WARPS = 4;
-constexpr int RP_MAXK = 256;
 
 __global__ void __launch_bounds__(RP_WARPS * 32) reuse_plan_kernel(const int32_t* __restrict__ ids_new, int32_t* __restrict__ slot_ids,
                                                                     int32_t* __restrict__ fetch, int32_t* __restrict__ n_fetch,
                                                                     int n_rows, int k) {
-    __shared__ int32_t s_new[RP_WARPS][RP_MAXK];
-    __shared__ int32_t s_owner[RP_WARPS][RP_MAXK];
-    __shared__ int16_t s_free[RP_WARPS][RP_MAXK], s_miss[RP_WARPS][RP_MAXK];
+    __shared__ ReusePlanScratch sc[RP_WARPS];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int r = blockIdx.x * RP_WARPS + w;
     if (r >= n_rows) return;
-    const unsigned lt = (1u << lane) - 1u;
-    int32_t* nw = s_new[w];
-    int32_t* owner = s_owner[w];
-    const int32_t* in = ids_new + (size_t)r * k;
-    int32_t* slots = slot_ids + (size_t)r * k;
-    int32_t* fo = fetch + (size_t)r * k;
-
-    int m = 0;   // valid entries of the selection (ascending, then -1 padding)
-    for (int c = 0; c < k; c += 32) {
-        const int i = c + lane;
-        const int32_t v = i < k ? in[i] : -1;
-        if (i < k) { nw[i] = v; owner[i] = 0x7fffffff; }
-        m += __popc(__ballot_sync(0xffffffffu, v >= 0));
-    }
-    __syncwarp();
-    // hits: resident blocks that are selected again
-    for (int c = 0; c < k; c += 32) {
-        const int s = c + lane;
-        const int32_t b = s < k ? slots[s] : -1;
-        if (b >= 0) {
-            int lo = 0, hi = m;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (nw[mid] < b) lo = mid + 1; else hi = mid;
-            }
-            if (lo < m && nw[lo] == b) atomicMin(&owner[lo], s);
-        }
-    }
-    __syncwarp();
-    // freed slots (ascending) and missing blocks (ascending position = ascending id)
-    int n_free = 0, n_miss = 0;
-    for (int c = 0; c < k; c += 32) {
-        const int s = c + lane;
-        bool kept = false;
-        if (s < k) {
-            const int32_t b = slots[s];
-            if (b >= 0) {
-                int lo = 0, hi = m;
-                while (lo < hi) {
-                    const int mid = (lo + hi) >> 1;
-                    if (nw[mid] < b) lo = mid + 1; else hi = mid;
-                }
-                kept = lo < m && nw[lo] == b && owner[lo] == s;
-            }
-        }
-        const unsigned fb = __ballot_sync(0xffffffffu, s < k && !kept);
-        if (s < k && !kept) s_free[w][n_free + __popc(fb & lt)] = (int16_t)s;
-        n_free += __popc(fb);
-        const bool miss = s < m && owner[s] == 0x7fffffff;
-        const unsigned mb = __ballot_sync(0xffffffffu, miss);
-        if (miss) s_miss[w][n_miss + __popc(mb & lt)] = (int16_t)s;
-        n_miss += __popc(mb);
-        if (s < k && kept) fo[s] = -1;
-    }
-    __syncwarp();
-    for (int j = lane; j < n_free; j += 32) {
-        const int s = s_free[w][j];
-        const int32_t b = j < n_miss ? nw[s_miss[w][j]] : -1;
-        slots[s] = b;
-        fo[s] = b;
-    }
+    const int n_miss = reuse_plan_row(ids_new + (size_t)r * k, slot_ids + (size_t)r * k, fetch + (size_t)r * k, k, sc[w], lane);
     if (lane == 0 && n_fetch) n_fetch[r] = n_miss;
 }
 
 }  // namespace
-
 int sparda_launch_reuse_plan(sparda_ctx* ctx, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch,
                              int32_t* n_fetch, cudaStream_t st) {
     if (topk > RP_MAXK) return SPARDA_EINVAL;

@@ -15,6 +15,7 @@
 // exactly "sort by (score desc, id asc), take k, sort by id".  Scores never touch global memory; there is no
 // ticket, no fence and no scratch.  HBM-bound: R*n_cand*D*2 bytes of Kpool.
 #include "sparda_internal.cuh"
+#include "reuse_plan.cuh"
 
 #ifdef SPARDA_TRACE
 __device__ unsigned long long* g_sel_trace;   // [gridDim.x][16] globaltimer stamps (debug builds only)
@@ -258,6 +259,11 @@ struct SelParams {
     int32_t* ids;
     int n_blocks, n_cand, topk;
     int per;   // pooled keys per CTA of the cluster (the last CTA's range may be shorter or empty)
+    // optional fused reuse plan (f1, reuse_plan.cuh): after the row's ids are out, one warp of the selecting CTA updates
+    // the row's slot table and fetch list -- one launch less per layer of the cached decode step
+    int32_t* slot_ids;
+    int32_t* fetch;
+    int32_t* n_fetch;
 };
 
 template <int D>
@@ -275,6 +281,7 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
     __shared__ uint32_t s_bcast[4];
     __shared__ uint32_t s_cand[2 * SEL_CAND_CAP];
     __shared__ uint32_t s_mm[2][SEL_MAX_CS * NW];    // per (CTA of the cluster, warp): min / max key; lives in CTA 0
+    __shared__ ReusePlanScratch s_plan;
 
     uint8_t* ring = (uint8_t*)(((uintptr_t)sel_smem_raw + 127) & ~(uintptr_t)127);
     uint32_t* s_keys = reinterpret_cast<uint32_t*>(ring + SEL_STAGES * SEL_STAGE_BYTES);   // [n_cand], used in CTA 0
@@ -287,8 +294,16 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
     int32_t* ids_row = p.ids + (size_t)r * p.topk;
 
     if (p.n_cand <= p.topk) {  // every candidate is selected (reading q5); no scoring needed
-        if (c == 0)
+        if (c == 0) {
             for (int i = tid; i < p.topk; i += SEL_CTA_THREADS) ids_row[i] = i < p.n_cand ? i : -1;
+            if (p.slot_ids) {
+                __syncthreads();
+                if (w == 0) {
+                    const int nm = reuse_plan_row(ids_row, p.slot_ids + (size_t)r * p.topk, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
+                    if (lane == 0 && p.n_fetch) p.n_fetch[r] = nm;
+                }
+            }
+        }
         return;
     }
 
@@ -397,6 +412,13 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
     kmax = __reduce_max_sync(0xffffffffu, kmax);
     topk_emit(s_keys, p.n_cand, p.topk, kmin, kmax, ids_row, s_hist, s_wtot, s_bcast, s_cand);
     SEL_TRACE(3);
+    if (p.slot_ids) {
+        consumer_sync();   // the row's ids are in global memory (read back through L2)
+        if (w == 0) {
+            const int nm = reuse_plan_row(ids_row, p.slot_ids + (size_t)r * p.topk, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
+            if (lane == 0 && p.n_fetch) p.n_fetch[r] = nm;
+        }
+    }
 }
 
 // a0: Kpool[r,j,d] = bf16( (1/S) sum_t K[r,j,t,d] ), fp32 sum in ascending t (Eq.2, kernel = stride = S).
@@ -441,11 +463,11 @@ static int select_launch(sparda_ctx* ctx, const SelParams& p0, cudaStream_t st) 
     static int cluster_ok[SEL_MAX_CS + 1];   // 0 = not asked, 1 = schedulable, -1 = not
     const size_t smem_max = 127 + (size_t)SEL_STAGES * SEL_STAGE_BYTES + (size_t)ctx->cfg.max_blocks * sizeof(uint32_t);
     if (!attr_set) {
-        SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 4096));
+        SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 8192));
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         attr_set = true;
     }
-    if (smem_max > 227 * 1024 - 4096) return SPARDA_EINVAL;
+    if (smem_max > 227 * 1024 - 8192) return SPARDA_EINVAL;
     SelParams p = p0;
     const size_t smem = 127 + (size_t)SEL_STAGES * SEL_STAGE_BYTES + (size_t)(p.n_cand > p.topk ? p.n_cand : 0) * sizeof(uint32_t);
     cudaLaunchConfig_t lc = {};
@@ -480,8 +502,12 @@ static int select_launch(sparda_ctx* ctx, const SelParams& p0, cudaStream_t st) 
 }
 
 int sparda_launch_select(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
-                         int32_t* ids, cudaStream_t st) {
+                         int32_t* ids, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch, cudaStream_t st) {
+    if (slot_ids && topk > RP_MAXK) return SPARDA_EINVAL;
     SelParams p;
+    p.slot_ids = slot_ids;
+    p.fetch = fetch;
+    p.n_fetch = n_fetch;
     p.F = (const uint4*)F;
     p.Kpool = (const char*)Kpool;
     p.ids = ids;

@@ -148,7 +148,16 @@ int sparda_forecast_select(sparda_ctx* ctx, const void* F, const void* Kpool, in
     if (!ctx || !sparda_aligned(F, 16) || !sparda_aligned(Kpool, 16) || !sparda_aligned(ids_out, 4)) return SPARDA_EINVAL;
     if (n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || n_cand < 0 || n_cand > n_blocks) return SPARDA_EINVAL;
     if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
-    return sparda_launch_select(ctx, F, Kpool, n_blocks, n_cand, topk, ids_out, (cudaStream_t)stream);
+    return sparda_launch_select(ctx, F, Kpool, n_blocks, n_cand, topk, ids_out, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int sparda_forecast_select_plan(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
+                                int32_t* ids_out, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch, void* stream) {
+    if (!ctx || !sparda_aligned(F, 16) || !sparda_aligned(Kpool, 16) || !sparda_aligned(ids_out, 4)) return SPARDA_EINVAL;
+    if (!sparda_aligned(slot_ids, 4) || !sparda_aligned(fetch, 4) || (n_fetch && !sparda_aligned(n_fetch, 4))) return SPARDA_EINVAL;
+    if (n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || n_cand < 0 || n_cand > n_blocks) return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    return sparda_launch_select(ctx, F, Kpool, n_blocks, n_cand, topk, ids_out, slot_ids, fetch, n_fetch, (cudaStream_t)stream);
 }
 
 int sparda_prefetch_launch(sparda_ctx* ctx, const void* host_kv, int n_blocks, const int32_t* ids, int topk,
@@ -275,9 +284,8 @@ int sparda_decode_step_cached(sparda_ctx* ctx, const sparda_cached_layer* layers
         if (l + 1 < n_layers) {
             const sparda_cached_layer* nx = &layers[l + 1];
             SPARDA_PROF_BEGIN(0, cs);
-            rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, cs);
-            if (rc) return rc;
-            rc = sparda_reuse_plan(ctx, nx->base.ids, topk, nx->slot_ids, nx->fetch, nx->n_fetch, cs);
+            rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids,
+                                             nx->slot_ids, nx->fetch, nx->n_fetch, cs);   // select + plan in one launch
             if (rc) return rc;
             SPARDA_PROF_END(0, cs);
             if (ps != cs) {

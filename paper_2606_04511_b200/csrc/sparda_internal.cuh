@@ -60,7 +60,8 @@ static inline bool sparda_aligned(const void* p, uintptr_t a) { return p != null
 // launchers implemented in the kernel translation units
 int sparda_launch_pool_keys(sparda_ctx*, const void* kv, int64_t n_rows, int n_blocks, void* kpool, cudaStream_t);
 int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
-                         int32_t* ids, cudaStream_t);
+                         int32_t* ids, int32_t* slot_ids /* optional fused reuse plan */, int32_t* fetch, int32_t* n_fetch,
+                         cudaStream_t);
 int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
                          cudaStream_t);
 int sparda_launch_reuse_plan(sparda_ctx*, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch,

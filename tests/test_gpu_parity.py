@@ -353,6 +353,33 @@ def test_reuse_plan_matches_oracle(sp, oracle):
         np.testing.assert_array_equal(nf.cpu().numpy(), (want_fetch >= 0).sum(1))
 
 
+@pytest.mark.parametrize("cfg", [MID, MID64, G16], ids=lambda c: c.name)
+def test_forecast_select_plan_equals_select_then_plan(cfg, sp, oracle):
+    """The fused launch (select + reuse plan in the selecting CTA) gives bit-identical ids, slot tables, fetch lists and
+    counts to the two separate launches, over drifting Forecasts and including the n_cand <= k shortcut."""
+    L, ctx, kpool = _setup(cfg, sp)
+    R, k, Nb = cfg.rows, cfg.topk, cfg.n_blocks
+    g = torch.Generator(device="cuda").manual_seed(5)
+    slot_a = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
+    slot_b = slot_a.clone()
+    for t, n_cand in enumerate([Nb, Nb, Nb - 3, k, Nb, max(k - 2, 1), Nb]):
+        F = (L["F"].float() + 0.4 * t * torch.randn(L["F"].shape, generator=g, device="cuda")).to(torch.bfloat16)
+        ids_a = torch.full((R, k), -7, dtype=torch.int32, device="cuda")
+        ids_b = ids_a.clone()
+        fa, fb = torch.full((R, k), -7, dtype=torch.int32, device="cuda"), torch.full((R, k), -7, dtype=torch.int32, device="cuda")
+        na, nb = torch.full((R,), -7, dtype=torch.int32, device="cuda"), torch.full((R,), -7, dtype=torch.int32, device="cuda")
+        ctx.forecast_select(F, kpool, Nb, k, ids_a, n_cand=n_cand)
+        ctx.reuse_plan(ids_a, k, slot_a, fa, na)
+        ctx.forecast_select_plan(F, kpool, Nb, k, ids_b, slot_b, fb, nb, n_cand=n_cand)
+        torch.cuda.synchronize()
+        for x, y in ((ids_a, ids_b), (slot_a, slot_b), (fa, fb), (na, nb)):
+            assert torch.equal(x, y), f"step {t}"
+        want_after, want_fetch = oracle.reuse_plan(ids_a.cpu().numpy(), prev if t else np.full((R, k), -1, dtype=np.int32))
+        np.testing.assert_array_equal(slot_b.cpu().numpy(), want_after)
+        np.testing.assert_array_equal(fb.cpu().numpy(), want_fetch)
+        prev = want_after
+
+
 @pytest.mark.parametrize("cfg", [synth.CFG1_TINY.with_(n_layers=4), G16.with_(n_layers=3, batch=3)], ids=lambda c: c.name)
 def test_decode_step_cached_multi_step(cfg, sp, oracle):
     """Several decode steps with the per-layer block cache (f1) while the Forecast drifts: every step the slot

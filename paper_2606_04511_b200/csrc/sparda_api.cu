@@ -89,11 +89,14 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
               cudaMemset(ctx->tickets, 0, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
     ctx->ev_gather = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
+    ctx->ev_top = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
     ctx->ev_prof = (cudaEvent_t*)calloc((size_t)3 * (ctx->max_layers + 1) * 2, sizeof(cudaEvent_t));
-    ok = ok && ctx->ev_sel && ctx->ev_gather && ctx->ev_prof;
+    ok = ok && ctx->ev_sel && ctx->ev_gather && ctx->ev_top && ctx->ev_prof &&
+         cudaStreamCreateWithFlags(&ctx->select_stream, cudaStreamNonBlocking) == cudaSuccess;
     for (int i = 0; ok && i <= ctx->max_layers; ++i)
         ok = cudaEventCreateWithFlags(&ctx->ev_sel[i], cudaEventDisableTiming) == cudaSuccess &&
-             cudaEventCreateWithFlags(&ctx->ev_gather[i], cudaEventDisableTiming) == cudaSuccess;
+             cudaEventCreateWithFlags(&ctx->ev_gather[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&ctx->ev_top[i], cudaEventDisableTiming) == cudaSuccess;
     for (int i = 0; ok && i < 3 * (ctx->max_layers + 1) * 2; ++i) ok = cudaEventCreate(&ctx->ev_prof[i]) == cudaSuccess;
     const size_t f_bytes = (size_t)ctx->R * D * 2, q_bytes = (size_t)cfg->batch * cfg->n_q_heads * D * 2;
     ok = ok && cudaMalloc(&ctx->stage_F, f_bytes * (ctx->max_layers + 1)) == cudaSuccess &&
@@ -123,6 +126,7 @@ int sparda_destroy(sparda_ctx* ctx) {
     for (int i = 0; i <= ctx->max_layers; ++i) {
         if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);
         if (ctx->ev_gather && ctx->ev_gather[i]) cudaEventDestroy(ctx->ev_gather[i]);
+        if (ctx->ev_top && ctx->ev_top[i]) cudaEventDestroy(ctx->ev_top[i]);
     }
     for (int i = 0; ctx->ev_prof && i < 3 * (ctx->max_layers + 1) * 2; ++i)
         if (ctx->ev_prof[i]) cudaEventDestroy(ctx->ev_prof[i]);
@@ -131,6 +135,8 @@ int sparda_destroy(sparda_ctx* ctx) {
     cudaFree(ctx->stage_O);
     free(ctx->ev_sel);
     free(ctx->ev_gather);
+    free(ctx->ev_top);
+    if (ctx->select_stream) cudaStreamDestroy(ctx->select_stream);
     free(ctx->ev_prof);
     (void)cudaGetLastError();
     delete ctx;
@@ -192,11 +198,17 @@ int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* K
     return sparda_launch_prefill_baseline(ctx, Q, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, (cudaStream_t)stream);
 }
 
-// Algorithm 2, lines 4-7, for n_layers layers.  Compute-stream order per layer l:
-//   select B_{l+1} (F_l vs Kpool_{l+1})  ->  record ev_sel[l+1]  ->  [prefetch stream: wait, gather, record ev_gather[l+1]]
-//   ->  wait ev_gather[l]  ->  attention l.
-// Buffer hand-off (double-buffered pool): gather l+1 writes pool[(l+1)&1], last read by attention l-1, which
-// precedes select B_{l+1} on the compute stream, so ev_sel[l+1] also releases the buffer.
+// Algorithm 2, lines 4-7, for n_layers layers, plain (double-buffered pool, every block fetched) or with the
+// previous step's blocks kept per layer.  Given layer l's projections, line 4 (select B_{l+1}) and line 7
+// (attention l) do not depend on each other, so in overlap mode they run concurrently on two streams; the prefetch has
+// its own:
+//   compute stream  cs:  record ev_top[l]  ->  wait ev_gather[l]  ->  attention l
+//   select stream   ss:  wait ev_top[l]    ->  select B_{l+1} (+ reuse plan)  ->  record ev_sel[l+1]
+//   prefetch stream ps:  wait ev_sel[l+1]  ->  gather B_{l+1}  ->  record ev_gather[l+1]
+// ev_top[l] follows attention l-1 on cs, so a select never runs more than one layer ahead of the attention (in a model,
+// F_l exists only once layer l-1 is complete) and it releases the buffers gather l+1 writes: pool[(l+1)&1] was last read
+// by attention l-1 (plain); pool_{l+1} and slot_ids_{l+1} by attention l+1 of the previous step (cached).  The step ends
+// with cs joined to ss.  Serial mode: the same kernels on cs in Algorithm-2 order.
 // timing events around one launch of `kind` (0 select, 1 gather, 2 attention) on stream st
 static inline cudaEvent_t* prof_slot(sparda_ctx* ctx, int kind) {
     return &ctx->ev_prof[((size_t)kind * (ctx->max_layers + 1) + ctx->prof_n[kind]) * 2];
@@ -209,50 +221,77 @@ static inline cudaEvent_t* prof_slot(sparda_ctx* ctx, int kind) {
         ctx->prof_n[kind]++;                                                    \
     }
 
+static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur, int n_blocks,
+                            int topk, cudaStream_t cs, cudaStream_t ps_in, int mode) {
+    const bool overlap = mode == SPARDA_STEP_OVERLAP;
+    cudaStream_t ps = overlap ? ps_in : cs;
+    cudaStream_t ss = overlap ? ctx->select_stream : cs;
+    int rc;
+    ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
+    // layer 0: same-layer selection with F0cur; its attention needs it, so it stays on the compute stream
+    SPARDA_PROF_BEGIN(0, cs);
+    rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_blocks, topk, layers[0].base.ids, cs);
+    if (rc) return rc;
+    SPARDA_PROF_END(0, cs);
+    for (int l = 0; l < n_layers; ++l) {
+        if (l + 1 < n_layers) {
+            const sparda_cached_layer* nx = &layers[l + 1];
+            if (overlap) {
+                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_top[l], cs));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ss, ctx->ev_top[l], 0));
+            }
+            SPARDA_PROF_BEGIN(0, ss);
+            if (nx->slot_ids)   // select + reuse plan in one launch
+                rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids,
+                                                 nx->slot_ids, nx->fetch, nx->n_fetch, ss);
+            else
+                rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, ss);
+            if (rc) return rc;
+            SPARDA_PROF_END(0, ss);
+            if (overlap) {
+                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], ss));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ps, ctx->ev_sel[l + 1], 0));
+            }
+            SPARDA_PROF_BEGIN(1, ps);
+            rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->slot_ids ? nx->fetch : nx->base.ids, topk, nx->pool, ps);
+            if (rc) return rc;
+            SPARDA_PROF_END(1, ps);
+            if (overlap) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], ps));
+        }
+        if (l == 0) {
+            SPARDA_PROF_BEGIN(2, cs);
+            rc = sparda_sparse_decode(ctx, layers[0].base.Q, layers[0].base.kv, layers[0].base.ids, topk, 1, n_blocks, layers[0].base.O, cs);
+        } else {
+            if (overlap) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
+            SPARDA_PROF_BEGIN(2, cs);
+            rc = sparda_sparse_decode(ctx, layers[l].base.Q, layers[l].pool, layers[l].slot_ids ? layers[l].slot_ids : layers[l].base.ids,
+                                      topk, 0, topk, layers[l].base.O, cs);
+        }
+        if (rc) return rc;
+        SPARDA_PROF_END(2, cs);
+    }
+    // every select has been consumed by a gather that an attention waited for, so cs already follows all work of ss and
+    // ps; the explicit join keeps that true for n_layers == 1 and makes the step capturable (all forks rejoin cs)
+    if (overlap && n_layers > 1) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_sel[n_layers - 1], 0));
+    return SPARDA_OK;
+}
+
 int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                        int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
                        int mode) {
     if (!ctx || !layers || n_layers < 1 || n_layers > ctx->max_layers || !F0cur) return SPARDA_EINVAL;
     if (mode != SPARDA_STEP_OVERLAP && mode != SPARDA_STEP_SERIAL) return SPARDA_EINVAL;
     if (n_layers > 1 && (!dev_pool0 || !dev_pool1)) return SPARDA_EINVAL;
-    cudaStream_t cs = (cudaStream_t)compute_stream;
-    cudaStream_t ps = mode == SPARDA_STEP_OVERLAP ? (cudaStream_t)prefetch_stream : cs;
     void* pools[2] = {dev_pool0, dev_pool1};
-    int rc;
-    ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
-    // layer 0: same-layer selection with F0cur
-    SPARDA_PROF_BEGIN(0, cs);
-    rc = sparda_forecast_select(ctx, F0cur, layers[0].Kpool, n_blocks, n_blocks, topk, layers[0].ids, cs);
-    if (rc) return rc;
-    SPARDA_PROF_END(0, cs);
+    sparda_cached_layer* cl = (sparda_cached_layer*)alloca(sizeof(sparda_cached_layer) * (size_t)n_layers);
     for (int l = 0; l < n_layers; ++l) {
-        if (l + 1 < n_layers) {
-            SPARDA_PROF_BEGIN(0, cs);
-            rc = sparda_forecast_select(ctx, layers[l].F, layers[l + 1].Kpool, n_blocks, n_blocks, topk, layers[l + 1].ids, cs);
-            if (rc) return rc;
-            SPARDA_PROF_END(0, cs);
-            if (ps != cs) {
-                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], cs));
-                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ps, ctx->ev_sel[l + 1], 0));
-            }
-            SPARDA_PROF_BEGIN(1, ps);
-            rc = sparda_prefetch_launch(ctx, layers[l + 1].kv, n_blocks, layers[l + 1].ids, topk, pools[(l + 1) & 1], ps);
-            if (rc) return rc;
-            SPARDA_PROF_END(1, ps);
-            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], ps));
-        }
-        if (l == 0) {
-            SPARDA_PROF_BEGIN(2, cs);
-            rc = sparda_sparse_decode(ctx, layers[0].Q, layers[0].kv, layers[0].ids, topk, 1, n_blocks, layers[0].O, cs);
-        } else {
-            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
-            SPARDA_PROF_BEGIN(2, cs);
-            rc = sparda_sparse_decode(ctx, layers[l].Q, pools[l & 1], layers[l].ids, topk, 0, topk, layers[l].O, cs);
-        }
-        if (rc) return rc;
-        SPARDA_PROF_END(2, cs);
+        cl[l].base = layers[l];
+        cl[l].pool = pools[l & 1];   // double-buffered: gather l+1 lands while attention l reads the other buffer
+        cl[l].slot_ids = nullptr;
+        cl[l].fetch = nullptr;
+        cl[l].n_fetch = nullptr;
     }
-    return SPARDA_OK;
+    return decode_step_impl(ctx, cl, n_layers, F0cur, n_blocks, topk, (cudaStream_t)compute_stream, (cudaStream_t)prefetch_stream, mode);
 }
 
 int sparda_reuse_plan(sparda_ctx* ctx, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch,
@@ -263,53 +302,13 @@ int sparda_reuse_plan(sparda_ctx* ctx, const int32_t* ids_new, int topk, int32_t
     return sparda_launch_reuse_plan(ctx, ids_new, topk, slot_ids, fetch, n_fetch, (cudaStream_t)stream);
 }
 
-// Algorithm 2 lines 4-7 with the per-layer block cache of the previous step.  Hand-off: gather l+1 writes
-// pool_{l+1}, last read by attention l+1 of the PREVIOUS step, which precedes this step's select on the compute stream,
-// so ev_sel[l+1] releases it; reuse_plan updates slot_ids_{l+1} in place under the same ordering.
 int sparda_decode_step_cached(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                               int topk, void* compute_stream, void* prefetch_stream, int mode) {
     if (!ctx || !layers || n_layers < 1 || n_layers > ctx->max_layers || !F0cur) return SPARDA_EINVAL;
     if (mode != SPARDA_STEP_OVERLAP && mode != SPARDA_STEP_SERIAL) return SPARDA_EINVAL;
     for (int l = 1; l < n_layers; ++l)
         if (!layers[l].pool || !layers[l].slot_ids || !layers[l].fetch) return SPARDA_EINVAL;
-    cudaStream_t cs = (cudaStream_t)compute_stream;
-    cudaStream_t ps = mode == SPARDA_STEP_OVERLAP ? (cudaStream_t)prefetch_stream : cs;
-    int rc;
-    ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
-    SPARDA_PROF_BEGIN(0, cs);
-    rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_blocks, topk, layers[0].base.ids, cs);
-    if (rc) return rc;
-    SPARDA_PROF_END(0, cs);
-    for (int l = 0; l < n_layers; ++l) {
-        if (l + 1 < n_layers) {
-            const sparda_cached_layer* nx = &layers[l + 1];
-            SPARDA_PROF_BEGIN(0, cs);
-            rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids,
-                                             nx->slot_ids, nx->fetch, nx->n_fetch, cs);   // select + plan in one launch
-            if (rc) return rc;
-            SPARDA_PROF_END(0, cs);
-            if (ps != cs) {
-                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], cs));
-                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ps, ctx->ev_sel[l + 1], 0));
-            }
-            SPARDA_PROF_BEGIN(1, ps);
-            rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->fetch, topk, nx->pool, ps);
-            if (rc) return rc;
-            SPARDA_PROF_END(1, ps);
-            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], ps));
-        }
-        if (l == 0) {
-            SPARDA_PROF_BEGIN(2, cs);
-            rc = sparda_sparse_decode(ctx, layers[0].base.Q, layers[0].base.kv, layers[0].base.ids, topk, 1, n_blocks, layers[0].base.O, cs);
-        } else {
-            if (ps != cs) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
-            SPARDA_PROF_BEGIN(2, cs);
-            rc = sparda_sparse_decode(ctx, layers[l].base.Q, layers[l].pool, layers[l].slot_ids, topk, 0, topk, layers[l].base.O, cs);
-        }
-        if (rc) return rc;
-        SPARDA_PROF_END(2, cs);
-    }
-    return SPARDA_OK;
+    return decode_step_impl(ctx, layers, n_layers, F0cur, n_blocks, topk, (cudaStream_t)compute_stream, (cudaStream_t)prefetch_stream, mode);
 }
 
 int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,

@@ -31,6 +31,8 @@ struct sparda_ctx {
     float* pf_scratch;      // prefill comparison selector: [sm_count][512][128] fp32 group-summed scores (lazy)
     cudaEvent_t* ev_sel;    // [max_layers + 1]
     cudaEvent_t* ev_gather; // [max_layers + 1]
+    cudaEvent_t* ev_top;    // [max_layers + 1]: layer l may begin (attention l-1 is enqueued before it on the compute stream)
+    cudaStream_t select_stream;  // internal: select B_{l+1} runs here, concurrently with attention l (decode_step, overlap mode)
     int max_layers;
     // host-buffer step staging (device): F [(max_layers+1)][R][D] (slot max_layers = F0cur), Q and O [max_layers][B][Hq][D]
     char* stage_F;

@@ -316,3 +316,24 @@ def decode_pipeline_cached(steps, k: int, state=None):
                         "O": O, "O64": O64})
         out.append(res)
     return out, state
+
+
+# ---- o13: decode-time cache maintenance -----------------------------------
+def append_kv(kv: np.ndarray, kpool: np.ndarray, k_new: np.ndarray, v_new: np.ndarray, t: int):
+    """o13: Algorithm 2 lines 2-3: append the new token's K and V at position t of every row's cache and
+    "update K~ incrementally" (P:L89): when the token completes block j = t // S (t % S == S - 1) the block's pooled
+    key becomes the mean of its S keys (Eq.2, kernel = stride = S; computed by o1 on the finished block).
+
+    kv [R][Nb][2][S][D] and kpool [R][Nb][D] are modified in place; k_new, v_new [R][D] (bf16 bits).
+    Returns the number of complete blocks after the append, (t + 1) // S: the candidate range of the next selection."""
+    kv, kpool = _u16(kv), _u16(kpool)
+    R, Nb, two, S, D = kv.shape
+    j, o = divmod(int(t), S)
+    assert 0 <= j < Nb and k_new.shape == (R, D) and v_new.shape == (R, D)
+    for r in range(R):
+        kv[r, j, 0, o, :] = k_new[r]
+        kv[r, j, 1, o, :] = v_new[r]
+    if o == S - 1:
+        done = pool_keys(np.ascontiguousarray(kv[:, j:j + 1]))       # o1 on the finished block only
+        kpool[:, j, :] = done[:, 0, :]
+    return (int(t) + 1) // S

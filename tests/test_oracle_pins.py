@@ -442,6 +442,46 @@ def test_cached_pipeline_equals_plain_pipeline_step_by_step(oracle):
     assert 0 < fetched_total < 3 * 2 * cfg.rows * cfg.topk       # the drift really produced partial reuse
 
 
+# ---------------------------------------------------------------- o13 cache maintenance
+def test_append_kv_fills_a_block_like_the_prefilled_cache(oracle):
+    """Appending a block's 64 tokens one by one to an empty cache must leave exactly the bytes of the prefilled cache and,
+    when the block completes, exactly o1's pooled key for it; nothing else changes, and the candidate range grows by one
+    block only on completion."""
+    cfg = SMALL
+    L = _layer(cfg)
+    want_kv = L["kv"]
+    want_pool = oracle.pool_keys(want_kv)
+    R, Nb, _, S, D = want_kv.shape
+    kv = np.full_like(want_kv, 0x7FC0)                       # NaN pattern: untouched bytes stay recognisable
+    kpool = np.full_like(want_pool, 0x7FC0)
+    for t in range(2 * S + 5):                               # two full blocks and a partial third
+        j, o = divmod(t, S)
+        n = oracle.append_kv(kv, kpool, want_kv[:, j, 0, o], want_kv[:, j, 1, o], t)
+        assert n == (t + 1) // S
+        if o == S - 1:
+            np.testing.assert_array_equal(kpool[:, j], want_pool[:, j])
+        else:
+            assert np.all(kpool[:, j] == 0x7FC0)             # a partial block has no pooled key yet
+    np.testing.assert_array_equal(kv[:, :2], want_kv[:, :2])
+    np.testing.assert_array_equal(kv[:, 2, :, :5], want_kv[:, 2, :, :5])
+    assert np.all(kv[:, 2, :, 5:] == 0x7FC0) and np.all(kv[:, 3:] == 0x7FC0) and np.all(kpool[:, 2:] == 0x7FC0)
+
+
+def test_appended_block_becomes_selectable_when_complete(oracle):
+    """Planted needle through o13 + o3/o4: a block whose keys all equal 8*F is not a candidate while partial and is
+    selected by the first selection after its last token arrives (the index is updated incrementally)."""
+    cfg = SMALL.with_(topk=3)
+    L = _layer(cfg)
+    kv, kpool = L["kv"].copy(), oracle.pool_keys(L["kv"])
+    R, Nb, _, S, D = kv.shape
+    j = Nb - 1                                               # re-append the last block with needle keys
+    needle = bf.f64_to_bf16_bits(8.0 * bf.bits_to_f64(L["F"]))
+    for o in range(S):
+        n = oracle.append_kv(kv, kpool, needle, L["kv"][:, j, 1, o], j * S + o)
+        ids, _ = oracle.forecast_select(L["F"], kpool, cfg.topk, n)
+        assert all((j in ids[r]) == (o == S - 1) for r in range(R))
+
+
 # ---------------------------------------------------------------- closed forms the paper prints
 def test_paper_closed_forms_golden():
     """tests/golden/paper_closed_forms.txt: P:L95 (33.5M Forecast parameters, 0.41% of 8B) and the

@@ -334,6 +334,46 @@ def bench_prefill(torch, binding, peaks_all):
     return out
 
 
+def bench_append(torch, binding):
+    """f2 (Alg.2 lines 2-3): one token appended per launch to a device-resident cache and to a pinned host cache written
+    through UVA, batch-32 rows (R = 64, D = 128), 64 consecutive positions (one of them completes a block), replayed from
+    a CUDA graph.  4 KiB of K/V + 64 KiB of fp32 running sums per launch: launch-latency-sized."""
+    from paper_2606_04511_b200 import synth
+    cfg = synth.CFG4_128K.with_(n_blocks=64)
+    R, Nb, D = cfg.rows, cfg.n_blocks, cfg.head_dim
+    ctx = binding.Sparda.from_config(cfg)
+    g = torch.Generator(device="cuda").manual_seed(12)
+    kn = torch.randn((64, R, D), generator=g, device="cuda").to(torch.bfloat16)
+    vn = torch.randn((64, R, D), generator=g, device="cuda").to(torch.bfloat16)
+    kpool = torch.zeros((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+    out = {}
+    for where in ("device", "host_uva"):
+        kv = torch.zeros((R, Nb, 2, 64, D), dtype=torch.bfloat16, device="cuda") if where == "device" else \
+            torch.zeros((R, Nb, 2, 64, D), dtype=torch.bfloat16).pin_memory()
+        ksum = torch.zeros((R, D), dtype=torch.float32, device="cuda")
+        for t in range(64):
+            ctx.append_kv(kn[t], vn[t], 64 + t, kv, Nb, ksum, kpool)
+        torch.cuda.synchronize()
+        graph, cap = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        with torch.cuda.graph(graph, stream=cap):
+            for t in range(64):
+                ctx.append_kv(kn[t], vn[t], 128 + t, kv, Nb, ksum, kpool, stream=torch.cuda.current_stream())
+        graph.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            graph.replay()
+        e1.record()
+        e1.synchronize()
+        out[f"us_per_append_{where}"] = e0.elapsed_time(e1) * 1e3 / (5 * 64)
+        del graph, kv
+    out["workload"] = f"append_kv_kernel<128>, R = {R} rows (batch 32), one token per launch, 64 launches per graph"
+    out["bytes_per_launch"] = R * D * 2 * 2 + 2 * R * D * 4
+    ctx.close()
+    return out
+
+
 def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps):
     """SURVEY 8(f) f1 / 8(d) "gather hidden": the same 32-layer decode step with the previous step's blocks kept per
     layer, so only newly selected blocks cross the host link.  The Forecast alternates between F_A and
@@ -430,7 +470,7 @@ def run_sparda(args):
     peaks = load_peaks()
     if args.section == "kernels":
         print(json.dumps({"section": "kernels", "roofline_kernels": bench_kernels_b32(torch, binding, peaks, args),
-                          "prefill_select": bench_prefill(torch, binding, peaks)}))
+                          "prefill_select": bench_prefill(torch, binding, peaks), "cache_maintenance": bench_append(torch, binding)}))
         return 0
     cfg = workload_config(args)
     cfg = cfg.with_(seed=cfg.seed + 1000 * rank)             # every rank decodes its own sequences
@@ -577,11 +617,12 @@ def run_sparda(args):
          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": att_bytes / t_att / 1e9 / peaks["hbm_gbs"], "traffic": None,
          "note": "launch-latency-sized at batch 4 (ideal 2.6 us)"},
     ]
-    prefill = None
+    prefill = append = None
     if not args.no_kernels:
         del pools
         kernels += bench_kernels_b32(torch, binding, peaks, args)
         prefill = bench_prefill(torch, binding, peaks)
+        append = bench_append(torch, binding)
 
     base = None
     if not args.no_cpu_baseline and world == 1:
@@ -624,6 +665,7 @@ def run_sparda(args):
         "cpu_baseline": base,
         "prefill_select": prefill,
         "reuse_cache": reuse,
+        "cache_maintenance": append,
         "pipeline": {"ms_per_step_overlap": ms_per_step, "ms_per_step_serial": ms_serial,
                      "us_per_layer_step": ms_per_step * 1e3 / NL,
                      "us_select": t_sel * 1e6, "us_gather": t_gat * 1e6, "us_attn": t_att * 1e6,

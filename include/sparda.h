@@ -101,6 +101,17 @@ int sparda_destroy(sparda_ctx* ctx);
  * Pre-condition of the path ("kept on GPU and updated incrementally"), not on the timed path.  */
 int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_blocks, void* kpool, void* stream);
 
+/* (f2) Decode-time cache maintenance, Alg.2 lines 2-3: append the new token's key and value at position t
+ * (0-based; block t / S, offset t % S) of every row's cache and "update K~ incrementally".  k_new, v_new
+ * [R][D] device; kv_cache [R][n_blocks][2][S][D]: a device pointer (layer 0) or a host-mapped pointer (the offloaded
+ * layers: the 2*D*2 bytes per row are written through UVA, the asynchronous CPU write-back of P:L159); ksum [R][D] fp32
+ * device, owned by the caller, zero-initialised, carried from call to call: the running fp32 sum of the open block's
+ * keys in arrival order; kpool [R][n_blocks][D] device: row j is written when t % S == S - 1, bit-identical to
+ * sparda_pool_keys on the finished block, and ksum is reset.  Tokens must be appended in ascending t.  The candidate
+ * range of the next selection is the complete blocks, n_cand = (t + 1) / S.  One small kernel on `stream`.          */
+int sparda_append_kv(sparda_ctx* ctx, const void* k_new, const void* v_new, int64_t t, void* kv_cache, int n_blocks,
+                     float* ksum, void* kpool, void* stream);
+
 /* (a1+a2) Forecast indexer, Eq.4: s[r,j] = sum_d F[r,d]*Kpool[r,j,d] (raw logits, fp32
  * accumulate, no softmax, no scale) for candidate blocks j in [0, n_cand); ids_out[r] = the min(topk, n_cand)
  * best blocks, ties to the lowest block id, emitted in ascending block id and padded with -1.

@@ -18,7 +18,7 @@ GATHER_TMA, GATHER_LDG = 0, 1
 STEP_OVERLAP, STEP_SERIAL = 0, 1
 
 EXPORTS = [
-    "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_select", "sparda_prefetch_launch",
+    "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_append_kv", "sparda_forecast_select", "sparda_prefetch_launch",
     "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
     "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
@@ -62,6 +62,7 @@ def lib() -> ctypes.CDLL:
         L.sparda_create.argtypes = [ctypes.POINTER(SpardaConfig), ctypes.POINTER(vp)]
         L.sparda_destroy.argtypes = [vp]
         L.sparda_pool_keys.argtypes = [vp, vp, i64, i32, vp, vp]
+        L.sparda_append_kv.argtypes = [vp, vp, vp, i64, vp, i32, vp, vp, vp]
         L.sparda_forecast_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_prefetch_launch.argtypes = [vp, vp, i32, vp, i32, vp, vp]
         L.sparda_sparse_decode.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
@@ -142,6 +143,10 @@ class Sparda:
     # ---- entry points (same names as include/sparda.h without the prefix) ----
     def pool_keys(self, kv, n_rows, n_blocks, kpool, stream=None):
         self._check(self._L.sparda_pool_keys(self._h, _ptr(kv), n_rows, n_blocks, _ptr(kpool), _stream(stream)), "pool_keys")
+
+    def append_kv(self, k_new, v_new, t, kv_cache, n_blocks, ksum, kpool, stream=None):
+        self._check(self._L.sparda_append_kv(self._h, _ptr(k_new), _ptr(v_new), int(t), _ptr(kv_cache), n_blocks, _ptr(ksum),
+                                             _ptr(kpool), _stream(stream)), "append_kv")
 
     def forecast_select(self, F, Kpool, n_blocks, topk, ids_out, n_cand=None, stream=None):
         n_cand = n_blocks if n_cand is None else n_cand

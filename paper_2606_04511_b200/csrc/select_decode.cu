@@ -448,6 +448,44 @@ __global__ void __launch_bounds__(256) pool_keys_kernel(const uint4* __restrict_
     kpool[rb * LPK + dl] = o;
 }
 
+// f2, Alg.2 lines 2-3: append the new token's K and V at position t of every row's cache (device-resident, or
+// pinned host memory written through UVA: the asynchronous write-back of P:L159) and update the pooled keys incrementally
+// (P:L89): ksum accumulates the open block's keys in fp32 in arrival (= ascending t) order, exactly the sum order of
+// pool_keys_kernel, so the pooled key written when the block completes is bit-identical to pooling the finished block.
+template <int D>
+__global__ void __launch_bounds__(256) append_kv_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
+                                                         uint4* __restrict__ kv, float* __restrict__ ksum, uint4* __restrict__ kpool,
+                                                         int n_rows, int n_blocks, int64_t t) {
+    constexpr int LPK = D / 8, S = 64;
+    const int gthread = blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = gthread / LPK, dl = gthread % LPK;
+    if (r >= n_rows) return;
+    const int64_t j = t / S;
+    const int o = (int)(t % S);
+    const uint4 k = __ldg(k_new + (size_t)r * LPK + dl), v = __ldg(v_new + (size_t)r * LPK + dl);
+    uint4* blk = kv + ((size_t)r * n_blocks + j) * (2 * S * LPK);
+    blk[(size_t)o * LPK + dl] = k;                      // plane 0 = K
+    blk[(size_t)(S + o) * LPK + dl] = v;                // plane 1 = V
+    float* acc = ksum + ((size_t)r * LPK + dl) * 8;
+    float a[8];
+    const float4 a0 = *reinterpret_cast<const float4*>(acc), a1 = *reinterpret_cast<const float4*>(acc + 4);
+    a[0] = a0.x + bf16_lo(k.x); a[1] = a0.y + bf16_hi(k.x); a[2] = a0.z + bf16_lo(k.y); a[3] = a0.w + bf16_hi(k.y);
+    a[4] = a1.x + bf16_lo(k.z); a[5] = a1.y + bf16_hi(k.z); a[6] = a1.z + bf16_lo(k.w); a[7] = a1.w + bf16_hi(k.w);
+    if (o == S - 1) {
+        const float inv = 1.0f / S;
+        uint4 p;
+        p.x = pack_bf16(a[0] * inv, a[1] * inv);
+        p.y = pack_bf16(a[2] * inv, a[3] * inv);
+        p.z = pack_bf16(a[4] * inv, a[5] * inv);
+        p.w = pack_bf16(a[6] * inv, a[7] * inv);
+        kpool[((size_t)r * n_blocks + j) * LPK + dl] = p;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) a[i] = 0.f;
+    }
+    *reinterpret_cast<float4*>(acc) = make_float4(a[0], a[1], a[2], a[3]);
+    *reinterpret_cast<float4*>(acc + 4) = make_float4(a[4], a[5], a[6], a[7]);
+}
+
 }  // namespace
 
 // Cluster size of the select launch: the largest power of two <= 16 such that R*CS CTAs fit the SMs (the
@@ -530,6 +568,20 @@ int sparda_launch_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int
         pool_keys_kernel<128><<<grid, 256, 0, st>>>((const uint4*)kv, (uint4*)kpool, n_rb);
     else
         pool_keys_kernel<64><<<grid, 256, 0, st>>>((const uint4*)kv, (uint4*)kpool, n_rb);
+    SPARDA_CUDA_TRY(ctx, cudaGetLastError());
+    ctx->launches++;
+    return SPARDA_OK;
+}
+
+int sparda_launch_append_kv(sparda_ctx* ctx, const void* k_new, const void* v_new, int64_t t, void* kv, int n_blocks, float* ksum,
+                            void* kpool, cudaStream_t st) {
+    const int lpk = ctx->cfg.head_dim / 8;
+    const int threads = ctx->R * lpk;
+    const unsigned grid = (unsigned)((threads + 255) / 256);
+    if (ctx->cfg.head_dim == 128)
+        append_kv_kernel<128><<<grid, 256, 0, st>>>((const uint4*)k_new, (const uint4*)v_new, (uint4*)kv, ksum, (uint4*)kpool, ctx->R, n_blocks, t);
+    else
+        append_kv_kernel<64><<<grid, 256, 0, st>>>((const uint4*)k_new, (const uint4*)v_new, (uint4*)kv, ksum, (uint4*)kpool, ctx->R, n_blocks, t);
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;
     return SPARDA_OK;

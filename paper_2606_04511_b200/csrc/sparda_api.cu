@@ -149,6 +149,15 @@ int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_bloc
     return sparda_launch_pool_keys(ctx, kv, n_rows, n_blocks, kpool, (cudaStream_t)stream);
 }
 
+int sparda_append_kv(sparda_ctx* ctx, const void* k_new, const void* v_new, int64_t t, void* kv_cache, int n_blocks, float* ksum,
+                     void* kpool, void* stream) {
+    if (!ctx || !sparda_aligned(k_new, 16) || !sparda_aligned(v_new, 16) || !sparda_aligned(kv_cache, 16) || !sparda_aligned(ksum, 16) ||
+        !sparda_aligned(kpool, 16))
+        return SPARDA_EINVAL;
+    if (n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || t < 0 || t >= (int64_t)n_blocks * ctx->cfg.block_size) return SPARDA_EINVAL;
+    return sparda_launch_append_kv(ctx, k_new, v_new, t, kv_cache, n_blocks, ksum, kpool, (cudaStream_t)stream);
+}
+
 int sparda_forecast_select(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
                            int32_t* ids_out, void* stream) {
     if (!ctx || !sparda_aligned(F, 16) || !sparda_aligned(Kpool, 16) || !sparda_aligned(ids_out, 4)) return SPARDA_EINVAL;

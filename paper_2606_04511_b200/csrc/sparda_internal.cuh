@@ -66,6 +66,8 @@ int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_bl
                          cudaStream_t);
 int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
                          cudaStream_t);
+int sparda_launch_append_kv(sparda_ctx*, const void* k_new, const void* v_new, int64_t t, void* kv, int n_blocks, float* ksum,
+                            void* kpool, cudaStream_t);
 int sparda_launch_reuse_plan(sparda_ctx*, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch,
                              cudaStream_t);
 int sparda_launch_attn(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,

@@ -463,6 +463,55 @@ def test_decode_step_cached_multi_step(cfg, sp, oracle):
     assert 0 < moved < (n_steps - 1) * (NL - 1) * R * k, "the drift should give partial reuse"
 
 
+@pytest.mark.parametrize("where", ["device", "host"])
+@pytest.mark.parametrize("cfg", [MID64.with_(n_blocks=6), G16.with_(n_blocks=5)], ids=lambda c: c.name)
+def test_append_kv_matches_oracle(cfg, where, sp, oracle):
+    """f2 (o13): tokens appended one by one to a device-resident cache (layer 0) and to a pinned host cache written through
+    UVA (offloaded layers): cache bytes exact and nothing else touched, pooled keys written only when a block completes
+    and bit-identical to the pooling kernel on the finished block (<= 1 bf16 ulp from the fp64 oracle, as a0), the running
+    sum reset afterwards; then a selection over the complete blocks and attention on the appended cache match the oracle."""
+    L, ctx, kpool_full = _setup(cfg, sp)
+    R, Nb, S, D, k = cfg.rows, cfg.n_blocks, 64, cfg.head_dim, min(cfg.topk, 2)
+    src = L["kv"]
+    n_tok = 3 * S + 17
+    kv_dev = torch.full_like(src, float("nan")) if where == "device" else torch.full_like(src, float("nan")).cpu().pin_memory()
+    kpool = torch.full((R, Nb, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    ksum = torch.zeros((R, D), dtype=torch.float32, device="cuda")
+    o_kv = np.full(_bits(src).shape, 0x7FC0, dtype=np.uint16)
+    o_pool = np.full((R, Nb, D), 0x7FC0, dtype=np.uint16)
+    src_bits = _bits(src)
+    for t in range(n_tok):
+        j, o = divmod(t, S)
+        ctx.append_kv(src[:, j, 0, o].contiguous(), src[:, j, 1, o].contiguous(), t, kv_dev, Nb, ksum, kpool)
+        n_cand = oracle.append_kv(o_kv, o_pool, src_bits[:, j, 0, o], src_bits[:, j, 1, o], t)
+    torch.cuda.synchronize()
+    got_kv = _bits(kv_dev)
+    assert got_kv[:, :3].tobytes() == o_kv[:, :3].tobytes() and got_kv[:, 3, :, :17].tobytes() == o_kv[:, 3, :, :17].tobytes()
+    nan_bits = _bits(torch.full((1,), float("nan"), dtype=torch.bfloat16))[0]
+    assert np.all(got_kv[:, 3, :, 17:] == nan_bits) and np.all(got_kv[:, 4:] == nan_bits), "bytes outside the appended tokens touched"
+    got_pool = _bits(kpool)
+    assert got_pool[:, :3].tobytes() == _bits(kpool_full)[:, :3].tobytes(), "incremental pooled keys != pooling the finished blocks"
+    assert parity.ulp_diff_bf16(got_pool[:, :3], o_pool[:, :3]).max() <= 1
+    assert np.all(got_pool[:, 3:] == nan_bits), "a partial block must not have a pooled key"
+    # the running sum holds exactly the 17 keys of the open block (fp32, ascending t)
+    want_sum = torch.zeros((R, D), dtype=torch.float32, device="cuda")
+    for o in range(17):
+        want_sum += src[:, 3, 0, o].float()
+    assert torch.equal(ksum, want_sum)
+    assert n_cand == 3
+    ids = torch.full((R, k), -7, dtype=torch.int32, device="cuda")
+    ctx.forecast_select(L["F"], kpool, Nb, k, ids, n_cand=n_cand)
+    torch.cuda.synchronize()
+    want, sc = oracle.forecast_select(_bits(L["F"]), np.where(o_pool == 0x7FC0, 0, o_pool).astype(np.uint16), k, n_cand)
+    parity.check_ids(ids.cpu().numpy(), want, sc[:, :n_cand] if sc.shape[1] > n_cand else sc, n_cand)
+    if where == "device":
+        O = torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda")
+        ctx.sparse_decode(L["Q"], kv_dev, ids, k, O, pool_is_indexed=True, n_slots=Nb)
+        torch.cuda.synchronize()
+        wantO, _ = oracle.sparse_attn(_bits(L["Q"]), np.where(o_kv == 0x7FC0, 0, o_kv).astype(np.uint16), ids.cpu().numpy(), pool_is_indexed=True)
+        parity.check_attn(_bits(O), wantO, "attention on the appended cache")
+
+
 def test_cfg2_full_size_layer(sp, oracle):
     """BASELINE.json configs[1] at full size: batch 8, 32/2 heads, D=128, 512 blocks, top-64, KV pinned on host."""
     cfg = synth.CFG2_32K

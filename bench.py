@@ -271,6 +271,9 @@ def bench_kernels_b32(torch, binding, peaks, args):
                     "bound": "hbm", "us_per_launch": t * 1e6, "algorithmic_bytes": b, "achieved": b / t / 1e9,
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": b / t / 1e9 / peaks["hbm_gbs"],
                     "frac_of_nominal_8tbs": b / t / 1e9 / 8000.0, "peak_source": peaks["source"], "traffic": None})
+    # DRAM read + write bytes per launch of the same shapes from the committed ncu --set full captures
+    out[0]["traffic"], out[0]["traffic_source"] = 33612800, "profiles/r1b_ncu_summary.md (prof_b32_select_b: dram read 33.61 MB, write 0)"
+    out[1]["traffic"], out[1]["traffic_source"] = 134556160 + 4178688, "profiles/r1b_ncu_summary.md (prof_b32_attn_b: dram read 134.56 MB, write 4.18 MB of split-K partials)"
     out[1]["attn_splits"] = ctx.attn_splits(k)
     ctx.close()
     del kpools, pools
@@ -473,7 +476,8 @@ def run_sparda(args):
                           "prefill_select": bench_prefill(torch, binding, peaks), "cache_maintenance": bench_append(torch, binding)}))
         return 0
     cfg = workload_config(args)
-    cfg = cfg.with_(seed=cfg.seed + 1000 * rank)             # every rank decodes its own sequences
+    from paper_2606_04511_b200 import shard
+    cfg = shard.rank_config(cfg, rank)                       # every rank decodes its own sequences
     R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
 
     mode = binding.GATHER_TMA if args.gather_mode == "tma" else binding.GATHER_LDG
@@ -537,12 +541,7 @@ def run_sparda(args):
             fn()
         e1.record(cs)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return shard.max_over_ranks(e0.elapsed_time(e1), device="cuda")
 
     # ---- timed region: device-resident Q/F/Kpool, KV in pinned host memory (the method's offload tier)
     for _ in range(args.warmup):
@@ -585,8 +584,8 @@ def run_sparda(args):
 
     ms_per_step = ms_total / args.steps
     tokens = cfg.batch * world
-    value = tokens / (ms_per_step * 1e-3)
-    e2e_value = tokens / (ms_e2e / args.steps * 1e-3)
+    value = shard.whole_job_value(cfg.batch, world, ms_per_step)
+    e2e_value = shard.whole_job_value(cfg.batch, world, ms_e2e / args.steps)
 
     if rank != 0:
         if world > 1:
@@ -602,7 +601,10 @@ def run_sparda(args):
     att_bytes = cfg.gather_bytes_per_layer + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
     roofline = {"kernel": "gather_tma_kernel" if args.gather_mode == "tma" else "gather_ldg_kernel",
                 "bound": "host_link", "achieved": gather_bytes / t_gat / 1e9, "peak": ceiling, "unit": "GB/s",
-                "frac": gather_bytes / t_gat / 1e9 / ceiling, "traffic": None,
+                "frac": gather_bytes / t_gat / 1e9 / ceiling,
+                "traffic": 56064 if cfg.name == "cfg3_128k_pipeline" else None,
+                "traffic_note": "DRAM bytes of one batch-4 launch (ncu, profiles/r1b_ncu_summary.md): the ids only; the payload crosses the "
+                                "host link (sysmem read sectors x 32 B = the algorithmic 16 MiB, profiles/r1_ncu_summary.md) and lands in L2",
                 "peak_source": "cudaMemcpyAsync pinned host->device, measured in this run on this box",
                 "us_per_launch": t_gat * 1e6, "algorithmic_bytes": gather_bytes,
                 "share_of_step": prof["gather"][0] / args.steps / ms_per_step,

@@ -16,6 +16,9 @@
 // ticket, no fence and no scratch.  HBM-bound: R*n_cand*D*2 bytes of Kpool.
 #include "sparda_internal.cuh"
 #include "reuse_plan.cuh"
+#ifdef SEL_CS_ENV
+#include <cstdlib>
+#endif
 
 #ifdef SPARDA_TRACE
 __device__ unsigned long long* g_sel_trace;   // [gridDim.x][16] globaltimer stamps (debug builds only)
@@ -519,6 +522,9 @@ static int select_launch(sparda_ctx* ctx, const SelParams& p0, cudaStream_t st) 
     int cs = 1;
     if (p.n_cand > p.topk)
         while (cs * 2 <= SEL_MAX_CS && (long long)ctx->R * cs * 2 <= ctx->sm_count && cs * 2 <= (p.n_cand + KPS - 1) / KPS) cs *= 2;
+#ifdef SEL_CS_ENV
+    if (getenv("SPARDA_SELECT_CS") && p.n_cand > p.topk) cs = atoi(getenv("SPARDA_SELECT_CS"));
+#endif
     for (; cs > 1; cs /= 2) {
         if (cluster_ok[cs] == 0) {
             int n = 0;

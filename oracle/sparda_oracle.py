@@ -337,3 +337,57 @@ def append_kv(kv: np.ndarray, kpool: np.ndarray, k_new: np.ndarray, v_new: np.nd
         done = pool_keys(np.ascontiguousarray(kv[:, j:j + 1]))       # o1 on the finished block only
         kpool[:, j, :] = done[:, 0, :]
     return (int(t) + 1) // S
+
+
+# ---- o14 / o15: the paper's selector geometry -- PARITY UNPINNED BY THE PAPER ------
+# The paper compresses keys with overlapping windows (l_C, s) = (32, 16) (Eq.2) and says f_top
+# "max-pools compressed-key-grid scores to block-level scores" without giving the pooling kernel, stride or
+# padding.  Reading q19: compressed key j covers tokens [16 j, 16 j + 32), j = 0 .. T/16 - 2;
+# block b's score is the maximum over the compressed keys whose window STARTS inside the block (j = 4b .. 4b+3, the
+# last one reaching 16 tokens into the next block; block Nb-1 has three).  Initial and local blocks do not take part
+# in the ranking and are always attended (Eq.1): B = init U local U top-k.  These two functions are
+# pinned to brute force and invariants written independently in tests/, not to anything the paper prints.
+def pool_keys_grid(kv: np.ndarray, window: int = 32, stride: int = 16) -> np.ndarray:
+    """o14 (Eq.2, P:L60 with (l_C, s) = (32, 16)): Kgrid[r, j, :] = bf16(mean of keys stride*j .. stride*j+window-1),
+    fp64 sum in ascending token order.  kv [R][Nb][2][S][D] -> Kgrid [R][Nb*S/stride][D]; rows j >= n_comp =
+    (T - window)/stride + 1 (windows that would cross the end of the context) are zero."""
+    kv = _u16(kv)
+    R, Nb, two, S, D = kv.shape
+    T = Nb * S
+    n_rows, n_comp = T // stride, (T - window) // stride + 1
+    keys = bf16_bits_to_f64(kv[:, :, 0]).reshape(R, T, D)
+    out = np.zeros((R, n_rows, D), dtype=np.uint16)
+    for r in range(R):
+        for j in range(n_comp):
+            acc = np.zeros(D, dtype=np.float64)
+            for t in range(stride * j, stride * j + window):
+                acc += keys[r, t]
+            mean = acc / window
+            out[r, j] = [double_to_bf16(float(x)) for x in mean]
+    return out
+
+
+def forecast_select_grid(F: np.ndarray, kgrid: np.ndarray, k_total: int, n_cand: int, n_init: int, n_local: int, per_block: int = 4):
+    """o15 (Eq.1, Eq.4, f_top P:L78, reading q19): compressed-key scores s_j = F . Kgrid_j (o3), block score =
+    max of the per_block compressed keys that start in the block and exist (j < per_block * n_cand - 1), blocks
+    [0, n_init) and [n_cand - n_local, n_cand) always selected, the other k_total - n_init - n_local picked by block score
+    (o4: score descending, lowest id on ties) among the remaining candidates; ascending ids, -1 padded.
+    Returns (ids [R][k_total], block_scores [R][n_cand] fp32 with forced blocks at +inf)."""
+    s = score(F, kgrid)                                       # [R][n_rows] fp32, raw logits
+    R = s.shape[0]
+    n_keys = per_block * n_cand - 1
+    ids = np.full((R, k_total), -1, dtype=np.int32)
+    bs = np.full((R, max(n_cand, 0)), -np.inf, dtype=np.float32)
+    for r in range(R):
+        for b in range(n_cand):
+            js = [j for j in range(per_block * b, per_block * b + per_block) if j < n_keys]
+            bs[r, b] = max(s[r, j] for j in js)
+        forced = [b for b in range(n_cand) if b < n_init or b >= n_cand - n_local]
+        assert len(forced) <= k_total
+        free = [b for b in range(n_cand) if b not in forced]
+        free.sort(key=lambda b: (-float(bs[r, b]), b))
+        chosen = sorted(forced + free[:k_total - len(forced)])
+        ids[r, :len(chosen)] = chosen
+        for b in forced:
+            bs[r, b] = np.inf
+    return ids, bs

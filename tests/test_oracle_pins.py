@@ -482,6 +482,56 @@ def test_appended_block_becomes_selectable_when_complete(oracle):
         assert all((j in ids[r]) == (o == S - 1) for r in range(R))
 
 
+# ---------------------------------------------------------------- o14 / o15 the (32,16) grid + max-pool (reading q19; unpinned by the paper)
+def test_pool_keys_grid_bruteforce_and_special_cases(oracle):
+    cfg = SMALL
+    L = _layer(cfg)
+    R, Nb, _, S, D = L["kv"].shape
+    grid = oracle.pool_keys_grid(L["kv"])
+    T = Nb * S
+    assert grid.shape == (R, T // 16, D)
+    keys = bf.bits_to_f64(L["kv"][:, :, 0]).reshape(R, T, D)
+    n_comp = (T - 32) // 16 + 1
+    for j in (0, 1, 5, n_comp - 1):
+        want = bf.f64_to_bf16_bits(keys[:, 16 * j:16 * j + 32].mean(axis=1))        # numpy mean, independent of the loops
+        assert np.max(np.abs(grid[:, j].astype(np.int32) - want.astype(np.int32))) <= 1
+    assert np.all(grid[:, n_comp:] == 0)                                           # windows crossing the end do not exist
+    # window = stride = S reduces to o1 (one key per block)
+    np.testing.assert_array_equal(oracle.pool_keys_grid(L["kv"], window=S, stride=S), oracle.pool_keys(L["kv"]))
+    # a constant context pools to that constant
+    const = L["kv"].copy()
+    const[:, :, 0] = const[:, :1, 0, :1]
+    g2 = oracle.pool_keys_grid(const)
+    assert np.all(g2[:, :n_comp] == const[:, :1, 0, 0])
+
+
+def test_select_grid_bruteforce_forced_blocks_and_needle(oracle):
+    rng = np.random.default_rng(11)
+    cfg = SMALL.with_(n_blocks=20)
+    L = _layer(cfg)
+    grid = oracle.pool_keys_grid(L["kv"])
+    R, Nb = cfg.rows, cfg.n_blocks
+    s = bf.bits_to_f64(L["F"])[:, None, :] * bf.bits_to_f64(grid)
+    s = s.sum(-1)                                                                   # [R][4 Nb] fp64, brute force
+    for n_cand, n_init, n_local, k in [(20, 1, 4, 9), (20, 0, 0, 5), (13, 2, 3, 7), (6, 1, 4, 9), (3, 1, 4, 9)]:
+        ids, bs = oracle.forecast_select_grid(L["F"], grid, k, n_cand, n_init, n_local)
+        for r in range(R):
+            block = [max(s[r, j] for j in range(4 * b, 4 * b + 4) if j < 4 * n_cand - 1) for b in range(n_cand)]
+            forced = set(b for b in range(n_cand) if b < n_init or b >= n_cand - n_local)
+            got = [int(x) for x in ids[r] if x >= 0]
+            assert got == sorted(got) and forced <= set(got) and len(got) == min(k, n_cand)
+            rest = sorted((b for b in range(n_cand) if b not in forced), key=lambda b: (-block[b], b))
+            assert set(got) - forced == set(rest[:max(0, min(k, n_cand) - len(forced))])
+    # needle: keys equal to 8 F only in tokens [64 b + 16, 64 b + 48) -- exactly window 4b+1 -- pull block b in, and the
+    # window that starts in block b-1 and reaches into b (j = 4b - 1) does not pull block b-1 above it
+    b = 9
+    kv = L["kv"].copy()
+    needle = bf.f64_to_bf16_bits(8.0 * bf.bits_to_f64(L["F"]))
+    kv[:, b, 0, 16:48] = needle[:, None, :]
+    ids, bs = oracle.forecast_select_grid(L["F"], oracle.pool_keys_grid(kv), 3, Nb, 0, 0)
+    assert all(b in ids[r] for r in range(R)) and np.all(bs[:, b] > bs[:, b - 1])
+
+
 # ---------------------------------------------------------------- closed forms the paper prints
 def test_paper_closed_forms_golden():
     """tests/golden/paper_closed_forms.txt: P:L95 (33.5M Forecast parameters, 0.41% of 8B) and the

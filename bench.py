@@ -265,8 +265,18 @@ def bench_kernels_b32(torch, binding, peaks, args):
     t_att = timed(lambda i, s: ctx.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT)
     sel_bytes = cfg.kpool_bytes_per_layer + R * D * 2 + R * k * 4
     att_bytes = cfg.gather_bytes_per_layer + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
+    # f3: the paper's geometry -- (32,16) compressed-key grid (4 keys per block), max-pool to blocks, budget 96 = 1 + 32 + 63
+    del kpools
+    grids = [torch.randn((R, 4 * Nb, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(2)]
+    ids96 = torch.empty((R, 96), dtype=torch.int32, device="cuda")
+    ctx96 = binding.Sparda(cfg.batch, cfg.n_q_heads, cfg.n_kv_heads, D, Nb, 96)
+    t_grid = timed(lambda i, s: ctx96.forecast_select_grid(Fs[i], grids[i], Nb, 96, ids96, n_init=1, n_local=32, stream=s), 2)
+    grid_bytes = R * (4 * Nb - 1) * D * 2 + R * D * 2 + R * 96 * 4
+    ctx96.close()
+    del grids
     out = []
-    for name, t, b in (("forecast_select_kernel<128>", t_sel, sel_bytes), ("sparse_decode_kernel<128>", t_att, att_bytes)):
+    for name, t, b in (("forecast_select_kernel<128>", t_sel, sel_bytes), ("sparse_decode_kernel<128>", t_att, att_bytes),
+                       ("forecast_select_kernel<128,grid>", t_grid, grid_bytes)):
         out.append({"kernel": name, "workload": "cfg4 shape, batch 32, one layer, cold HBM (rotating buffer sets > L2), launches replayed from a CUDA graph",
                     "bound": "hbm", "us_per_launch": t * 1e6, "algorithmic_bytes": b, "achieved": b / t / 1e9,
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": b / t / 1e9 / peaks["hbm_gbs"],
@@ -275,8 +285,10 @@ def bench_kernels_b32(torch, binding, peaks, args):
     out[0]["traffic"], out[0]["traffic_source"] = 33612800, "profiles/r1b_ncu_summary.md (prof_b32_select_b: dram read 33.61 MB, write 0)"
     out[1]["traffic"], out[1]["traffic_source"] = 134556160 + 4178688, "profiles/r1b_ncu_summary.md (prof_b32_attn_b: dram read 134.56 MB, write 4.18 MB of split-K partials)"
     out[1]["attn_splits"] = ctx.attn_splits(k)
+    out[2]["workload"] = ("f3 (reading q19, unpinned by the paper): batch 32, 2048 blocks x 4 compressed keys, max-pool to blocks, "
+                          "top-96 = 1 initial + 32 local + 63 ranked; cold HBM (two 128 MiB grids > L2), CUDA-graph replay")
     ctx.close()
-    del kpools, pools
+    del pools
     torch.cuda.empty_cache()
     return out
 

@@ -178,6 +178,20 @@ int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_l
 int sparda_reuse_plan(sparda_ctx* ctx, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch,
                       int32_t* n_fetch, void* stream);
 
+/* (f3) The paper's selector geometry.  PARITY UNPINNED BY THE PAPER: Eq.2 with (l_C, s) = (32, 16) fixes
+ * the compressed keys, but the max-pool that turns compressed-grid scores into block scores has no stated
+ * kernel, stride or padding; this library takes reading q19.
+ * sparda_pool_keys_grid: Kgrid[r, j, :] = bf16(mean of keys 16 j .. 16 j + 31), fp32 sum in ascending token order,
+ *   j < 4 * n_blocks - 1; kv [R][n_blocks][2][S][D] device, kgrid [R][4 * n_blocks][D] device (last row zero).
+ * sparda_forecast_select_grid: s_j = F[r] . Kgrid[r, j] (raw logits, Eq.4); block b's score = max of s_j over the
+ *   compressed keys whose window starts inside the block, j = 4b .. 4b+3 with j < 4 * n_cand - 1 (f_top); blocks
+ *   [0, n_init) (initial) and [n_cand - n_local, n_cand) (local window) are always selected and do not compete (Eq.1,
+ *   P:L53); the remaining topk - n_init - n_local places go to the best other candidates, ties to the lowest id;
+ *   ids_out [R][topk] ascending, -1 padded.  The paper's budget is topk = 96 = 1 + 32 + 63.              */
+int sparda_pool_keys_grid(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_blocks, void* kgrid, void* stream);
+int sparda_forecast_select_grid(sparda_ctx* ctx, const void* F, const void* Kgrid, int n_blocks, int n_cand, int n_init,
+                                int n_local, int topk, int32_t* ids_out, void* stream);
+
 /* sparda_forecast_select followed by sparda_reuse_plan on its result, in ONE launch: the CTA that selects a row also
  * updates the row's slot table and fetch list (same results as the two calls; saves a launch per layer of the cached
  * decode step).  Arguments as in the two calls.                                                                   */

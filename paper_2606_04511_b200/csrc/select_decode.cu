@@ -261,7 +261,10 @@ struct SelParams {
     const char* Kpool;
     int32_t* ids;
     int n_blocks, n_cand, topk;
-    int per;   // pooled keys per CTA of the cluster (the last CTA's range may be shorter or empty)
+    int per;   // candidates (blocks) per CTA of the cluster (the last CTA's range may be shorter or empty)
+    // grid mode (f3): Kpool is the (32,16) compressed-key grid, 4 keys per block; keys_valid = 4*n_cand - 1 of them exist;
+    // blocks [0, n_init) and [n_cand - n_local, n_cand) are always selected
+    int keys_valid, n_init, n_local;
     // optional fused reuse plan (f1, reuse_plan.cuh): after the row's ids are out, one warp of the selecting CTA updates
     // the row's slot table and fetch list -- one launch less per layer of the cached decode step
     int32_t* slot_ids;
@@ -269,8 +272,9 @@ struct SelParams {
     int32_t* n_fetch;
 };
 
-template <int D>
+template <int D, bool GRID>
 __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(SelParams p) {
+    constexpr int KPB = GRID ? 4 : 1;                // keys per candidate block
     constexpr int LPK = D / 8;                       // lanes per key (16 B = 8 bf16 each)
     constexpr int KPL = 32 / LPK;                    // keys per warp-wide read
     constexpr int NW = SEL_THREADS / 32;
@@ -320,16 +324,17 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
 
     const int k_lo = min((int)c * p.per, p.n_cand);
     const int n_local = min(p.per, p.n_cand - k_lo);
-    const int n_st = (n_local + KPS - 1) / KPS;
+    const int n_keys_local = n_local * KPB;         // rows of Kpool this CTA streams
+    const int n_st = (n_keys_local + KPS - 1) / KPS;
 
     if (w == NW) {
         // =============================== producer warp: bulk copies into the ring ===============================
         if (lane == 0) {
-            const char* src = p.Kpool + ((size_t)r * p.n_blocks + k_lo) * ROW_BYTES;
+            const char* src = p.Kpool + ((size_t)r * p.n_blocks + k_lo) * KPB * ROW_BYTES;
             for (int i = 0; i < n_st; ++i) {
                 const int s = i % SEL_STAGES;
                 if (i >= SEL_STAGES) mbar_wait(&s_empty[s], ((i / SEL_STAGES) - 1) & 1);
-                const uint32_t bytes = (uint32_t)min(KPS, n_local - i * KPS) * ROW_BYTES;
+                const uint32_t bytes = (uint32_t)min(KPS, n_keys_local - i * KPS) * ROW_BYTES;
                 mbar_arrive_expect_tx(&s_full[s], bytes);
                 bulk_g2s(ring + (size_t)s * SEL_STAGE_BYTES, src + (size_t)i * SEL_STAGE_BYTES, bytes, &s_full[s]);
             }
@@ -345,13 +350,14 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
         uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
         for (int i = 0; i < n_st; ++i) {
             const int s = i % SEL_STAGES;
-            const int nk = min(KPS, n_local - i * KPS);
+            const int nk = min(KPS, n_keys_local - i * KPS);
             mbar_wait(&s_full[s], (i / SEL_STAGES) & 1);
             const uint8_t* st = ring + (size_t)s * SEL_STAGE_BYTES;
             uint4 kv[PASSES];
 #pragma unroll
             for (int ps = 0; ps < PASSES; ++ps) {
-                const int kl = ps * (NW * KPL) + w * KPL + sub;
+                // plain: pass ps takes key ps*16 + group; grid: the group takes the 4 keys of one block, one per pass
+                const int kl = GRID ? (w * KPL + sub) * 4 + ps : ps * (NW * KPL) + w * KPL + sub;
                 kv[ps] = kl < nk ? *reinterpret_cast<const uint4*>(st + (size_t)kl * ROW_BYTES + dl * 16) : make_uint4(0, 0, 0, 0);
             }
             __syncwarp();
@@ -385,12 +391,28 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
 #pragma unroll
             for (int o = LPK / 8; o >= 1; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
             const int mine = (hi1 ? 2 : 0) + (hi2 ? 1 : 0);
-            const int kl = mine * (NW * KPL) + w * KPL + sub;
-            if ((dl & (LPK / 4 - 1)) == 0 && kl < nk) {
-                const uint32_t key = orderable(tot + 0.0f);      // +0: -0 -> +0
-                st_cluster_u32(keys0 + 4u * (uint32_t)(k_lo + i * KPS + kl), key);
-                kmin = min(kmin, key);
-                kmax = max(kmax, key);
+            if (GRID) {
+                // f_top's max-pool (reading q19): block score = max over the compressed keys that start in the block
+                const int blk = i * (KPS / 4) + w * KPL + sub;                     // block within this CTA's range
+                const int jkey = (k_lo + blk) * 4 + mine;                            // compressed key index in the row
+                float bsc = jkey < p.keys_valid ? tot : -INFINITY;
+                bsc = fmaxf(bsc, __shfl_xor_sync(0xffffffffu, bsc, LPK / 2));
+                bsc = fmaxf(bsc, __shfl_xor_sync(0xffffffffu, bsc, LPK / 4));
+                if (dl == 0 && blk < n_local) {
+                    const int b = k_lo + blk;
+                    const bool forced = b < p.n_init || b >= p.n_cand - p.n_local;   // init / local blocks: always attended
+                    const uint32_t key = forced ? 0xFFFFFFFFu : orderable(bsc + 0.0f);
+                    st_cluster_u32(keys0 + 4u * (uint32_t)b, key);
+                    if (!forced) { kmin = min(kmin, key); kmax = max(kmax, key); }
+                }
+            } else {
+                const int kl = mine * (NW * KPL) + w * KPL + sub;
+                if ((dl & (LPK / 4 - 1)) == 0 && kl < nk) {
+                    const uint32_t key = orderable(tot + 0.0f);      // +0: -0 -> +0
+                    st_cluster_u32(keys0 + 4u * (uint32_t)(k_lo + i * KPS + kl), key);
+                    kmin = min(kmin, key);
+                    kmax = max(kmax, key);
+                }
             }
         }
         kmin = __reduce_min_sync(0xffffffffu, kmin);
@@ -451,6 +473,39 @@ __global__ void __launch_bounds__(256) pool_keys_kernel(const uint4* __restrict_
     kpool[rb * LPK + dl] = o;
 }
 
+// a0 for f3: compressed keys with overlapping windows, Eq.2 with (l_C, s) = (32, 16):
+// Kgrid[r,j,:] = bf16( (1/32) sum_{t=16j}^{16j+31} K[r,t,:] ), fp32 sum in ascending t; j < n_comp = T/16 - 1, the
+// remaining row of the [R][4*Nb][D] grid is zero.  D/8 lanes per compressed key.
+template <int D>
+__global__ void __launch_bounds__(256) pool_keys_grid_kernel(const uint4* __restrict__ kv, uint4* __restrict__ kgrid, int n_blocks,
+                                                              int64_t n_rj /* rows * 4 * n_blocks */) {
+    constexpr int LPK = D / 8, S = 64, WIN = 32, STR = 16;
+    const int64_t gthread = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t rj = gthread / LPK;
+    const int dl = (int)(gthread % LPK);
+    if (rj >= n_rj) return;
+    const int per_row = n_blocks * (S / STR);
+    const int64_t r = rj / per_row;
+    const int j = (int)(rj % per_row);
+    uint4 o = make_uint4(0, 0, 0, 0);
+    if (j < per_row - 1) {
+        float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll 8
+        for (int i = 0; i < WIN; ++i) {
+            const int t = j * STR + i;
+            const uint4 v = __ldg(kv + ((r * n_blocks + t / S) * 2 * S + (t % S)) * LPK + dl);   // plane 0 = K
+            acc[0] += bf16_lo(v.x); acc[1] += bf16_hi(v.x); acc[2] += bf16_lo(v.y); acc[3] += bf16_hi(v.y);
+            acc[4] += bf16_lo(v.z); acc[5] += bf16_hi(v.z); acc[6] += bf16_lo(v.w); acc[7] += bf16_hi(v.w);
+        }
+        const float inv = 1.0f / WIN;
+        o.x = pack_bf16(acc[0] * inv, acc[1] * inv);
+        o.y = pack_bf16(acc[2] * inv, acc[3] * inv);
+        o.z = pack_bf16(acc[4] * inv, acc[5] * inv);
+        o.w = pack_bf16(acc[6] * inv, acc[7] * inv);
+    }
+    kgrid[rj * LPK + dl] = o;
+}
+
 // f2, Alg.2 lines 2-3: append the new token's K and V at position t of every row's cache (device-resident, or
 // pinned host memory written through UVA: the asynchronous write-back of P:L159) and update the pooled keys incrementally
 // (P:L89): ksum accumulates the open block's keys in fp32 in arrival (= ascending t) order, exactly the sum order of
@@ -496,10 +551,10 @@ __global__ void __launch_bounds__(256) append_kv_kernel(const uint4* __restrict_
 // such a cluster (asked once per size; sizes above 8 are non-portable and need the opt-in attribute).  Measured on
 // B200 (batch 32, 2048 blocks, cold HBM): a 6 x 16 KiB ring streams as fast as 10 stages and lets two CTAs share an
 // SM, so with R > SM count the selection of one row overlaps the stream of the next.
-template <int D>
+template <int D, bool GRID>
 static int select_launch(sparda_ctx* ctx, const SelParams& p0, cudaStream_t st) {
-    auto kern = forecast_select_kernel<D>;
-    constexpr int KPS = SEL_STAGE_BYTES / (D * 2);
+    auto kern = forecast_select_kernel<D, GRID>;
+    constexpr int KPS = SEL_STAGE_BYTES / (D * 2) / (GRID ? 4 : 1);   // candidates per stage
     static bool attr_set = false;
     static int cluster_ok[SEL_MAX_CS + 1];   // 0 = not asked, 1 = schedulable, -1 = not
     const size_t smem_max = 127 + (size_t)SEL_STAGES * SEL_STAGE_BYTES + (size_t)ctx->cfg.max_blocks * sizeof(uint32_t);
@@ -559,7 +614,31 @@ int sparda_launch_select(sparda_ctx* ctx, const void* F, const void* Kpool, int 
     p.n_cand = n_cand;
     p.topk = topk;
     p.per = n_cand;
-    int rc = ctx->cfg.head_dim == 128 ? select_launch<128>(ctx, p, st) : select_launch<64>(ctx, p, st);
+    p.keys_valid = n_cand;
+    p.n_init = p.n_local = 0;
+    int rc = ctx->cfg.head_dim == 128 ? select_launch<128, false>(ctx, p, st) : select_launch<64, false>(ctx, p, st);
+    if (rc) return rc;
+    ctx->launches++;
+    return SPARDA_OK;
+}
+
+// f3: the same launch over the (32,16) compressed-key grid [R][4*n_blocks][D] with the max-pool to blocks and the
+// init / local blocks forced in (reading q19).
+int sparda_launch_select_grid(sparda_ctx* ctx, const void* F, const void* Kgrid, int n_blocks, int n_cand, int n_init, int n_local,
+                              int topk, int32_t* ids, cudaStream_t st) {
+    SelParams p;
+    p.slot_ids = p.fetch = p.n_fetch = nullptr;
+    p.F = (const uint4*)F;
+    p.Kpool = (const char*)Kgrid;
+    p.ids = ids;
+    p.n_blocks = n_blocks;
+    p.n_cand = n_cand;
+    p.topk = topk;
+    p.per = n_cand;
+    p.keys_valid = 4 * n_cand - 1;
+    p.n_init = n_init;
+    p.n_local = n_local;
+    int rc = ctx->cfg.head_dim == 128 ? select_launch<128, true>(ctx, p, st) : select_launch<64, true>(ctx, p, st);
     if (rc) return rc;
     ctx->launches++;
     return SPARDA_OK;
@@ -588,6 +667,19 @@ int sparda_launch_append_kv(sparda_ctx* ctx, const void* k_new, const void* v_ne
         append_kv_kernel<128><<<grid, 256, 0, st>>>((const uint4*)k_new, (const uint4*)v_new, (uint4*)kv, ksum, (uint4*)kpool, ctx->R, n_blocks, t);
     else
         append_kv_kernel<64><<<grid, 256, 0, st>>>((const uint4*)k_new, (const uint4*)v_new, (uint4*)kv, ksum, (uint4*)kpool, ctx->R, n_blocks, t);
+    SPARDA_CUDA_TRY(ctx, cudaGetLastError());
+    ctx->launches++;
+    return SPARDA_OK;
+}
+
+int sparda_launch_pool_keys_grid(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_blocks, void* kgrid, cudaStream_t st) {
+    const int64_t n_rj = n_rows * n_blocks * 4;
+    const int lpk = ctx->cfg.head_dim / 8;
+    const unsigned grid = (unsigned)((n_rj * lpk + 255) / 256);
+    if (ctx->cfg.head_dim == 128)
+        pool_keys_grid_kernel<128><<<grid, 256, 0, st>>>((const uint4*)kv, (uint4*)kgrid, n_blocks, n_rj);
+    else
+        pool_keys_grid_kernel<64><<<grid, 256, 0, st>>>((const uint4*)kv, (uint4*)kgrid, n_blocks, n_rj);
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;
     return SPARDA_OK;

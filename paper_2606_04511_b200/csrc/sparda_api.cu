@@ -166,6 +166,20 @@ int sparda_forecast_select(sparda_ctx* ctx, const void* F, const void* Kpool, in
     return sparda_launch_select(ctx, F, Kpool, n_blocks, n_cand, topk, ids_out, nullptr, nullptr, nullptr, (cudaStream_t)stream);
 }
 
+int sparda_pool_keys_grid(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_blocks, void* kgrid, void* stream) {
+    if (!ctx || !sparda_aligned(kv, 16) || !sparda_aligned(kgrid, 16) || n_rows < 1 || n_blocks < 1) return SPARDA_EINVAL;
+    if (n_rows * (int64_t)n_blocks > (int64_t)1 << 29) return SPARDA_EINVAL;
+    return sparda_launch_pool_keys_grid(ctx, kv, n_rows, n_blocks, kgrid, (cudaStream_t)stream);
+}
+
+int sparda_forecast_select_grid(sparda_ctx* ctx, const void* F, const void* Kgrid, int n_blocks, int n_cand, int n_init, int n_local,
+                                int topk, int32_t* ids_out, void* stream) {
+    if (!ctx || !sparda_aligned(F, 16) || !sparda_aligned(Kgrid, 16) || !sparda_aligned(ids_out, 4)) return SPARDA_EINVAL;
+    if (n_blocks < 1 || n_blocks > ctx->cfg.max_blocks || n_cand < 0 || n_cand > n_blocks) return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk || n_init < 0 || n_local < 0 || n_init + n_local > topk) return SPARDA_EINVAL;
+    return sparda_launch_select_grid(ctx, F, Kgrid, n_blocks, n_cand, n_init, n_local, topk, ids_out, (cudaStream_t)stream);
+}
+
 int sparda_forecast_select_plan(sparda_ctx* ctx, const void* F, const void* Kpool, int n_blocks, int n_cand, int topk,
                                 int32_t* ids_out, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch, void* stream) {
     if (!ctx || !sparda_aligned(F, 16) || !sparda_aligned(Kpool, 16) || !sparda_aligned(ids_out, 4)) return SPARDA_EINVAL;

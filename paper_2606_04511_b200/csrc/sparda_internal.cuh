@@ -66,6 +66,9 @@ int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_bl
                          cudaStream_t);
 int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
                          cudaStream_t);
+int sparda_launch_pool_keys_grid(sparda_ctx*, const void* kv, int64_t n_rows, int n_blocks, void* kgrid, cudaStream_t);
+int sparda_launch_select_grid(sparda_ctx*, const void* F, const void* Kgrid, int n_blocks, int n_cand, int n_init, int n_local, int topk,
+                              int32_t* ids, cudaStream_t);
 int sparda_launch_append_kv(sparda_ctx*, const void* k_new, const void* v_new, int64_t t, void* kv, int n_blocks, float* ksum,
                             void* kpool, cudaStream_t);
 int sparda_launch_reuse_plan(sparda_ctx*, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch,

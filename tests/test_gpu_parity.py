@@ -512,6 +512,55 @@ def test_append_kv_matches_oracle(cfg, where, sp, oracle):
         parity.check_attn(_bits(O), wantO, "attention on the appended cache")
 
 
+GRID_CASES = [synth.DecodeConfig("grid_d128", batch=2, n_q_heads=32, n_kv_heads=2, head_dim=128, n_blocks=150, topk=96, seed=71),
+              synth.DecodeConfig("grid_d64", batch=3, n_q_heads=4, n_kv_heads=1, head_dim=64, n_blocks=77, topk=20, seed=72, bias_std=2.0)]
+
+
+@pytest.mark.parametrize("cfg", GRID_CASES, ids=lambda c: c.name)
+def test_pool_keys_grid_and_select_grid(cfg, sp, oracle):
+    """f3 (o14 / o15, reading q19 -- unpinned by the paper): (32,16) compressed keys within 1 bf16 ulp of the fp64 oracle;
+    grid selection with the max-pool to blocks and forced initial / local blocks against the oracle on the SAME grid,
+    over candidate ranges that leave ragged per-CTA block ranges, and the paper's budget 96 = 1 + 32 + 63."""
+    L, ctx, _ = _setup(cfg, sp)
+    R, Nb, D, k = cfg.rows, cfg.n_blocks, cfg.head_dim, cfg.topk
+    kgrid = torch.full((R, 4 * Nb, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    ctx.pool_keys_grid(L["kv"], R, Nb, kgrid)
+    torch.cuda.synchronize()
+    want_grid = oracle.pool_keys_grid(_bits(L["kv"]))
+    ulps = parity.ulp_diff_bf16(_bits(kgrid), want_grid)
+    assert ulps.max() <= 1 and (ulps > 0).mean() < 1e-3
+    grid_dev = torch.from_numpy(want_grid.view(np.int16)).view(torch.bfloat16).cuda()
+    n_init, n_local = (1, 32) if k == 96 else (2, 5)
+    for n_cand, ni, nl in [(Nb, n_init, n_local), (Nb - 7, n_init, n_local), (Nb, 0, 0), (k + 1, n_init, n_local), (k, n_init, n_local), (3, 1, 1)]:
+        ids = torch.full((R, k), -7, dtype=torch.int32, device="cuda")
+        ctx.forecast_select_grid(L["F"], grid_dev, Nb, k, ids, n_init=ni, n_local=nl, n_cand=n_cand)
+        torch.cuda.synchronize()
+        want, bs = oracle.forecast_select_grid(_bits(L["F"]), want_grid, k, n_cand, ni, nl)
+        got = ids.cpu().numpy()
+        forced = [b for b in range(n_cand) if b < ni or b >= n_cand - nl]
+        assert all(set(forced) <= set(got[r].tolist()) for r in range(R)), "initial / local blocks must always be selected"
+        finite = np.where(np.isinf(bs), np.float32(3.0e38), bs)
+        parity.check_ids(got, want, finite, n_cand)
+
+
+def test_select_grid_full_size_128k(sp, oracle):
+    """The paper's shape at 128K: 2048 blocks, 8191 compressed keys per row, budget 96 = 1 initial + 32 local + 63
+    ranked; batch 4 (16 CTAs per row) and batch 32 (2 per row)."""
+    for batch in (4, 32):
+        cfg = synth.DecodeConfig("grid128k", batch=batch, n_q_heads=32, n_kv_heads=2, head_dim=128, n_blocks=2048, topk=96, seed=73)
+        ctx = sp.Sparda.from_config(cfg)
+        g = torch.Generator(device="cuda").manual_seed(73 + batch)
+        R, Nb = cfg.rows, cfg.n_blocks
+        bias = torch.randn((R, Nb, 1, 1), generator=g, device="cuda") * 1.5
+        grid = (torch.randn((R, Nb, 4, 128), generator=g, device="cuda") * 0.2 + bias).to(torch.bfloat16).reshape(R, 4 * Nb, 128).contiguous()
+        F = torch.randn((R, 128), generator=g, device="cuda").to(torch.bfloat16)
+        ids = torch.full((R, 96), -7, dtype=torch.int32, device="cuda")
+        ctx.forecast_select_grid(F, grid, Nb, 96, ids, n_init=1, n_local=32)
+        torch.cuda.synchronize()
+        want, bs = oracle.forecast_select_grid(_bits(F), _bits(grid), 96, Nb, 1, 32)
+        parity.check_ids(ids.cpu().numpy(), want, np.where(np.isinf(bs), np.float32(3.0e38), bs), Nb)
+
+
 def test_cfg2_full_size_layer(sp, oracle):
     """BASELINE.json configs[1] at full size: batch 8, 32/2 heads, D=128, 512 blocks, top-64, KV pinned on host."""
     cfg = synth.CFG2_32K

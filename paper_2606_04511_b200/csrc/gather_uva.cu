@@ -21,8 +21,12 @@ namespace {
 
 using namespace sparda;
 
-constexpr int GATHER_STAGE_BYTES = 16384;
-constexpr int GATHER_STAGES = 6;  // 96 KiB ring per CTA, up to 5 loads in flight while one stage drains
+#ifndef GATHER_STAGE_BYTES_V
+#define GATHER_STAGE_BYTES_V 16384
+#define GATHER_STAGES_V 6
+#endif
+constexpr int GATHER_STAGE_BYTES = GATHER_STAGE_BYTES_V;
+constexpr int GATHER_STAGES = GATHER_STAGES_V;  // 96 KiB ring per CTA, up to 5 loads in flight while one stage drains
 
 constexpr int GATHER_WIN = 1024;  // tasks compacted per window (32 per lane, held in registers)
 

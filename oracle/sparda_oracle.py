@@ -1,9 +1,12 @@
 """numpy/ctypes wrapper around ``sparda_oracle.c`` -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
 
-Argument marshalling only; every number is computed by the plain C loops in
-``sparda_oracle.c`` (which cites the paper passage each function follows).  ``decode_pipeline``
-(o10) is the one function written here: it is Algorithm 2 lines 4-7 run strictly
-in order, calling o3-o6 layer by layer.
+o1-o9: argument marshalling only; every number is computed by the plain C loops in ``sparda_oracle.c`` (which cites
+the paper passage each function follows).  Written here, as plain Python / numpy loops that call those:
+``decode_pipeline`` (o10: Algorithm 2 lines 4-7, strictly in order), ``reuse_plan`` /
+``decode_pipeline_cached`` (o11 / o12: the previous-step block cache, reading q18), ``append_kv`` (o13: Algorithm 2
+lines 2-3) and ``pool_keys_grid`` / ``forecast_select_grid`` (o14 / o15: the (32,16) compressed-key grid with
+the max-pool to blocks, reading q19 -- PARITY UNPINNED BY THE PAPER, which does not state the pooling geometry).
+Every function is pinned in ``tests/test_oracle_pins.py``.
 
 bf16 tensors are numpy ``uint16`` arrays holding the raw upper halves of fp32 values.
 """

@@ -282,8 +282,8 @@ def bench_kernels_b32(torch, binding, peaks, args):
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": b / t / 1e9 / peaks["hbm_gbs"],
                     "frac_of_nominal_8tbs": b / t / 1e9 / 8000.0, "peak_source": peaks["source"], "traffic": None})
     # DRAM read + write bytes per launch of the same shapes from the committed ncu --set full captures
-    out[0]["traffic"], out[0]["traffic_source"] = 33612800, "profiles/r1b_ncu_summary.md (prof_b32_select_b: dram read 33.61 MB, write 0)"
-    out[1]["traffic"], out[1]["traffic_source"] = 134556160 + 4178688, "profiles/r1b_ncu_summary.md (prof_b32_attn_b: dram read 134.56 MB, write 4.18 MB of split-K partials)"
+    out[0]["traffic"], out[0]["traffic_source"] = 33612800, "profiles/r1c_ncu_summary.md (prof_b32_select_c: dram read 33.61 MB, write 0)"
+    out[1]["traffic"], out[1]["traffic_source"] = 134556160 + 4178688, "profiles/r1c_ncu_summary.md (prof_b32_attn_c: dram read 134.56 MB, write 4.18 MB of split-K partials)"
     out[1]["attn_splits"] = ctx.attn_splits(k)
     out[2]["workload"] = ("f3 (reading q19, unpinned by the paper): batch 32, 2048 blocks x 4 compressed keys, max-pool to blocks, "
                           "top-96 = 1 initial + 32 local + 63 ranked; cold HBM (two 128 MiB grids > L2), CUDA-graph replay")
@@ -615,7 +615,7 @@ def run_sparda(args):
                 "bound": "host_link", "achieved": gather_bytes / t_gat / 1e9, "peak": ceiling, "unit": "GB/s",
                 "frac": gather_bytes / t_gat / 1e9 / ceiling,
                 "traffic": 56064 if cfg.name == "cfg3_128k_pipeline" else None,
-                "traffic_note": "DRAM bytes of one batch-4 launch (ncu, profiles/r1b_ncu_summary.md): the ids only; the payload crosses the "
+                "traffic_note": "DRAM bytes of one batch-4 launch (ncu, profiles/r1c_ncu_summary.md): the ids only; the payload crosses the "
                                 "host link (sysmem read sectors x 32 B = the algorithmic 16 MiB, profiles/r1_ncu_summary.md) and lands in L2",
                 "peak_source": "cudaMemcpyAsync pinned host->device, measured in this run on this box",
                 "us_per_launch": t_gat * 1e6, "algorithmic_bytes": gather_bytes,

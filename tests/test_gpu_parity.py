@@ -606,6 +606,17 @@ def test_argument_validation(sp):
         ctx.forecast_select(0, t, 64, 8, ids)                        # null pointer
     with pytest.raises(sp.SpardaError):
         ctx.sparse_decode(t, t[4:], ids, 8, t)                       # pool not 16-byte aligned
+    with pytest.raises(sp.SpardaError):
+        ctx.forecast_select_grid(t, t, 64, 8, ids, n_init=4, n_local=5)      # forced blocks exceed the budget
+    with pytest.raises(sp.SpardaError):
+        ctx.reuse_plan(ids, 9, ids, ids)                             # topk > configured
+    with pytest.raises(sp.SpardaError):
+        ctx.forecast_select_plan(t, t, 64, 8, ids, 0, ids)           # null slot table
+    ksum = torch.zeros(64, dtype=torch.float32, device="cuda")
+    with pytest.raises(sp.SpardaError):
+        ctx.append_kv(t, t, 64 * 64, t, 64, ksum, t)                 # position beyond the cache
+    with pytest.raises(sp.SpardaError):
+        ctx.append_kv(t, t, -1, t, 64, ksum, t)
 
 
 # ------------------------------------------------------------------------------------------------

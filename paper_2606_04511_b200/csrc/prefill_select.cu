@@ -17,9 +17,12 @@
 // combining per-row partial results through shared memory behind a named barrier.  Per row, all in registers except a
 // <= 24-entry boundary list:
 //   pass 0   row min / max
-//   7 passes bisection over 128 equal-width value buckets of [min, max]: count(s >= t) per pass
-//   pass 8   collect the elements of the boundary bucket (value, id); exact k-th by (value desc, id asc) among them
-//   pass 9   selected count per chunk;  pass 10  emit ids with s > T or (s == T and id <= id_T) at the chunk's offset
+//   search   over equal-width value buckets of [min, max]: count(s >= t) per pass, 7 one-threshold passes over 128 buckets
+//            (4 three-threshold passes over 256 buckets in the replicated mode below)
+//   collect  the elements of the boundary bucket (value, id); the parts rank them by (value desc, id asc) between them:
+//            the k-th is the threshold T, with id_T the last id taken among its equals
+//   count    selected elements per chunk;  emit  ids with s > T or (s == T and id <= id_T) at the chunk's offset of the
+//            row's output in global memory
 // Columns beyond a row's causal candidates read as -inf, so the passes compare values only.  A row whose boundary
 // bucket holds more than 24 elements (heavy ties) takes an exact bitwise radix search over order-preserving keys in
 // part 0 alone (33 passes; warp-uniform because tcgen05.ld is warp-collective), which hands (T, id_T) to the others.
@@ -27,6 +30,19 @@
 // into softmax probabilities (two TMEM passes) summed into an L2-resident per-CTA scratch tile, and runs the same
 // selection on that tile.
 #include "sparda_internal.cuh"
+
+#ifdef SPARDA_TRACE
+__device__ unsigned long long* g_pf_trace;   // [gridDim.x][32] globaltimer stamps of warp 2 lane 0 (debug builds only)
+extern "C" void sparda_debug_set_pf_trace(unsigned long long* p) { cudaMemcpyToSymbol(g_pf_trace, &p, sizeof(p)); }
+#define PF_TRACE(i)                                                                           \
+    if (threadIdx.x == 64) {                                                                  \
+        unsigned long long t__;                                                               \
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));                               \
+        g_pf_trace[blockIdx.x * 32 + (i)] = t__;                                              \
+    }
+#else
+#define PF_TRACE(i)
+#endif
 
 namespace {
 
@@ -43,7 +59,6 @@ constexpr int PF_CAP = 24;        // boundary-list capacity per row
 constexpr int PF_LIST_WORDS = 2 * PF_CAP;
 constexpr int PF_WSTRIDE = 129;   // words between a thread's consecutive private words (bank-conflict free)
 constexpr int PF_MAXK = 64;       // ids staged per row
-constexpr int PF_OPITCH = PF_ROWS * 2 + 4;  // bytes between consecutive output positions (u16 per thread)
 constexpr int PF_BUCKET_BITS = 7;
 
 template <int D>
@@ -54,8 +69,7 @@ struct PfSmem {
     static constexpr int OFF_B = 0;
     static constexpr int OFF_A = OFF_B + KH * B_SLAB;
     static constexpr int OFF_LIST = OFF_A + KH * A_SLAB;
-    static constexpr int OFF_OUT = OFF_LIST + PF_LIST_WORDS * PF_WSTRIDE * 4;
-    static constexpr int OFF_STAT = OFF_OUT + PF_MAXK * PF_OPITCH;          // a7': (m, 1/l) per row, 1 KB
+    static constexpr int OFF_STAT = OFF_LIST + PF_LIST_WORDS * PF_WSTRIDE * 4;   // a7': (m, 1/l) per row, 1 KB
     static constexpr int OFF_COMB = OFF_STAT + PF_ROWS * 8;                   // exchange cells: [2][PF_NP][rows] float2
     static constexpr int OFF_NLIST = OFF_COMB + 2 * PF_NP * PF_ROWS * 8;      // boundary-list length per row
     static constexpr int OFF_CCNT = OFF_NLIST + PF_ROWS * 4;                  // selected count per (chunk, row), u8
@@ -163,32 +177,35 @@ __device__ __forceinline__ float key_to_float(uint32_t key) {
 // between them (chunk c belongs to part c % PF_NP) and combine per-row partial results through shared memory:
 // write own partial, named barrier of the quadrant's PF_NP warps, read all parts.  Two buffers alternate, so one
 // barrier per exchange is enough.
+template <int NP>
 struct PartComm {
-    float2* comb;       // this row's cell of part 0, buffer 0; part stride PF_ROWS, buffer stride PF_NP * PF_ROWS
+    float2* comb;       // this row's cell of part 0, buffer 0; part stride PF_ROWS / (NP / PF_NP), see cell()
     int part, bar_id, buf;
-    __device__ __forceinline__ void sync() const { asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(PF_NP * 32) : "memory"); }
+    // cells: [2 buffers][NP parts][PF_ROWS * PF_NP / NP rows]: 4 parts x 128 rows, or 16 parts x 32 rows (replicated tile)
+    static constexpr int ROWS = PF_ROWS * PF_NP / NP;
+    __device__ __forceinline__ void sync() const { asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(NP * 32) : "memory"); }
     __device__ __forceinline__ void put(float2 v) {
         buf ^= 1;
-        comb[(buf * PF_NP + part) * PF_ROWS] = v;
+        comb[(buf * NP + part) * ROWS] = v;
         sync();
     }
-    __device__ __forceinline__ float2 get(int p) const { return comb[(buf * PF_NP + p) * PF_ROWS]; }
+    __device__ __forceinline__ float2 get(int p) const { return comb[(buf * NP + p) * ROWS]; }
     __device__ __forceinline__ int sum_int(int a) {
         put(make_float2(__int_as_float(a), 0.f));
         int s = 0;
 #pragma unroll
-        for (int p = 0; p < PF_NP; ++p) s += __float_as_int(get(p).x);
+        for (int p = 0; p < NP; ++p) s += __float_as_int(get(p).x);
         return s;
     }
 };
 
 // Exact per-row top-k of src[0 .. ncand) for the PF_NP threads that own one query row (one per part); the whole quadrant
 // group calls it together (loads are warp-collective, exchanges are group barriers); a thread with active == false
-// only keeps the others company.  On return the row's k ids (ascending) are staged as u16 at out_base[pos * PF_OPITCH].
-template <class Src>
-__device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int k, bool active, PartComm& pc,
+// only keeps the others company.  The row's k ids are written to dst in ascending order.
+template <int BPP, class Src, int NP>
+__device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int k, bool active, PartComm<NP>& pc,
                                          uint32_t* list /* row's list, stride PF_WSTRIDE */, uint32_t* n_list /* row's counter */,
-                                         uint8_t* chunk_cnt /* row's [16] chunk counts, stride PF_ROWS */, uint8_t* out_base) {
+                                         uint8_t* chunk_cnt /* row's [16] chunk counts, stride PF_ROWS */, int32_t* dst /* row's k ids in global memory */) {
     float v[32];
     const float NEG = -INFINITY;
     const int part = pc.part;
@@ -205,7 +222,7 @@ __device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int
     };
     // ---- pass 0: min / max over the candidates
     float lo = INFINITY, hi = -INFINITY;
-    for (int c = part; c < nch; c += PF_NP) {
+    for (int c = part; c < nch; c += NP) {
         src.load(c, v);
 #pragma unroll
         for (int e = 0; e < 32; ++e)
@@ -213,36 +230,64 @@ __device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int
     }
     pc.put(make_float2(lo, hi));
 #pragma unroll
-    for (int p = 0; p < PF_NP; ++p) { const float2 o = pc.get(p); lo = fminf(lo, o.x); hi = fmaxf(hi, o.y); }
-    // ---- bisection over 2^7 equal-width buckets: largest bucket edge t_b with count(s >= t_b) >= k
-    const float w = (hi - lo) * (1.0f / (1 << PF_BUCKET_BITS));
-    int blo = 0, bhi = 1 << PF_BUCKET_BITS;          // count(s >= t_blo) >= k > count(s >= t_bhi);  t_128 = +inf
+    for (int p = 0; p < NP; ++p) { const float2 o = pc.get(p); lo = fminf(lo, o.x); hi = fmaxf(hi, o.y); }
+    PF_TRACE(2);
+    // ---- bucket search over 2^PF_BUCKET_BITS equal-width buckets of [min, max]: the largest bucket edge t_b with
+    // count(s >= t_b) >= k.  BPP bits per pass: one threshold per pass (7 passes) when a thread holds several chunks, three
+    // thresholds per pass (4 passes) in the replicated mode, where a pass is one chunk and mostly exchange latency.
+    // Counts are accumulated as floats (FSET + FADD; exact up to 2^24).
+    constexpr int NBITS = BPP == 2 ? 8 : PF_BUCKET_BITS;
+    const float w = (hi - lo) * (1.0f / (1 << NBITS));
+    int blo = 0, bhi = 1 << NBITS;                    // count(s >= t_blo) >= k > count(s >= t_bhi);  t_top = +inf
     int c_lo = ncand, c_hi = 0;
 #pragma unroll 1
-    for (int step = 0; step < PF_BUCKET_BITS; ++step) {
-        const int mid = (blo + bhi) >> 1;
-        const float t = fmaf((float)mid, w, lo);
-        int cnt0 = 0, cnt1 = 0;
-        for (int c = part; c < nch; c += PF_NP) {
-            load(c, v);
+    for (int step = 0; step < NBITS / BPP; ++step) {
+        if (BPP == 1) {
+            const int mid = (blo + bhi) >> 1;
+            const float t = fmaf((float)mid, w, lo);
+            float cnt0 = 0.f, cnt1 = 0.f;
+            for (int c = part; c < nch; c += NP) {
+                load(c, v);
 #pragma unroll
-            for (int e = 0; e < 32; e += 2) {
-                cnt0 += v[e] >= t ? 1 : 0;
-                cnt1 += v[e + 1] >= t ? 1 : 0;
+                for (int e = 0; e < 32; e += 2) {
+                    cnt0 += v[e] >= t ? 1.0f : 0.0f;
+                    cnt1 += v[e + 1] >= t ? 1.0f : 0.0f;
+                }
             }
+            const int cnt = pc.sum_int((int)(cnt0 + cnt1));
+            if (cnt >= k) { blo = mid; c_lo = cnt; } else { bhi = mid; c_hi = cnt; }
+        } else {
+            const int q = (bhi - blo) >> 2;
+            const float t1 = fmaf((float)(blo + q), w, lo), t2 = fmaf((float)(blo + 2 * q), w, lo), t3 = fmaf((float)(blo + 3 * q), w, lo);
+            float n1 = 0.f, n2 = 0.f, n3 = 0.f;
+            for (int c = part; c < nch; c += NP) {
+                load(c, v);
+#pragma unroll
+                for (int e = 0; e < 32; ++e) {
+                    n1 += v[e] >= t1 ? 1.0f : 0.0f;
+                    n2 += v[e] >= t2 ? 1.0f : 0.0f;
+                    n3 += v[e] >= t3 ? 1.0f : 0.0f;
+                }
+            }
+            // three counts <= 512 each in one word: the sum over the parts cannot carry between the 10-bit fields
+            const int packed = pc.sum_int((int)n1 | ((int)n2 << 10) | ((int)n3 << 20));
+            const int c1 = packed & 1023, c2 = (packed >> 10) & 1023, c3 = (packed >> 20) & 1023;
+            if (c3 >= k) { blo += 3 * q; c_lo = c3; }
+            else if (c2 >= k) { blo += 2 * q; bhi = blo + q; c_lo = c2; c_hi = c3; }
+            else if (c1 >= k) { blo += q; bhi = blo + q; c_lo = c1; c_hi = c2; }
+            else { bhi = blo + q; c_hi = c1; }
         }
-        const int cnt = pc.sum_int(cnt0 + cnt1);
-        if (cnt >= k) { blo = mid; c_lo = cnt; } else { bhi = mid; c_hi = cnt; }
+        PF_TRACE(3 + step);
     }
     const float tlo = fmaf((float)blo, w, lo);
-    const float thi = bhi == (1 << PF_BUCKET_BITS) ? INFINITY : fmaf((float)bhi, w, lo);
+    const float thi = bhi == (1 << NBITS) ? INFINITY : fmaf((float)bhi, w, lo);
     const int need = k - c_hi;                        // how many of the boundary bucket are selected (>= 1)
     const int n_b = c_lo - c_hi;                      // population of the boundary bucket
     const bool slow = active && (n_b > PF_CAP);
     float T = NEG;                                    // k-th largest value
     int jT = -1;                                      // selected among s == T: ids <= jT
     // ---- collect the boundary bucket (any order; entries carry their id) and resolve it exactly
-    for (int c = part; c < nch; c += PF_NP) {
+    for (int c = part; c < nch; c += NP) {
         load(c, v);
 #pragma unroll
         for (int e = 0; e < 32; ++e) {
@@ -257,18 +302,42 @@ __device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int
         }
     }
     pc.sync();
-    if (active && !slow) {
-        // the need-th largest of the list by (value desc, id asc), redundantly in every part
-        for (int e = 0; e < n_b; ++e) {
-            const float se = __uint_as_float(list[(2 * e) * PF_WSTRIDE]);
-            const int je = (int)list[(2 * e + 1) * PF_WSTRIDE];
-            int rank = 0;
-            for (int f = 0; f < n_b; ++f) {
-                const float sf = __uint_as_float(list[(2 * f) * PF_WSTRIDE]);
-                const int jf = (int)list[(2 * f + 1) * PF_WSTRIDE];
-                rank += (sf > se || (sf == se && jf < je)) ? 1 : 0;
+    PF_TRACE(10);
+    {
+        // the need-th largest of the list by (value desc, id asc): part p ranks the members e = p, p + NP, ... (their
+        // ranks are distinct, so exactly one part finds the k-th) and the finder hands (T, jT) to the others
+        float Tm = NEG;
+        int jm = -1;
+        if (active && !slow) {
+            for (int e = part; e < n_b; e += NP) {
+                const float se = __uint_as_float(list[(2 * e) * PF_WSTRIDE]);
+                const int je = (int)list[(2 * e + 1) * PF_WSTRIDE];
+                int rank = 0;
+                int f = 0;
+                for (; f + 4 <= n_b; f += 4) {       // four independent loads in flight
+                    float sf[4];
+                    int jf[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        sf[u] = __uint_as_float(list[(2 * (f + u)) * PF_WSTRIDE]);
+                        jf[u] = (int)list[(2 * (f + u) + 1) * PF_WSTRIDE];
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) rank += (sf[u] > se || (sf[u] == se && jf[u] < je)) ? 1 : 0;
+                }
+                for (; f < n_b; ++f) {
+                    const float sf = __uint_as_float(list[(2 * f) * PF_WSTRIDE]);
+                    const int jf = (int)list[(2 * f + 1) * PF_WSTRIDE];
+                    rank += (sf > se || (sf == se && jf < je)) ? 1 : 0;
+                }
+                if (rank == need - 1) { Tm = se; jm = je; }
             }
-            if (rank == need - 1) { T = se; jT = je; }
+        }
+        pc.put(make_float2(Tm, __int_as_float(jm)));
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const float2 o = pc.get(p);
+            if (__float_as_int(o.y) >= 0) { T = o.x; jT = __float_as_int(o.y); }
         }
     }
     // ---- heavy ties (rare): part 0 alone searches the k-th largest order-preserving key bit by bit over all chunks, finds
@@ -306,9 +375,10 @@ __device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int
         pc.put(make_float2(T, __int_as_float(jT)));
         if (slow) { const float2 o = pc.get(0); T = o.x; jT = __float_as_int(o.y); }
     }
+    PF_TRACE(11);
     // ---- selected element: s > T, or s == T with id <= jT (+-0 compare equal, as in the oracle's ordering).  Count per
-    // chunk, exchange, then emit every chunk at its offset: ascending ids.
-    for (int c = part; c < nch; c += PF_NP) {
+    // chunk, exchange, then every chunk writes its ids at its offset of the row's output: ascending ids.
+    for (int c = part; c < nch; c += NP) {
         load(c, v);
         int n = 0;
 #pragma unroll
@@ -319,25 +389,33 @@ __device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int
         chunk_cnt[c * PF_ROWS] = (uint8_t)n;
     }
     pc.sync();
-    for (int c = part; c < nch; c += PF_NP) {
+    PF_TRACE(12);
+    for (int c = part; c < nch; c += NP) {
         int pos = 0;
-        for (int cc = 0; cc < c; ++cc) pos += chunk_cnt[cc * PF_ROWS];
+#pragma unroll
+        for (int cc = 0; cc < PF_MAXN / 32; ++cc) {     // independent loads; chunks at or beyond nch are never read as < c
+            const int n = cc < c ? (int)chunk_cnt[cc * PF_ROWS] : 0;
+            pos += n;
+        }
         load(c, v);
 #pragma unroll
         for (int e = 0; e < 32; ++e) {
             const int j = c * 32 + e;
-            if ((v[e] > T || (v[e] == T && j <= jT)) && pos < PF_MAXK) {
-                *reinterpret_cast<uint16_t*>(out_base + pos * PF_OPITCH) = (uint16_t)j;
-                ++pos;
-            }
+            if ((v[e] > T || (v[e] == T && j <= jT)) && pos < k) dst[pos++] = j;
         }
     }
-    pc.sync();   // the staged ids of the row are complete
 }
 
-template <int D, bool BASELINE>
+// REPL (chunk launches with few tiles): a CTA owns 32 query rows instead of 128.  Its A tile holds the same 32 rows four
+// times (four 32-row TMA boxes), so the four TMEM lane quadrants carry four copies of the rows' scores and ALL 16 epilogue
+// warps work on those 32 rows, 16 threads per row (chunk c -> part c % 16).  The contraction is done four times over --
+// it is ~1 % of the kernel -- and a 2048-row chunk spreads over 128 CTAs instead of 32.
+template <int D, bool BASELINE, bool REPL>
 __global__ void __launch_bounds__(PF_THREADS, 1)
 prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB, PfParams p) {
+    constexpr int TROWS = REPL ? 32 : PF_ROWS;        // query rows per tile
+    constexpr int NP = REPL ? 4 * PF_NP : PF_NP;      // threads per query row
+    static_assert(!REPL || PF_NP == 4, "the replicated mode spreads a row over 16 epilogue warps");
     using SM = PfSmem<D>;
     constexpr int KH = SM::KH;
     extern __shared__ uint8_t smem_raw[];
@@ -372,6 +450,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    PF_TRACE(0);
 
     // Tile schedule (identical in every role): tiles sorted by cost (descending row index), dealt in a snake over the
     // group's CTAs.  Tile s covers rows [m0, m0 + 128), m0 = (mt_lo + n_tiles - 1 - s) * 128.
@@ -380,7 +459,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
         return s < p.n_tiles ? (p.mt_lo + p.n_tiles - 1 - s) : -1;
     };
     const int n_rounds = (p.n_tiles + n_cta - 1) / n_cta;
-    auto tile_ncols = [&](int mt) -> int { return min(p.n_blocks, (mt * PF_ROWS + PF_ROWS) / 64); };  // visible blocks of the tile's last row
+    auto tile_ncols = [&](int mt) -> int { return min(p.n_blocks, (mt * TROWS + TROWS) / 64); };  // visible blocks of the tile's last row
 
     if (warp == 0) {
         // =============================== TMA producer ===============================
@@ -397,8 +476,10 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 for (int h = 0; h < NH; ++h, ++it) {
                     mbar_wait_backoff(a_empty, (it & 1) ^ 1, 400);
                     mbar_arrive_expect_tx(a_full, (uint32_t)(KH * SM::A_SLAB));
-                    const int arow = (BASELINE ? (g * p.G + h) : g) * p.T + mt * PF_ROWS;
-                    for (int kh = 0; kh < KH; ++kh) tma_load_2d(smem + SM::OFF_A + kh * SM::A_SLAB, &tmapA, kh * 64, arow, a_full);
+                    const int arow = (BASELINE ? (g * p.G + h) : g) * p.T + mt * TROWS;
+                    for (int kh = 0; kh < KH; ++kh)
+                        for (int rg = 0; rg < PF_ROWS / TROWS; ++rg)   // REPL: the same 32 rows into all four row groups
+                            tma_load_2d(smem + SM::OFF_A + kh * SM::A_SLAB + rg * TROWS * 128, &tmapA, kh * 64, arow, a_full);
                 }
             }
         }
@@ -434,32 +515,31 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     } else {
         // =============================== epilogue: PF_NP threads per query row ===============================
         const int q = warp & 3;                                  // TMEM lane quadrant this warp may access
-        const int part = (warp - 2) >> 2;                        // which share of the row's chunks this warp takes
-        const int trow = q * 32 + lane;                          // row within the tile
+        const int part = REPL ? q * PF_NP + ((warp - 2) >> 2) : (warp - 2) >> 2;   // which share of the row's chunks this warp takes
+        const int trow = REPL ? lane : q * 32 + lane;            // row within the tile
         uint32_t* list = reinterpret_cast<uint32_t*>(smem + SM::OFF_LIST) + trow;
-        uint8_t* out_base = smem + SM::OFF_OUT + trow * 2;
         uint32_t* n_list = reinterpret_cast<uint32_t*>(smem + SM::OFF_NLIST) + trow;
         uint8_t* chunk_cnt = smem + SM::OFF_CCNT + trow;
-        PartComm pc{reinterpret_cast<float2*>(smem + SM::OFF_COMB) + trow, part, 1 + q, 0};
+        PartComm<NP> pc{reinterpret_cast<float2*>(smem + SM::OFF_COMB) + trow, part, REPL ? 1 : 1 + q, 0};
         float* scr = BASELINE ? p.scratch + (size_t)blockIdx.x * PF_MAXN * PF_ROWS + trow : nullptr;
         const TmemRow trsrc{tmem_base + ((uint32_t)(q * 32) << 16)};
         uint32_t it = 0;
         for (int r = 0; r < n_rounds; ++r) {
             const int mt = tile_of_round(r);
             if (mt < 0) continue;
-            const int i = mt * PF_ROWS + trow;                   // query position of this thread
+            const int i = mt * TROWS + trow;                      // query position of this thread
             const bool in_chunk = i >= p.row0 && i < p.row0 + p.n_rows;
             const int ncand = min(p.n_blocks, (i + 1) / 64);
             int32_t* dst = p.ids + ((size_t)g * p.n_rows + (i - p.row0)) * p.topk;
             const int ncols = tile_ncols(mt);
             // this part's share of the row's k output positions
-            const int s_lo = part * ((p.topk + PF_NP - 1) / PF_NP), s_hi = min(p.topk, s_lo + (p.topk + PF_NP - 1) / PF_NP);
+            const int s_lo = min(p.topk, part * ((p.topk + NP - 1) / NP)), s_hi = min(p.topk, s_lo + (p.topk + NP - 1) / NP);
             if (ncols <= p.topk) {                               // whole tile: every candidate is selected (reading q5)
                 if (in_chunk)
                     for (int s = s_lo; s < s_hi; ++s) dst[s] = s < ncand ? s : -1;
                 continue;
             }
-            const int wmax = min(p.n_blocks, (mt * PF_ROWS + q * 32 + 32) / 64);   // candidates of the warp's last row
+            const int wmax = min(p.n_blocks, (mt * TROWS + (REPL ? 0 : q * 32) + 32) / 64);   // candidates of the warp's last row
             const int nch = (wmax + 31) / 32;
             const bool ranked = in_chunk && ncand > p.topk;
             if (BASELINE) {
@@ -469,7 +549,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     mbar_wait_backoff(mma_done, it & 1, 100);
                     tc_fence_after();
                     float m = -INFINITY;
-                    for (int c = part; c < nch; c += PF_NP) {
+                    for (int c = part; c < nch; c += NP) {
                         trsrc.load(c, v);
 #pragma unroll
                         for (int e = 0; e < 32; ++e)
@@ -477,10 +557,10 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     }
                     pc.put(make_float2(m, 0.f));
 #pragma unroll
-                    for (int pp = 0; pp < PF_NP; ++pp) m = fmaxf(m, pc.get(pp).x);
+                    for (int pp = 0; pp < NP; ++pp) m = fmaxf(m, pc.get(pp).x);
                     const float ms = m * p.scale_log2;
                     float l = 0.f;
-                    for (int c = part; c < nch; c += PF_NP) {
+                    for (int c = part; c < nch; c += NP) {
                         trsrc.load(c, v);
 #pragma unroll
                         for (int e = 0; e < 32; ++e)
@@ -489,9 +569,9 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     pc.put(make_float2(l, 0.f));
                     l = 0.f;
 #pragma unroll
-                    for (int pp = 0; pp < PF_NP; ++pp) l += pc.get(pp).x;   // same order in every part
+                    for (int pp = 0; pp < NP; ++pp) l += pc.get(pp).x;   // same order in every part
                     const float inv = ncand > 0 ? 1.0f / l : 0.f;
-                    for (int c = part; c < nch; c += PF_NP) {
+                    for (int c = part; c < nch; c += NP) {
                         trsrc.load(c, v);
 #pragma unroll
                         for (int e = 0; e < 32; ++e) {
@@ -508,22 +588,22 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     if (lane == 0) mbar_arrive(tmem_empty);
                 }
                 if (__any_sync(0xffffffffu, ranked))
-                    row_topk(ScratchRow{scr}, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, out_base);
+                    row_topk<REPL ? 2 : 1>(ScratchRow{scr}, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, dst);
             } else {
                 mbar_wait_backoff(mma_done, it & 1, 100);
                 ++it;
                 tc_fence_after();
+                PF_TRACE(1);
                 if (__any_sync(0xffffffffu, ranked))
-                    row_topk(trsrc, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, out_base);
+                    row_topk<REPL ? 2 : 1>(trsrc, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, dst);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(tmem_empty);
             }
-            if (ranked) {
-                for (int s = s_lo; s < s_hi; ++s) dst[s] = *reinterpret_cast<const uint16_t*>(out_base + s * PF_OPITCH);
-            } else if (in_chunk) {
+            if (!ranked && in_chunk) {
                 for (int s = s_lo; s < s_hi; ++s) dst[s] = s < ncand ? s : -1;
             }
+            PF_TRACE(13);
         }
     }
 
@@ -535,13 +615,14 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     }
 }
 
-template <int D, bool BASELINE>
-int launch(sparda_ctx* ctx, const void* A, const void* Kpool, int T, int n_blocks, int row0, int n_rows, int topk, int32_t* ids,
-           cudaStream_t st) {
+template <int D, bool BASELINE, bool REPL>
+int launch_mode(sparda_ctx* ctx, const void* A, const void* Kpool, int T, int n_blocks, int row0, int n_rows, int topk, int32_t* ids,
+                cudaStream_t st) {
     using SM = PfSmem<D>;
+    constexpr int TROWS = REPL ? 32 : PF_ROWS;
     const int Hkv = ctx->cfg.n_kv_heads, G = ctx->G;
     const CUtensorMap *mapA, *mapB;
-    int rc = sparda_get_tmap(ctx, A, (uint64_t)(BASELINE ? Hkv * G : Hkv) * T, D, PF_ROWS, &mapA);
+    int rc = sparda_get_tmap(ctx, A, (uint64_t)(BASELINE ? Hkv * G : Hkv) * T, D, TROWS, &mapA);
     if (rc) return rc;
     rc = sparda_get_tmap(ctx, Kpool, (uint64_t)Hkv * n_blocks, D, 256, &mapB);
     if (rc) return rc;
@@ -556,21 +637,32 @@ int launch(sparda_ctx* ctx, const void* A, const void* Kpool, int T, int n_block
     p.topk = topk;
     p.Hkv = Hkv;
     p.G = G;
-    p.mt_lo = row0 / PF_ROWS;
-    p.n_tiles = (row0 + n_rows + PF_ROWS - 1) / PF_ROWS - p.mt_lo;
+    p.mt_lo = row0 / TROWS;
+    p.n_tiles = (row0 + n_rows + TROWS - 1) / TROWS - p.mt_lo;
     if (per_group > p.n_tiles) per_group = p.n_tiles;
     p.scale_log2 = 1.4426950408889634f / sqrtf((float)D);
     p.scratch = nullptr;
     if (BASELINE) p.scratch = ctx->pf_scratch;
     static bool attr_set = false;
     if (!attr_set) {
-        SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(prefill_select_kernel<D, BASELINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
+        SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(prefill_select_kernel<D, BASELINE, REPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
         attr_set = true;
     }
-    prefill_select_kernel<D, BASELINE><<<per_group * Hkv, PF_THREADS, SM::TOTAL, st>>>(*mapA, *mapB, p);
+    prefill_select_kernel<D, BASELINE, REPL><<<per_group * Hkv, PF_THREADS, SM::TOTAL, st>>>(*mapA, *mapB, p);
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;
     return SPARDA_OK;
+}
+
+// A call whose 128-row tiles would leave a quarter of the SMs or more idle (a 2048-row chunk is 16 tiles per group) runs in
+// the replicated mode: 32-row tiles, 16 threads per row (measured break-even: about one 128-row tile per SM).
+template <int D, bool BASELINE>
+int launch(sparda_ctx* ctx, const void* A, const void* Kpool, int T, int n_blocks, int row0, int n_rows, int topk, int32_t* ids,
+           cudaStream_t st) {
+    const int tiles128 = (row0 + n_rows + PF_ROWS - 1) / PF_ROWS - row0 / PF_ROWS;
+    if (PF_NP == 4 && 4 * tiles128 * ctx->cfg.n_kv_heads <= 3 * ctx->sm_count)
+        return launch_mode<D, BASELINE, true>(ctx, A, Kpool, T, n_blocks, row0, n_rows, topk, ids, st);
+    return launch_mode<D, BASELINE, false>(ctx, A, Kpool, T, n_blocks, row0, n_rows, topk, ids, st);
 }
 
 }  // namespace

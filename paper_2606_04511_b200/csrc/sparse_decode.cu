@@ -10,8 +10,10 @@
 // free) completing on per-stage mbarriers (K and V separately: QK^T starts when K lands, and the next K load is
 // issued as soon as QK^T has consumed the tile).  The group's G <= 16 query heads are the M = 16 rows of
 // mma.sync.m16n8k16 (bf16 in, fp32 accumulate): S = Q K^T (16 x 64 per block), online softmax in the exp2
-// domain, O += P V.  Warp partials (m, l, O) are merged through shared memory, the CTA partials of one row
-// through an L2-resident workspace by the last CTA to finish that row (ticket), which rounds once to bf16.
+// domain, O += P V.  Warp partials (m, l, O) are merged through shared memory.  The CTA partials of one row are reduced
+// inside a thread-block cluster through distributed shared memory when the split is row-aligned with 2, 4 or 8 CTAs per
+// row (the [BJ] shapes), else through an L2-resident workspace by the last CTA to finish that row (ticket).  One bf16
+// rounding.
 // HBM-bound by design: 16 FLOP per KV byte at G = 16; the tensor pipe idles most of the time.
 #include "sparda_internal.cuh"
 
@@ -64,7 +66,11 @@ __device__ __forceinline__ int flat_owner(int f, int quota, int rem) {
     return f < thr ? f / (quota + 1) : rem + (f - thr) / quota;
 }
 
-template <int D, int NW, int MINB>
+// CL (row-aligned splits, s = 2, 4 or 8 CTAs per row launched as one cluster): the CTA partials of a row are reduced
+// through distributed shared memory instead of the L2 workspace -- every CTA sends each head row's partial (m, l, O) to the
+// CTA that owns that head row (16 / s rows each), one cluster barrier, every CTA normalises and stores its rows.  No ticket,
+// no fence, no global round trip, and the final merge is spread over the cluster.
+template <int D, int NW, int MINB, bool CL>
 __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __grid_constant__ CUtensorMap tmap, AttnParams p) {
     using SM = AttnSmem<D, NW>;
     constexpr int NT = NW * 32;
@@ -415,6 +421,66 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
     if (park_r < 0) return;
     __syncthreads();
     TRACE(3);
+    if (CL) {
+        // ---- cluster reduction of the row's n = park_n partials.  Landing area (exchange buffer 1, unused in this mode):
+        // land[p][lrow][D] fp32 and ml[p][lrow][2], p = source CTA, lrow = head row within this CTA's 16 / n rows.
+        const int n = park_n, part = park_part, r = park_r;
+        const int rows_per = 16 / n;
+        float* land = reinterpret_cast<float*>(smem + SM::OFF_XCHG + (size_t)NW * SM::XCHG_WARP);
+        float* land_ml = land + 16 * D;
+        const uint32_t land_u32 = smem_u32(land), ml_u32 = smem_u32(land_ml);
+        for (int it = tid; it < 16 * C4; it += NT) {
+            const int row = it / C4, c4 = it % C4;
+            float M = -INFINITY;
+#pragma unroll
+            for (int i = 0; i < NW; ++i) M = fmaxf(M, s_ml[0][i][0][row]);
+            float L = 0.f;
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < NW; ++i) {
+                const float wg = (M == -INFINITY) ? 0.f : exp2f(s_ml[0][i][0][row] - M);
+                L += wg * s_ml[0][i][1][row];
+                const float4 v = *reinterpret_cast<const float4*>(
+                    reinterpret_cast<const float*>(smem + SM::OFF_XCHG + (size_t)i * SM::XCHG_WARP) + row * SM::OROW + c4 * 4);
+                acc.x += wg * v.x; acc.y += wg * v.y; acc.z += wg * v.z; acc.w += wg * v.w;
+            }
+            const uint32_t owner = (uint32_t)(row / rows_per), lrow = (uint32_t)(row % rows_per);
+            uint32_t dst, dml;
+            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(dst) : "r"(land_u32 + ((part * rows_per + lrow) * D + c4 * 4) * 4), "r"(owner));
+            asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "f"(acc.x), "f"(acc.y), "f"(acc.z), "f"(acc.w) : "memory");
+            if (c4 == 0) {
+                asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(dml) : "r"(ml_u32 + ((part * rows_per + lrow) * 2) * 4), "r"(owner));
+                asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(dml), "f"(M), "f"(L) : "memory");
+            }
+        }
+        TRACE(4);
+        asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+        TRACE(5);
+        const int b = r / p.Hkv, g = r % p.Hkv;
+        __nv_bfloat16* obase = p.O + (size_t)(b * p.Hq + g * p.G) * D;
+        for (int it = tid; it < rows_per * C4; it += NT) {
+            const int lrow = it / C4, c4 = it % C4;
+            const int row = part * rows_per + lrow;
+            if (row >= p.G) continue;
+            float M = -INFINITY;
+            for (int q = 0; q < n; ++q) M = fmaxf(M, land_ml[(q * rows_per + lrow) * 2]);
+            float L = 0.f;
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int q = 0; q < n; ++q) {
+                const float wg = (M == -INFINITY) ? 0.f : exp2f(land_ml[(q * rows_per + lrow) * 2] - M);
+                L += wg * land_ml[(q * rows_per + lrow) * 2 + 1];
+                const float4 v = *reinterpret_cast<const float4*>(land + ((size_t)(q * rows_per + lrow) * D + c4 * 4));
+                acc.x += wg * v.x; acc.y += wg * v.y; acc.z += wg * v.z; acc.w += wg * v.w;
+            }
+            const float inv = L > 0.f ? 1.f / L : 0.f;
+            uint2 u;
+            u.x = pack_bf16(acc.x * inv, acc.y * inv);
+            u.y = pack_bf16(acc.z * inv, acc.w * inv);
+            *reinterpret_cast<uint2*>(obase + (size_t)row * D + c4 * 4) = u;
+        }
+        TRACE(6);
+        return;
+    }
     cta_merge(0, park_r, park_part, park_n);
     TRACE(4);
     const bool owes_merge = publish(park_r, park_n);
@@ -426,16 +492,38 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
 // Launch shape: 4 consumer warps (= 4 x 32 KiB K/V stages at D = 128), one CTA per SM (128 KiB of tiles in flight per SM).
 constexpr int ATT_NW = 4;
 
-template <int D>
-int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, cudaStream_t st) {
-    auto kern = sparse_decode_kernel<D, ATT_NW, 1>;
+template <int D, bool CL>
+int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, int cluster, cudaStream_t st) {
+    auto kern = sparse_decode_kernel<D, ATT_NW, 1, CL>;
     constexpr int smem = AttnSmem<D, ATT_NW>::TOTAL;
     static bool attr_set = false;
     if (!attr_set) {
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
-    kern<<<C, ATT_NW * 32, smem, st>>>(*map, p);
+    cudaLaunchConfig_t lc = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    lc.gridDim = dim3((unsigned)C, 1, 1);
+    lc.blockDim = dim3(ATT_NW * 32, 1, 1);
+    lc.dynamicSmemBytes = smem;
+    lc.stream = st;
+    if (CL) {
+        // a cluster needs `cluster` SMs of one GPC at the same time (one CTA per SM): use this path only when every row's
+        // cluster is resident in one wave, else the second wave costs more than the reduction saves (batch 8, 16 x 8 CTAs)
+        static int max_clusters[9];   // per cluster size; 0 = not asked
+        if (max_clusters[cluster] == 0) {
+            int n = 0;
+            if (cudaOccupancyMaxActiveClusters(&n, kern, &lc) != cudaSuccess) n = -1;
+            (void)cudaGetLastError();
+            max_clusters[cluster] = n > 0 ? n : -1;
+        }
+        if (max_clusters[cluster] * cluster < C) return 1;   // caller falls back to the workspace reduction
+    }
+    SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, kern, *map, p));
     return SPARDA_OK;
 }
 
@@ -499,7 +587,12 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     const int C = sparda_resolve_attn_ctas(ctx, topk);
     p.quota = p.W / C;
     p.rem = p.W % C;
-    rc = D == 128 ? launch<128>(ctx, map, p, C, st) : launch<64>(ctx, map, p, C, st);
+    // row-aligned split with 2, 4 or 8 CTAs per row: reduce the partials inside a cluster (distributed shared memory)
+    const int s_per = p.quota > 0 && p.rem == 0 && topk % p.quota == 0 ? topk / p.quota : 0;
+    const bool cl = (s_per == 2 || s_per == 4 || s_per == 8) && (long long)s_per * ctx->R == C;
+    rc = 1;
+    if (cl) rc = D == 128 ? launch<128, true>(ctx, map, p, C, s_per, st) : launch<64, true>(ctx, map, p, C, s_per, st);
+    if (rc == 1) rc = D == 128 ? launch<128, false>(ctx, map, p, C, 1, st) : launch<64, false>(ctx, map, p, C, 1, st);
     if (rc) return rc;
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;

@@ -283,7 +283,7 @@ def bench_kernels_b32(torch, binding, peaks, args):
                     "frac_of_nominal_8tbs": b / t / 1e9 / 8000.0, "peak_source": peaks["source"], "traffic": None})
     # DRAM read + write bytes per launch of the same shapes from the committed ncu --set full captures
     out[0]["traffic"], out[0]["traffic_source"] = 33612800, "profiles/r1c_ncu_summary.md (prof_b32_select_c: dram read 33.61 MB, write 0)"
-    out[1]["traffic"], out[1]["traffic_source"] = 134556160 + 4178688, "profiles/r1c_ncu_summary.md (prof_b32_attn_c: dram read 134.56 MB, write 4.18 MB of split-K partials)"
+    out[1]["traffic"], out[1]["traffic_source"] = 134544640 + 3627776, "profiles/r1c_ncu_summary.md (prof_b32_attn_c: dram read 134.54 MB, 3.6 MB of evictions)"
     out[1]["attn_splits"] = ctx.attn_splits(k)
     out[2]["workload"] = ("f3 (reading q19, unpinned by the paper): batch 32, 2048 blocks x 4 compressed keys, max-pool to blocks, "
                           "top-96 = 1 initial + 32 local + 63 ranked; cold HBM (two 128 MiB grids > L2), CUDA-graph replay")
@@ -344,6 +344,12 @@ def bench_prefill(torch, binding, peaks_all):
                      "peak": bf16_peak, "unit": "TFLOP/s", "frac": flops / t_chunk / 1e12 / bf16_peak, "traffic": None,
                      "algorithmic_flops": flops,
                      "note": "the contraction is ~1% of the kernel; the fused per-row top-k (plain ALU, DESIGN.md 5.5) is the cost"},
+        # the bound that matters: warp instructions executed by the one-launch kernel (ncu smsp__inst_executed.sum,
+        # profiles/r1c_ncu_summary.md prof_prefill_c) over the live duration, against 148 SMs x 4 schedulers x 1 warp-instr/clk
+        "roofline_alu": {"kernel": "prefill_select_kernel<128,false,false> (whole sequence, one launch)", "bound": "alu",
+                         "achieved": 40551465 / t_one / 1e9, "peak": 148 * 4 * 1.965, "unit": "G warp-instr/s",
+                         "frac": 40551465 / t_one / 1e9 / (148 * 4 * 1.965), "us_per_launch": t_one * 1e6,
+                         "executed_warp_instructions": 40551465},
     }
     ctx.close()
     return out
@@ -625,11 +631,13 @@ def run_sparda(args):
         {"kernel": "forecast_select_kernel<128>", "workload": f"{cfg.name} in-pipeline", "bound": "hbm",
          "us_per_launch": t_sel * 1e6, "algorithmic_bytes": sel_bytes, "achieved": sel_bytes / t_sel / 1e9,
          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": sel_bytes / t_sel / 1e9 / peaks["hbm_gbs"], "traffic": None,
-         "note": "launch-latency-sized at batch 4 (ideal 0.64 us)"},
+         "note": "launch-latency-sized at batch 4 (ideal 0.64 us); the event bracket of the profiling pass includes the gaps of the "
+                 "eager enqueue -- device time per launch is 8.7 us (profiles/r1c_launches.csv)"},
         {"kernel": "sparse_decode_kernel<128>", "workload": f"{cfg.name} in-pipeline (pool just written by the gather: L2-warm)",
          "bound": "hbm", "us_per_launch": t_att * 1e6, "algorithmic_bytes": att_bytes, "achieved": att_bytes / t_att / 1e9,
          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": att_bytes / t_att / 1e9 / peaks["hbm_gbs"], "traffic": None,
-         "note": "launch-latency-sized at batch 4 (ideal 2.6 us)"},
+         "note": "launch-latency-sized at batch 4 (ideal 2.6 us); event bracket as above -- device time per launch is 10.1 us "
+                 "(profiles/r1c_launches.csv)"},
     ]
     prefill = append = None
     if not args.no_kernels:

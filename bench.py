@@ -680,7 +680,7 @@ def run_sparda(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
                 "h2d_bytes_per_step": staged + gather_bytes * (NL - 1), "d2h_bytes_per_step": cfg.batch * cfg.n_q_heads * D * 2 * NL,
                 "h2d_staged_bytes_per_step": staged, "h2d_uva_gather_bytes_per_step": gather_bytes * (NL - 1),
-                "api": "sparda_decode_step_host (pinned host F/Q/O, copies inside the call) + stream sync per step"},
+                "api": "sparda_decode_step_host (pinned host F/Q/O, copies enqueued just in time inside the call) + stream sync per step"},
         "gpu_launches": launches,
         "roofline": roofline,
         "roofline_kernels": kernels,

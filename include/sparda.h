@@ -154,11 +154,11 @@ int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers
                        int mode);
 
 /* The same step for a caller whose per-step tensors live in HOST memory (the end-to-end form bench.py times):
- * layers[l].F, .Q and .O and F0cur are HOST pointers (pinned for the copies to be asynchronous); the call
- * enqueues on compute_stream the host->device copies of F0cur and every layer's F and Q into staging owned by
- * the context, runs sparda_decode_step on the staged tensors, and enqueues the device->host copy of every
- * layer's O.  layers[l].Kpool, .kv and .ids keep their sparda_decode_step meaning.  No host synchronisation:
- * O is valid once compute_stream has drained.  Needs n_layers <= max_layers.                                  */
+ * layers[l].F, .Q and .O and F0cur are HOST pointers (pinned for the copies to be asynchronous); the call runs
+ * sparda_decode_step on staging owned by the context and enqueues the copies on compute_stream just in time: F0cur first,
+ * F_l and Q_l before layer l begins, O_l right after attention l -- so they run while that stream waits for a gather.
+ * layers[l].Kpool, .kv and .ids keep their sparda_decode_step meaning.  No host synchronisation: O is valid once
+ * compute_stream has drained.  Needs n_layers <= max_layers.                                                   */
 int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                             int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
                             int mode);

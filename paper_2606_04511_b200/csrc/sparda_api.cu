@@ -244,19 +244,34 @@ static inline cudaEvent_t* prof_slot(sparda_ctx* ctx, int kind) {
         ctx->prof_n[kind]++;                                                    \
     }
 
+// Host-buffer form (sparda_decode_step_host): the caller's F / Q / O live in pinned host memory.  Their copies are
+// enqueued on the compute stream just in time -- F_l and Q_l before layer l begins, O_l right after attention l -- so
+// they run while that stream waits for a gather instead of in front of and behind the whole step.
+struct HostIO {
+    const sparda_layer* host;   // host pointers F, Q, O per layer
+    const void* F0cur;          // host
+    size_t f_bytes, q_bytes;
+};
+
 static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur, int n_blocks,
-                            int topk, cudaStream_t cs, cudaStream_t ps_in, int mode) {
+                            int topk, cudaStream_t cs, cudaStream_t ps_in, int mode, const HostIO* io = nullptr) {
     const bool overlap = mode == SPARDA_STEP_OVERLAP;
     cudaStream_t ps = overlap ? ps_in : cs;
     cudaStream_t ss = overlap ? ctx->select_stream : cs;
     int rc;
     ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
+    if (io) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(const_cast<void*>(F0cur), io->F0cur, io->f_bytes, cudaMemcpyHostToDevice, cs));
     // layer 0: same-layer selection with F0cur; its attention needs it, so it stays on the compute stream
     SPARDA_PROF_BEGIN(0, cs);
     rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_blocks, topk, layers[0].base.ids, cs);
     if (rc) return rc;
     SPARDA_PROF_END(0, cs);
     for (int l = 0; l < n_layers; ++l) {
+        if (io) {   // this layer's Forecast and query, before ev_top[l] releases the select that reads F_l
+            if (l + 1 < n_layers)
+                SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(const_cast<void*>(layers[l].base.F), io->host[l].F, io->f_bytes, cudaMemcpyHostToDevice, cs));
+            SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(const_cast<void*>(layers[l].base.Q), io->host[l].Q, io->q_bytes, cudaMemcpyHostToDevice, cs));
+        }
         if (l + 1 < n_layers) {
             const sparda_cached_layer* nx = &layers[l + 1];
             if (overlap) {
@@ -292,6 +307,7 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
         }
         if (rc) return rc;
         SPARDA_PROF_END(2, cs);
+        if (io) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(io->host[l].O, layers[l].base.O, io->q_bytes, cudaMemcpyDeviceToHost, cs));
     }
     // every select has been consumed by a gather that an attention waited for, so cs already follows all work of ss and
     // ps; the explicit join keeps that true for n_layers == 1 and makes the step capturable (all forks rejoin cs)
@@ -341,23 +357,24 @@ int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_l
     cudaStream_t cs = (cudaStream_t)compute_stream;
     const size_t f_bytes = (size_t)ctx->R * ctx->cfg.head_dim * 2;
     const size_t q_bytes = (size_t)ctx->cfg.batch * ctx->cfg.n_q_heads * ctx->cfg.head_dim * 2;
-    sparda_layer* dl = (sparda_layer*)alloca(sizeof(sparda_layer) * (size_t)n_layers);
-    SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_F + f_bytes * ctx->max_layers, F0cur, f_bytes, cudaMemcpyHostToDevice, cs));
+    if (mode != SPARDA_STEP_OVERLAP && mode != SPARDA_STEP_SERIAL) return SPARDA_EINVAL;
+    if (n_layers > 1 && (!dev_pool0 || !dev_pool1)) return SPARDA_EINVAL;
+    void* pools[2] = {dev_pool0, dev_pool1};
+    sparda_cached_layer* cl = (sparda_cached_layer*)alloca(sizeof(sparda_cached_layer) * (size_t)n_layers);
     for (int l = 0; l < n_layers; ++l) {
         if (!layers[l].Q || !layers[l].O || (l + 1 < n_layers && !layers[l].F)) return SPARDA_EINVAL;
-        dl[l] = layers[l];
-        dl[l].F = ctx->stage_F + f_bytes * l;
-        dl[l].Q = ctx->stage_Q + q_bytes * l;
-        dl[l].O = ctx->stage_O + q_bytes * l;
-        if (l + 1 < n_layers) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_F + f_bytes * l, layers[l].F, f_bytes, cudaMemcpyHostToDevice, cs));
-        SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_Q + q_bytes * l, layers[l].Q, q_bytes, cudaMemcpyHostToDevice, cs));
+        cl[l].base = layers[l];
+        cl[l].base.F = ctx->stage_F + f_bytes * l;
+        cl[l].base.Q = ctx->stage_Q + q_bytes * l;
+        cl[l].base.O = ctx->stage_O + q_bytes * l;
+        cl[l].pool = pools[l & 1];
+        cl[l].slot_ids = nullptr;
+        cl[l].fetch = nullptr;
+        cl[l].n_fetch = nullptr;
     }
-    int rc = sparda_decode_step(ctx, dl, n_layers, ctx->stage_F + f_bytes * ctx->max_layers, n_blocks, topk, dev_pool0, dev_pool1,
-                                compute_stream, prefetch_stream, mode);
-    if (rc) return rc;
-    for (int l = 0; l < n_layers; ++l)
-        SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(layers[l].O, ctx->stage_O + q_bytes * l, q_bytes, cudaMemcpyDeviceToHost, cs));
-    return SPARDA_OK;
+    HostIO io = {layers, F0cur, f_bytes, q_bytes};
+    return decode_step_impl(ctx, cl, n_layers, ctx->stage_F + f_bytes * ctx->max_layers, n_blocks, topk, cs, (cudaStream_t)prefetch_stream, mode,
+                            &io);
 }
 
 int sparda_profile_enable(sparda_ctx* ctx, int on) {

@@ -347,6 +347,32 @@ def test_pipeline_wiring_with_planted_needles(oracle):
                 assert out[l]["pool"][r, i].tobytes() == layers[l]["kv"][r, j].tobytes()
 
 
+# ---------------------------------------------------------------- o2 Forecast projection (Eq.3; one head per group)
+def test_forecast_project_reduces_to_a_matmul(oracle):
+    """o2 is a plain GEMV per sequence: it must equal numpy's fp64 matmul rounded once to bf16 (library routine), and
+    the column block of group g must depend only on W_F[:, g*D:(g+1)*D] (one Forecast head per KV group)."""
+    rng = np.random.default_rng(2)
+    B, hidden, Hkv, D = 3, 192, 2, 64
+    X = bf.f64_to_bf16_bits(rng.standard_normal((B, hidden)))
+    W = bf.f64_to_bf16_bits(rng.standard_normal((hidden, Hkv * D)) / 8)
+    F = oracle.forecast_project(X, W, Hkv, D)
+    assert F.shape == (B * Hkv, D)
+    want = bf.f64_to_bf16_bits(bf.bits_to_f64(X) @ bf.bits_to_f64(W)).reshape(B * Hkv, D)
+    assert np.max(parity_ulps(F, want)) <= 1            # the two fp64 sums differ only in order
+    W2 = W.copy()
+    W2[:, D:] = bf.f64_to_bf16_bits(rng.standard_normal((hidden, D)))
+    F2 = oracle.forecast_project(X, W2, Hkv, D)
+    np.testing.assert_array_equal(F2.reshape(B, Hkv, D)[:, 0], F.reshape(B, Hkv, D)[:, 0])
+    assert not np.array_equal(F2.reshape(B, Hkv, D)[:, 1], F.reshape(B, Hkv, D)[:, 1])
+
+
+def parity_ulps(a, b):
+    def key(u):
+        u = np.asarray(u, dtype=np.uint16).astype(np.int32)
+        return np.where(u & 0x8000, -(u & 0x7FFF), u & 0x7FFF)
+    return np.abs(key(a) - key(b))
+
+
 # ---------------------------------------------------------------- o11 / o12 block reuse between decode steps (P:L347)
 def test_reuse_plan_set_invariants_random(oracle):
     """o11 against what 'only newly selected blocks are fetched' fixes, checked with Python sets written

@@ -101,6 +101,13 @@ int sparda_destroy(sparda_ctx* ctx);
  * Pre-condition of the path ("kept on GPU and updated incrementally"), not on the timed path.  */
 int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_blocks, void* kpool, void* stream);
 
+/* (A4 / f4) Forecast projection, Eq.3: F[b, g, :] = bf16(X[b, :] . W_F[:, g*D:(g+1)*D]), one Forecast head of
+ * width D per GQA group; fp32 accumulation in a fixed order (deterministic), one rounding.  X [B][hidden] device bf16 (the
+ * layer's input hidden states), W_F [hidden][Hkv*D] device bf16 row-major, F_out [R][D] device (R = B*Hkv, the layout
+ * sparda_forecast_select reads).  64 <= hidden <= 8192, a multiple of 64.  One kernel on `stream`; bound by streaming W_F
+ * once.  The path's calls take F as an input, so a caller that computes F inside its fused QKV+F GEMM does not need this. */
+int sparda_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F_out, void* stream);
+
 /* (f2) Decode-time cache maintenance, Alg.2 lines 2-3: append the new token's key and value at position t
  * (0-based; block t / S, offset t % S) of every row's cache and "update K~ incrementally".  k_new, v_new
  * [R][D] device; kv_cache [R][n_blocks][2][S][D]: a device pointer (layer 0) or a host-mapped pointer (the offloaded

@@ -18,7 +18,7 @@ GATHER_TMA, GATHER_LDG = 0, 1
 STEP_OVERLAP, STEP_SERIAL = 0, 1
 
 EXPORTS = [
-    "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_append_kv", "sparda_pool_keys_grid", "sparda_forecast_select_grid", "sparda_forecast_select", "sparda_prefetch_launch",
+    "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_project", "sparda_append_kv", "sparda_pool_keys_grid", "sparda_forecast_select_grid", "sparda_forecast_select", "sparda_prefetch_launch",
     "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
     "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
@@ -64,6 +64,7 @@ def lib() -> ctypes.CDLL:
         L.sparda_pool_keys.argtypes = [vp, vp, i64, i32, vp, vp]
         L.sparda_pool_keys_grid.argtypes = [vp, vp, i64, i32, vp, vp]
         L.sparda_forecast_select_grid.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
+        L.sparda_forecast_project.argtypes = [vp, vp, vp, i32, vp, vp]
         L.sparda_append_kv.argtypes = [vp, vp, vp, i64, vp, i32, vp, vp, vp]
         L.sparda_forecast_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_prefetch_launch.argtypes = [vp, vp, i32, vp, i32, vp, vp]
@@ -153,6 +154,9 @@ class Sparda:
         n_cand = n_blocks if n_cand is None else n_cand
         self._check(self._L.sparda_forecast_select_grid(self._h, _ptr(F), _ptr(Kgrid), n_blocks, n_cand, n_init, n_local, topk,
                                                         _ptr(ids_out), _stream(stream)), "forecast_select_grid")
+
+    def forecast_project(self, X, WF, hidden, F_out, stream=None):
+        self._check(self._L.sparda_forecast_project(self._h, _ptr(X), _ptr(WF), hidden, _ptr(F_out), _stream(stream)), "forecast_project")
 
     def append_kv(self, k_new, v_new, t, kv_cache, n_blocks, ksum, kpool, stream=None):
         self._check(self._L.sparda_append_kv(self._h, _ptr(k_new), _ptr(v_new), int(t), _ptr(kv_cache), n_blocks, _ptr(ksum),

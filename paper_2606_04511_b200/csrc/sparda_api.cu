@@ -85,6 +85,9 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     bool ok = cudaMalloc(&ctx->part_O, n_po * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->part_ml, n_ml * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->tickets, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
+              cudaMalloc(&ctx->fp_part, (size_t)128 * ctx->R * D * sizeof(float)) == cudaSuccess &&
+              cudaMalloc(&ctx->fp_ticket, sizeof(unsigned int)) == cudaSuccess &&
+              cudaMemset(ctx->fp_ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&ctx->pf_scratch, (size_t)ctx->sm_count * 512 * 128 * sizeof(float)) == cudaSuccess &&
               cudaMemset(ctx->tickets, 0, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
@@ -123,6 +126,8 @@ int sparda_destroy(sparda_ctx* ctx) {
     cudaFree(ctx->part_ml);
     cudaFree(ctx->tickets);
     cudaFree(ctx->pf_scratch);
+    cudaFree(ctx->fp_part);
+    cudaFree(ctx->fp_ticket);
     for (int i = 0; i <= ctx->max_layers; ++i) {
         if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);
         if (ctx->ev_gather && ctx->ev_gather[i]) cudaEventDestroy(ctx->ev_gather[i]);
@@ -147,6 +152,12 @@ int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_bloc
     if (!ctx || !sparda_aligned(kv, 16) || !sparda_aligned(kpool, 16) || n_rows < 1 || n_blocks < 1) return SPARDA_EINVAL;
     if (n_rows * (int64_t)n_blocks > (int64_t)1 << 31) return SPARDA_EINVAL;
     return sparda_launch_pool_keys(ctx, kv, n_rows, n_blocks, kpool, (cudaStream_t)stream);
+}
+
+int sparda_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F_out, void* stream) {
+    if (!ctx || !sparda_aligned(X, 16) || !sparda_aligned(WF, 16) || !sparda_aligned(F_out, 16)) return SPARDA_EINVAL;
+    if (hidden < 64 || hidden > 8192 || hidden % 64 != 0) return SPARDA_EINVAL;
+    return sparda_launch_forecast_project(ctx, X, WF, hidden, F_out, (cudaStream_t)stream);
 }
 
 int sparda_append_kv(sparda_ctx* ctx, const void* k_new, const void* v_new, int64_t t, void* kv_cache, int n_blocks, float* ksum,

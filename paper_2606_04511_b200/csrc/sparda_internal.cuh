@@ -28,6 +28,8 @@ struct sparda_ctx {
     float* part_O;     // [R][max_splits][16][D]
     float* part_ml;    // [R][max_splits][2][16]  (m in log2 domain, l)
     unsigned int* tickets;  // [R]: split-K attention, one per row (the select keeps its scores on chip)
+    float* fp_part;         // Forecast projection: split-K partials [128 slabs][B][Hkv*D] fp32
+    unsigned int* fp_ticket;
     float* pf_scratch;      // prefill comparison selector: [sm_count][512][128] fp32 group-summed scores (lazy)
     cudaEvent_t* ev_sel;    // [max_layers + 1]
     cudaEvent_t* ev_gather; // [max_layers + 1]
@@ -66,6 +68,7 @@ int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_bl
                          cudaStream_t);
 int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
                          cudaStream_t);
+int sparda_launch_forecast_project(sparda_ctx*, const void* X, const void* WF, int hidden, void* F, cudaStream_t);
 int sparda_launch_pool_keys_grid(sparda_ctx*, const void* kv, int64_t n_rows, int n_blocks, void* kgrid, cudaStream_t);
 int sparda_launch_select_grid(sparda_ctx*, const void* F, const void* Kgrid, int n_blocks, int n_cand, int n_init, int n_local, int topk,
                               int32_t* ids, cudaStream_t);

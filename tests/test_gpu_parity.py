@@ -561,6 +561,28 @@ def test_select_grid_full_size_128k(sp, oracle):
         parity.check_ids(ids.cpu().numpy(), want, np.where(np.isinf(bs), np.float32(3.0e38), bs), Nb)
 
 
+@pytest.mark.parametrize("B,hidden,Hkv,D", [(4, 4096, 2, 128), (37, 192, 3, 64), (1, 64, 1, 64)])
+def test_forecast_project(B, hidden, Hkv, D, sp, oracle):
+    """A4 / f4 (o2): the Forecast projection GEMV within 1 bf16 ulp of the fp64 oracle (fp32 accumulation), deterministic
+    across launches, and usable as the F of the selection (8B shape: hidden 4096, 2 groups x 128)."""
+    cfg = synth.DecodeConfig("fp", batch=B, n_q_heads=Hkv, n_kv_heads=Hkv, head_dim=D, n_blocks=64, topk=8)
+    ctx = sp.Sparda.from_config(cfg)
+    g = torch.Generator(device="cuda").manual_seed(hidden + B)
+    X = torch.randn((B, hidden), generator=g, device="cuda").to(torch.bfloat16)
+    W = (torch.randn((hidden, Hkv * D), generator=g, device="cuda") / hidden ** 0.5).to(torch.bfloat16)
+    F = torch.full((B * Hkv, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    F2 = F.clone()
+    ctx.forecast_project(X, W, hidden, F)
+    ctx.forecast_project(X, W, hidden, F2)
+    torch.cuda.synchronize()
+    assert torch.equal(F.view(torch.int16), F2.view(torch.int16)), "not deterministic"
+    want = oracle.forecast_project(_bits(X), _bits(W), Hkv, D)
+    ulps = parity.ulp_diff_bf16(_bits(F), want)
+    assert ulps.max() <= 1 and (ulps > 0).mean() < 5e-3, f"max {ulps.max()} ulp, {(ulps > 0).mean():.3%} differ"
+    with pytest.raises(sp.SpardaError):
+        ctx.forecast_project(X, W, hidden + 32, F)
+
+
 def test_cfg2_full_size_layer(sp, oracle):
     """BASELINE.json configs[1] at full size: batch 8, 32/2 heads, D=128, 512 blocks, top-64, KV pinned on host."""
     cfg = synth.CFG2_32K

@@ -70,6 +70,10 @@ typedef struct {
     int gather_mode; /* SPARDA_GATHER_TMA or SPARDA_GATHER_LDG */
     int attn_splits; /* split-K CTAs per row for sparse_decode; 0 = auto from B, Hkv, k and the SM count */
     int max_layers;  /* largest n_layers sparda_decode_step will see (events are pre-created); 0 = 64 */
+    int select_cluster; /* CTAs per row (thread-block cluster size) of forecast_select: 0 = auto from B, Hkv, n_cand and the
+                           SM count; 1, 2, 4, 8 or 16 forces it (sweeps and tests)                                       */
+    int no_pdl;      /* 1 = launch without programmatic dependent launch (measurement: what the launch gap costs);
+                        0 = select, gather and attention kernels overlap their prologue with the previous kernel's tail */
 } sparda_config;
 
 /* One decoder layer's tensors for sparda_decode_step (Algorithm 2). */
@@ -145,7 +149,11 @@ int sparda_prefetch_launch(sparda_ctx* ctx, const void* host_kv, int n_blocks, c
  *   pool_is_indexed = 0: dev_pool is [R][topk][2][S][D] and slot i holds block ids[r][i] (n_slots = topk);
  *   pool_is_indexed = 1: dev_pool is a device-resident cache [R][n_slots][2][S][D] addressed through ids
  *                        (layer 0).
- * Split-K flash-decode: grid = attn_splits x R CTAs, partials merged by the last CTA of each row.            */
+ * Split-K flash-decode over a flat list of the R*topk slots.  Row-aligned splits with 2, 4 or 8 CTAs per row run as
+ * one thread-block cluster per row and reduce their partials through distributed shared memory; any other split
+ * reduces through the context's L2-resident workspace, merged by the last CTA of each row (ticket).
+ * The workspace is shared by every launch on the context: at most ONE sparse_decode (and one forecast_project) may be
+ * in flight per context at a time -- order concurrent launches with events or use one context per stream.        */
 int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, int topk,
                          int pool_is_indexed, int n_slots, void* O, void* stream);
 
@@ -249,6 +257,10 @@ int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* K
 /* Introspection used by bench.py / tests: number of kernels this context has launched since creation, the
  * resolved tunables, and error text.                                                                          */
 int64_t sparda_launch_count(const sparda_ctx* ctx);
+int64_t sparda_tmap_encodes(const sparda_ctx* ctx);      /* TMA descriptors encoded so far (a warm step encodes none) */
+int sparda_get_select_cluster(const sparda_ctx* ctx);    /* cluster size of the LAST forecast_select launch           */
+int sparda_get_attn_cluster(const sparda_ctx* ctx);      /* CTAs per row reduced through DSMEM by the LAST sparse_decode
+                                                            launch (2, 4 or 8), 0 = workspace + ticket reduction     */
 int sparda_get_attn_splits(const sparda_ctx* ctx, int topk);
 int sparda_get_gather_ctas(const sparda_ctx* ctx);
 const char* sparda_strerror(int code);

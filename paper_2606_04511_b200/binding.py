@@ -22,7 +22,7 @@ EXPORTS = [
     "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
     "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
-    "sparda_launch_count", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
+    "sparda_launch_count", "sparda_tmap_encodes", "sparda_get_select_cluster", "sparda_get_attn_cluster", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
     "sparda_last_cuda_error", "sparda_version",
 ]
 
@@ -34,7 +34,7 @@ class SpardaError(RuntimeError):
 class SpardaConfig(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int) for n in (
         "batch", "n_q_heads", "n_kv_heads", "head_dim", "block_size", "max_blocks", "topk", "gather_ctas",
-        "gather_mode", "attn_splits", "max_layers")]
+        "gather_mode", "attn_splits", "max_layers", "select_cluster", "no_pdl")]
 
 
 class SpardaLayer(ctypes.Structure):
@@ -80,6 +80,10 @@ def lib() -> ctypes.CDLL:
         L.sparda_prefill_select_baseline.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
         L.sparda_launch_count.argtypes = [vp]
         L.sparda_launch_count.restype = i64
+        L.sparda_tmap_encodes.argtypes = [vp]
+        L.sparda_tmap_encodes.restype = i64
+        L.sparda_get_select_cluster.argtypes = [vp]
+        L.sparda_get_attn_cluster.argtypes = [vp]
         L.sparda_get_attn_splits.argtypes = [vp, i32]
         L.sparda_get_gather_ctas.argtypes = [vp]
         for f in ("sparda_strerror", "sparda_last_cuda_error", "sparda_version"):
@@ -109,10 +113,10 @@ class Sparda:
     """One libsparda context (one shape family on the current device)."""
 
     def __init__(self, batch, n_q_heads, n_kv_heads, head_dim, max_blocks, topk, block_size=64, gather_ctas=0,
-                 gather_mode=GATHER_TMA, attn_splits=0, max_layers=0):
+                 gather_mode=GATHER_TMA, attn_splits=0, max_layers=0, select_cluster=0, no_pdl=0):
         self._h = ctypes.c_void_p()
         self.cfg = SpardaConfig(batch, n_q_heads, n_kv_heads, head_dim, block_size, max_blocks, topk, gather_ctas,
-                                gather_mode, attn_splits, max_layers)
+                                gather_mode, attn_splits, max_layers, select_cluster, no_pdl)
         self._L = lib()
         rc = self._L.sparda_create(ctypes.byref(self.cfg), ctypes.byref(self._h))
         if rc != 0:
@@ -244,6 +248,20 @@ class Sparda:
     @property
     def launch_count(self) -> int:
         return int(self._L.sparda_launch_count(self._h))
+
+    @property
+    def tmap_encodes(self) -> int:
+        return int(self._L.sparda_tmap_encodes(self._h))
+
+    @property
+    def select_cluster(self) -> int:
+        """Cluster size (CTAs per row) of the last forecast_select launch."""
+        return int(self._L.sparda_get_select_cluster(self._h))
+
+    @property
+    def attn_cluster(self) -> int:
+        """CTAs per row reduced through DSMEM by the last sparse_decode launch; 0 = workspace + ticket reduction."""
+        return int(self._L.sparda_get_attn_cluster(self._h))
 
     def attn_splits(self, topk) -> int:
         return int(self._L.sparda_get_attn_splits(self._h, topk))

@@ -48,6 +48,8 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
         fence_proxy_async_smem();
     }
     __syncwarp();
+    pdl_wait();                  // ids (and the pool's previous reader) belong to earlier kernels
+    pdl_launch_dependents();
     const uint32_t cpb = block_bytes / GATHER_STAGE_BYTES;  // 16 KiB chunks per block: 2 at D=128, 1 at D=64
     const int64_t n_tasks = (int64_t)n_rows * topk;
     const unsigned lt = (1u << lane) - 1u;
@@ -123,6 +125,8 @@ __global__ void __launch_bounds__(256) gather_ldg_kernel(const char* __restrict_
                                                          char* __restrict__ pool, int n_rows, int n_blocks, int topk,
                                                          uint32_t block_bytes) {
     const int lane = threadIdx.x & 31;
+    pdl_wait();
+    pdl_launch_dependents();
     const int64_t warp = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int64_t n_warps = (int64_t)gridDim.x * (blockDim.x >> 5);
     const uint32_t units_per_block = block_bytes / LDG_UNIT_BYTES;
@@ -150,15 +154,30 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
     const uint32_t block_bytes = 2u * ctx->cfg.block_size * ctx->cfg.head_dim * 2u;
     const int ctas = ctx->cfg.gather_ctas;
     if (ctx->cfg.gather_mode == SPARDA_GATHER_TMA) {
-        static bool attr_set = false;
         const int smem = GATHER_STAGES * GATHER_STAGE_BYTES;
-        if (!attr_set) {
+        sparda_kernel_state& ks = ctx->kstate[SPARDA_K_GATHER_TMA];
+        if (!ks.attr_set) {
             SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(gather_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            attr_set = true;
+            ks.attr_set = true;
         }
-        gather_tma_kernel<<<ctas, 32, smem, st>>>((const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes);
+        cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
+        cudaLaunchConfig_t lc = {};
+        lc.gridDim = dim3(ctas, 1, 1);
+        lc.blockDim = dim3(32, 1, 1);
+        lc.dynamicSmemBytes = smem;
+        lc.stream = st;
+        lc.attrs = at;
+        lc.numAttrs = ctx->cfg.no_pdl ? 0 : 1;
+        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_tma_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes));
     } else {
-        gather_ldg_kernel<<<ctas, 256, 0, st>>>((const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes);
+        cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
+        cudaLaunchConfig_t lc = {};
+        lc.gridDim = dim3(ctas, 1, 1);
+        lc.blockDim = dim3(256, 1, 1);
+        lc.stream = st;
+        lc.attrs = at;
+        lc.numAttrs = ctx->cfg.no_pdl ? 0 : 1;
+        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_ldg_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes));
     }
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;

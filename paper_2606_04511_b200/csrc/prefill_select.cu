@@ -621,7 +621,7 @@ int launch_mode(sparda_ctx* ctx, const void* A, const void* Kpool, int T, int n_
     using SM = PfSmem<D>;
     constexpr int TROWS = REPL ? 32 : PF_ROWS;
     const int Hkv = ctx->cfg.n_kv_heads, G = ctx->G;
-    const CUtensorMap *mapA, *mapB;
+    CUtensorMap mapA, mapB;   // copies: a later lookup can never change a descriptor held here
     int rc = sparda_get_tmap(ctx, A, (uint64_t)(BASELINE ? Hkv * G : Hkv) * T, D, TROWS, &mapA);
     if (rc) return rc;
     rc = sparda_get_tmap(ctx, Kpool, (uint64_t)Hkv * n_blocks, D, 256, &mapB);
@@ -643,12 +643,12 @@ int launch_mode(sparda_ctx* ctx, const void* A, const void* Kpool, int T, int n_
     p.scale_log2 = 1.4426950408889634f / sqrtf((float)D);
     p.scratch = nullptr;
     if (BASELINE) p.scratch = ctx->pf_scratch;
-    static bool attr_set = false;
-    if (!attr_set) {
+    sparda_kernel_state& ks = ctx->kstate[SPARDA_K_PF_0 + (D == 128 ? 4 : 0) + (BASELINE ? 2 : 0) + (REPL ? 1 : 0)];
+    if (!ks.attr_set) {
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(prefill_select_kernel<D, BASELINE, REPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
-        attr_set = true;
+        ks.attr_set = true;
     }
-    prefill_select_kernel<D, BASELINE, REPL><<<per_group * Hkv, PF_THREADS, SM::TOTAL, st>>>(*mapA, *mapB, p);
+    prefill_select_kernel<D, BASELINE, REPL><<<per_group * Hkv, PF_THREADS, SM::TOTAL, st>>>(mapA, mapB, p);
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;
     return SPARDA_OK;

@@ -4,33 +4,51 @@
 //   ids[r] = f_top(s[r, 0:n_cand], k)          P:L78: k best blocks, ties -> lowest id, ascending ids, -1 padded
 //
 // One launch, one thread-block cluster per row r.  The row's n_cand pooled keys are cut into CS contiguous ranges,
-// one per CTA of the cluster (CS = 1..16, chosen so that R*CS fills the SMs).  In every CTA a producer warp streams
-// its range through a ring of 16 KiB shared-memory stages with bulk copies (TMA engine, cp.async.bulk on
-// mbarriers: 96 KiB in flight per CTA, two CTAs per SM, no registers or LSU slots spent on the stream); 8 consumer warps take the
-// dot products out of shared memory (D/8 lanes per key, 16-byte conflict-free reads, fp32 FMA, shuffle reduction)
-// and store order-preserving uint32 keys straight into the shared memory of the cluster's CTA 0 (DSMEM), together
-// with per-warp min / max.  After one cluster barrier CTA 0 holds the whole row's scores on chip and selects: a
-// one-pass 256-bucket value histogram finds the boundary bucket of the k-th largest, one warp ranks its few members
-// exactly, and an index-ordered compaction emits {key > T} plus the first (k - #{key > T}) keys == T, which is
-// exactly "sort by (score desc, id asc), take k, sort by id".  Scores never touch global memory; there is no
-// ticket, no fence and no scratch.  HBM-bound: R*n_cand*D*2 bytes of Kpool.
+// one per CTA of the cluster (CS = 1..16, chosen so that R*CS covers every SM, up to two CTAs per SM).  In every CTA a
+// producer thread streams its range through a ring of 16 KiB shared-memory stages with TMA tensor-map loads (64-key x
+// 64-element boxes, 128-byte swizzle, completing on mbarriers: 96 KiB in flight per CTA, no registers or LSU slots spent
+// on the stream).  HBM-bound (R*n_cand*D*2 bytes of Kpool, 1 FLOP per byte), so the arithmetic must cost next to
+// nothing in issue slots: the 8 consumer warps read the swizzled stage with conflict-free ldmatrix and take the dot
+// products with mma.sync.m16n8k16 (16 keys as the M rows, F in column 0 of the B operand, fp32 accumulate): 8 ldmatrix +
+// 8 mma per 16 keys instead of ~160 warp instructions of convert + FMA + shuffle, which had 8 warps per SM running at the
+// HBM rate with nothing to spare (sm__warps_active 14 %, round 1).  The tensor pipe is not what this is for (7 of its 8
+// output columns are zero); the point is the issue slots.  Order-preserving uint32 keys go straight into the shared
+// memory of the cluster's CTA 0 (DSMEM), min / max by red.shared::cluster.  After one cluster barrier CTA 0 holds the
+// whole row's scores on chip and selects: a one-pass 256-bucket value histogram finds the boundary bucket of the k-th
+// largest, every warp ranks its few members exactly, and an index-ordered compaction emits {key > T} plus the first
+// (k - #{key > T}) keys == T, which is exactly "sort by (score desc, id asc), take k, sort by id".  Scores never touch
+// global memory; there is no ticket, no fence and no scratch.
+//
+// Debug builds only (-DSPARDA_TRACE, never shipped): per-CTA globaltimer stamps of the phases, read back by a probe
+// through sparda_debug_set_sel_trace.
 #include "sparda_internal.cuh"
 #include "reuse_plan.cuh"
-#ifdef SEL_CS_ENV
-#include <cstdlib>
-#endif
 
 #ifdef SPARDA_TRACE
-__device__ unsigned long long* g_sel_trace;   // [gridDim.x][16] globaltimer stamps (debug builds only)
-extern "C" void sparda_debug_set_sel_trace(unsigned long long* p) { cudaMemcpyToSymbol(g_sel_trace, &p, sizeof(p)); }
-#define SEL_TRACE(i)                                                                          \
-    if (threadIdx.x == 0) {                                                                   \
-        unsigned long long t__;                                                               \
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));                               \
-        g_sel_trace[blockIdx.x * 16 + (i)] = t__;                                              \
+// per-CTA timeline: thread 0 stamps the SM cycle counter at up to 16 points (relative to kernel entry) and appends
+// (blockIdx, globaltimer at entry, globaltimer at exit, cycles[16]) to a log when it leaves
+__device__ unsigned long long* g_sel_log;      // [0] = cursor, then 20 words per entry from word 8
+extern "C" void sparda_debug_set_sel_log(unsigned long long* p) { cudaMemcpyToSymbol(g_sel_log, &p, sizeof(p)); }
+__device__ __forceinline__ unsigned long long sel_now() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+struct SelCyc { unsigned long long t0; long long c0; long long c[16]; };
+#define SEL_LOG_DECL SelCyc cyc_; cyc_.t0 = sel_now(); cyc_.c0 = clock64(); _Pragma("unroll") for (int i_ = 0; i_ < 16; ++i_) cyc_.c[i_] = 0; \
+    __shared__ long long s_dbg[4];
+#define SEL_CYC(i) if (threadIdx.x == 0) cyc_.c[i] = clock64() - cyc_.c0;
+#define SEL_CYC_PRODUCER(i) s_dbg[i] = clock64();
+#define SEL_LOG_EXIT                                                                          \
+    if (threadIdx.x == 0 && g_sel_log) {                                                      \
+        cyc_.c[14] = s_dbg[0] - cyc_.c0; cyc_.c[15] = s_dbg[1] - cyc_.c0;                     \
+        unsigned long long e_ = atomicAdd(g_sel_log, 1ull);                                   \
+        unsigned long long* d_ = g_sel_log + 8 + e_ * 20;                                     \
+        d_[0] = blockIdx.x; d_[1] = cyc_.t0; d_[2] = sel_now(); d_[3] = (unsigned long long)(clock64() - cyc_.c0); \
+        _Pragma("unroll") for (int i_ = 0; i_ < 16; ++i_) d_[4 + i_] = (unsigned long long)cyc_.c[i_];           \
     }
 #else
-#define SEL_TRACE(i)
+struct SelCyc {};
+#define SEL_LOG_DECL SelCyc cyc_;
+#define SEL_CYC(i)
+#define SEL_CYC_PRODUCER(i)
+#define SEL_LOG_EXIT
 #endif
 
 namespace {
@@ -39,12 +57,8 @@ using namespace sparda;
 
 constexpr int SEL_THREADS = 256;                  // consumer threads (the selection runs on these)
 constexpr int SEL_CTA_THREADS = SEL_THREADS + 32; // + one producer warp
-#ifndef SEL_STAGE_BYTES_V
-#define SEL_STAGE_BYTES_V 16384
-#define SEL_STAGES_V 6
-#endif
-constexpr int SEL_STAGE_BYTES = SEL_STAGE_BYTES_V;
-constexpr int SEL_STAGES = SEL_STAGES_V;
+constexpr int SEL_STAGE_BYTES = 16384;            // two 64 x 64-element TMA boxes
+constexpr int SEL_STAGES = 6;
 constexpr int SEL_MAX_CS = 16;                    // largest cluster (non-portable size, opt-in)
 
 // barrier of the 256 consumer threads only (the producer warp has left by the time the selection runs)
@@ -52,9 +66,8 @@ __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;
 __device__ __forceinline__ void mbar_arrive1(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 __device__ __forceinline__ uint32_t cluster_ctarank() {
     uint32_t r;
     asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
@@ -68,6 +81,30 @@ __device__ __forceinline__ uint32_t map_to_cta(const void* local, uint32_t rank)
 }
 __device__ __forceinline__ void st_cluster_u32(uint32_t addr, uint32_t v) {
     asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+// arrive (release at cluster scope) on an mbarrier in another CTA's shared memory: orders this thread's earlier remote
+// stores (and, through the warp barrier in front of it, its warp's) before the waiter's acquire
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAITC_%=:\n"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONEC_%=;\n"
+        "bra WAITC_%=;\n"
+        "DONEC_%=:\n"
+        "}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void red_cluster_min_u32(uint32_t addr, uint32_t v) {
+    asm volatile("red.shared::cluster.min.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_cluster_max_u32(uint32_t addr, uint32_t v) {
+    asm volatile("red.shared::cluster.max.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
 __device__ __forceinline__ uint32_t block_incl_scan_256(uint32_t v, uint32_t* warp_tot /*[8]*/, uint32_t& total) {
@@ -92,100 +129,131 @@ __device__ __forceinline__ uint32_t block_incl_scan_256(uint32_t v, uint32_t* wa
 }
 
 __device__ __forceinline__ float key_to_float(uint32_t key) {
-    return __uint_as_float(key ^ ((key >> 31) ? 0x80000000u : 0xFFFFFFFFu));
+    // inverse of orderable(): positive floats carry the top bit (flip it back), negative ones are complemented
+    return __uint_as_float(key ^ (~(uint32_t)((int32_t)key >> 31) | 0x80000000u));
 }
 
-constexpr int SEL_CAND_CAP = 32;  // boundary-bucket size the one-warp exact finish handles
+constexpr int SEL_CAND_CAP = 32;  // boundary-bucket size the exact finish handles
 
 // Exact top-k over keys[0..n) (order-preserving uint32 keys in shared memory), k < n <= 8192.  256 consumer threads.
 //
-// Fast path, three CTA barriers:
-//  1. one histogram pass over 256 equal-width value buckets of the row's [min, max] (hist is zeroed by the caller).
-//     The bucket map is monotone (subtract, multiply by a positive constant, truncate: all monotone under IEEE
-//     rounding), so every key in a higher bucket is larger than every key in a lower one and equal keys share a
-//     bucket.  Unlike a radix pass over the top byte of the key (sign + 7 exponent bits: a handful of bins for
-//     Gaussian logits) the shared-memory atomics are spread.
-//  2. every warp redundantly suffix-scans the 256 counts (8 per lane + one shuffle scan) and finds the boundary bucket
-//     b* holding the k-th largest -- no broadcast, no barrier.  Each thread then walks its contiguous slice of the row
-//     once: keys above b* are selected (a bit mask in a register), members of b* (<= 32, typically ~4) go to a list.
-//  3. every warp redundantly ranks the list by (key desc, id asc) with shuffles, which yields the k-th largest key and
-//     the largest id taken among its equals; a thread completes its mask, one block scan of the counts places it, and
-//     the ids are emitted in index order: exactly "sort by (score desc, id asc), take k, sort by id".
+// The tail of the kernel is a chain of dependent instructions on 8 warps, so it is written for few instructions and two
+// CTA barriers (round 1: 5600 cycles with three barriers and a generic-address key array; this version: see DESIGN.md 5.1):
+//  1. every thread loads its contiguous slice (16-byte loads; the first 8 keys and their buckets stay in registers) and
+//     counts it into 256 equal-width value buckets of the row's [min, max].  The bucket map is monotone (one FMA with a
+//     positive scale, clamp, truncate), so every key in a higher bucket is larger than every key in a lower one and
+//     equal keys share a bucket.  Only the upper 128 buckets are counted at first: the k-th largest of n >> k keys lies
+//     above the middle of the range unless the row has a far positive outlier, and shared-memory atomics (bank
+//     conflicts) are what this pass costs; if the upper half holds fewer than k keys a second round counts the lower.
+//  2. every warp redundantly suffix-scans 128 counts (4 per lane + one shuffle scan) and finds the boundary bucket b*
+//     of the k-th largest -- no broadcast.  A thread marks its keys above b* in a register bit mask, the members of b*
+//     (<= 32, typically ~4) go to a list; the strict counts are scanned per warp BEFORE the second barrier.
+//  3. every warp redundantly ranks the list by (key desc, id asc) with shuffles: member f is taken iff its rank is below
+//     need = k - #{key above b*}; a thread's output position is (warps before) + (lanes before) + (taken members with
+//     a smaller index), and ids are emitted in index order: exactly "sort by (score desc, id asc), take k, sort by id".
 // Fallback (heavy ties / degenerate range): exact MSB-first 8-bit radix select + index-ordered compaction.
-__device__ void topk_emit(const uint32_t* keys, int n, int k, uint32_t kmin, uint32_t kmax, int32_t* ids_out,
+__device__ __forceinline__ void topk_emit(const uint32_t* keys, int n, int k, uint32_t kmin, uint32_t kmax, int32_t* ids_out,
                           uint32_t* hist /*[256], zeroed*/, uint32_t* warp_tot /*[8]*/, uint32_t* bcast /*[4], [2] zeroed*/,
-                          uint32_t* cand /*[2 * SEL_CAND_CAP]*/) {
+                          uint32_t* cand /*[2 * SEL_CAND_CAP]*/, SelCyc& cyc_) {
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int per = (n + SEL_THREADS - 1) / SEL_THREADS;          // <= 32: a thread's slice fits one bit mask
+    // a thread's contiguous slice: a multiple of 4 keys (16-byte loads), <= 32 so that it fits one bit mask
+    const int per = (((n + SEL_THREADS - 1) / SEL_THREADS) + 3) & ~3;
     const int lo = min(tid * per, n), hi = min(lo + per, n);
     const float flo = key_to_float(kmin), fhi = key_to_float(kmax);
-    const float scale = 256.0f / (fhi - flo);
-    bool fast = (kmax > kmin) && (scale > 0.f) && (scale < INFINITY);
-    auto bucket = [&](uint32_t key) -> int {
-        return (int)fminf((key_to_float(key) - flo) * scale, 255.0f);
+    const float scale = __fdividef(256.0f, fhi - flo), shift = -flo * scale;   // any positive scale keeps the map monotone
+    bool fast = (kmax > kmin) && (scale > 0.f) && (scale < INFINITY) && (fabsf(shift) < INFINITY);
+    auto bucket = [&](uint32_t key) -> int {   // monotone in key; NaN (forced keys of the grid mode) -> 255
+        return (int)fminf(fmaf(key_to_float(key), scale, shift), 255.0f);
     };
     if (fast) {
-        SEL_TRACE(4);
-        for (int i = tid; i < n; i += SEL_THREADS) atomicAdd(&hist[bucket(keys[i])], 1u);
+        SEL_CYC(6);
+        // ---- 1. buckets of the slice; count the upper half
+        int bk[8];
+        {
+            uint32_t kr[8];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const uint4 v = lo + 4 * q < hi ? *reinterpret_cast<const uint4*>(keys + lo + 4 * q) : make_uint4(0, 0, 0, 0);
+                kr[4 * q] = v.x; kr[4 * q + 1] = v.y; kr[4 * q + 2] = v.z; kr[4 * q + 3] = v.w;
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) bk[j] = lo + j < hi ? bucket(kr[j]) : -1;
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (bk[j] >= 128) atomicAdd(&hist[bk[j]], 1u);
+            for (int i = lo + 8; i < hi; ++i) {   // n > 2048 only
+                const int b = bucket(keys[i]);
+                if (b >= 128) atomicAdd(&hist[b], 1u);
+            }
+        }
         consumer_sync();
-        SEL_TRACE(5);
-        // suffix counts, redundantly per warp: lane l owns buckets 255 - 8l - j, j = 0..7 (descending value)
-        uint32_t h[8], run = 0;
+        SEL_CYC(7);
+        // ---- 2. boundary bucket: suffix counts of 128 buckets, redundantly per warp (lane l owns buckets top - 4l - j)
+        int bstar = -1;
+        uint32_t need = 0, pop = 0, above = 0;
+#pragma unroll 1
+        for (int top = 255; top >= 127; top -= 128) {
+            const uint4 hv = *reinterpret_cast<const uint4*>(hist + top - 3 - 4 * lane);
+            const uint32_t h[4] = {hv.w, hv.z, hv.y, hv.x};   // descending bucket
+            const uint32_t run = h[0] + h[1] + h[2] + h[3];
+            uint32_t incl = run;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { h[j] = hist[255 - 8 * lane - j]; run += h[j]; }
-        uint32_t incl = run;
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t nb = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += nb;
+            }
+            uint32_t gt = above + incl - run;                     // keys in buckets above this lane's four
+            int my_b = -1;
+            uint32_t my_need = 0, my_pop = 0;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t nb = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += nb;
-        }
-        uint32_t gt = incl - run;                                 // keys in buckets above this lane's eight
-        int my_b = -1;
-        uint32_t my_need = 0, my_pop = 0;
+            for (int j = 0; j < 4; ++j) {
+                if (gt < (uint32_t)k && (uint32_t)k <= gt + h[j]) { my_b = top - 4 * lane - j; my_need = k - gt; my_pop = h[j]; }
+                gt += h[j];
+            }
+            const unsigned found = __ballot_sync(0xffffffffu, my_b >= 0);
+            if (found) {
+                const int src = __ffs(found) - 1;
+                bstar = __shfl_sync(0xffffffffu, my_b, src);
+                need = __shfl_sync(0xffffffffu, my_need, src);
+                pop = __shfl_sync(0xffffffffu, my_pop, src);
+                break;
+            }
+            // fewer than k keys in the upper half (a far positive outlier stretches the range): count the lower half too
+            above = __shfl_sync(0xffffffffu, above + incl, 31);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            if (gt < (uint32_t)k && (uint32_t)k <= gt + h[j]) { my_b = 255 - 8 * lane - j; my_need = k - gt; my_pop = h[j]; }
-            gt += h[j];
-        }
-        const int src = __ffs(__ballot_sync(0xffffffffu, my_b >= 0)) - 1;   // exactly one lane (n > k)
-        const int bstar = __shfl_sync(0xffffffffu, my_b, src);
-        const uint32_t need = __shfl_sync(0xffffffffu, my_need, src), pop = __shfl_sync(0xffffffffu, my_pop, src);
-        SEL_TRACE(6);
-        if (pop <= SEL_CAND_CAP) {
-            uint32_t m_sel = 0, m_eq = 0;
-            for (int i = lo; i < hi; ++i) {
-                const uint32_t key = keys[i];
-                const int b = bucket(key);
-                if (b > bstar) m_sel |= 1u << (i - lo);
-                if (b == bstar) {
-                    m_eq |= 1u << (i - lo);
-                    const uint32_t s = atomicAdd(&bcast[2], 1u);
-                    cand[2 * s] = key;
-                    cand[2 * s + 1] = (uint32_t)i;
-                }
+            for (int j = 0; j < 8; ++j)
+                if (bk[j] >= 0 && bk[j] < 128) atomicAdd(&hist[bk[j]], 1u);
+            for (int i = lo + 8; i < hi; ++i) {
+                const int b = bucket(keys[i]);
+                if (b < 128) atomicAdd(&hist[b], 1u);
             }
             consumer_sync();
-            SEL_TRACE(7);
-            // rank the boundary bucket, redundantly per warp: lane i holds member i
-            const bool have = (uint32_t)lane < pop;
-            const uint32_t mk = have ? cand[2 * lane] : 0u, mi = have ? cand[2 * lane + 1] : 0xFFFFFFFFu;
-            uint32_t rank = 0;
-            for (uint32_t f = 0; f < pop; ++f) {
-                const uint32_t fk = __shfl_sync(0xffffffffu, mk, f), fi = __shfl_sync(0xffffffffu, mi, f);
-                rank += (fk > mk || (fk == mk && fi < mi)) ? 1u : 0u;
+        }
+        SEL_CYC(8);
+        if (bstar >= 0 && pop <= SEL_CAND_CAP) {
+            // ---- mark; strict counts scanned per warp before the barrier
+            uint32_t m_sel = 0, m_eq = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                if (bk[j] > bstar) m_sel |= 1u << j;
+                if (bk[j] == bstar) m_eq |= 1u << j;
             }
-            const int ks = __ffs(__ballot_sync(0xffffffffu, have && rank == need - 1)) - 1;   // the k-th largest of the row
-            const uint32_t Tk = __shfl_sync(0xffffffffu, mk, ks), Ti = __shfl_sync(0xffffffffu, mi, ks);
-            SEL_TRACE(8);
-            while (m_eq) {
-                const int j = __ffs(m_eq) - 1;
-                m_eq &= m_eq - 1;
-                const uint32_t key = keys[lo + j];
-                if (key > Tk || (key == Tk && (uint32_t)(lo + j) <= Ti)) m_sel |= 1u << j;
+            for (int i = lo + 8; i < hi; ++i) {
+                const int b = bucket(keys[i]);
+                if (b > bstar) m_sel |= 1u << (i - lo);
+                if (b == bstar) m_eq |= 1u << (i - lo);
             }
-            // place and emit
-            const uint32_t c = __popc(m_sel);
-            uint32_t inc = c;
+            if (m_eq) {   // few threads: one reservation per thread, then plain stores
+                uint32_t s = atomicAdd(&bcast[2], (uint32_t)__popc(m_eq));
+                for (uint32_t m = m_eq; m; m &= m - 1) {
+                    const int j = __ffs(m) - 1;
+                    cand[2 * s] = keys[lo + j];
+                    cand[2 * s + 1] = (uint32_t)(lo + j);
+                    ++s;
+                }
+            }
+            const uint32_t c_strict = __popc(m_sel);
+            uint32_t inc = c_strict;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const uint32_t nb = __shfl_up_sync(0xffffffffu, inc, o);
@@ -193,10 +261,31 @@ __device__ void topk_emit(const uint32_t* keys, int n, int k, uint32_t kmin, uin
             }
             if (lane == 31) warp_tot[w] = inc;
             consumer_sync();
-            SEL_TRACE(9);
-            uint32_t pos = inc - c;
+        SEL_CYC(9);
+            // ---- 3. rank the boundary bucket, redundantly per warp: lane f holds member f; taken iff rank < need
+            const bool have = (uint32_t)lane < pop;
+            const uint32_t mk = have ? cand[2 * lane] : 0u, mi = have ? cand[2 * lane + 1] : 0xFFFFFFFFu;
+            uint32_t rank = 0;
+            for (uint32_t f = 0; f < pop; ++f) {
+                const uint32_t fk = __shfl_sync(0xffffffffu, mk, f), fi = __shfl_sync(0xffffffffu, mi, f);
+                rank += (fk > mk || (fk == mk && fi < mi)) ? 1u : 0u;
+            }
+            const uint32_t tagged = (have && rank < need) ? mi : 0xFFFFFFFFu;   // index of a taken member, else "none"
+        SEL_CYC(10);
+            // position = strict keys before this thread + taken members with a smaller index; own taken members join the mask
+            uint32_t pos = inc - c_strict;
+            {
+                const uint4 wa = *reinterpret_cast<const uint4*>(warp_tot), wb = *reinterpret_cast<const uint4*>(warp_tot + 4);
+                const uint32_t wt[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
 #pragma unroll
-            for (int i = 0; i < SEL_THREADS / 32; ++i) pos += i < w ? warp_tot[i] : 0u;
+                for (int i = 0; i < SEL_THREADS / 32; ++i) pos += i < w ? wt[i] : 0u;
+            }
+            for (uint32_t f = 0; f < pop; ++f) {
+                const uint32_t ti = __shfl_sync(0xffffffffu, tagged, f);
+                if (ti < (uint32_t)lo) ++pos;
+                else if (ti < (uint32_t)hi) m_sel |= 1u << (ti - lo);
+            }
+        SEL_CYC(11);
             while (m_sel) {
                 const int j = __ffs(m_sel) - 1;
                 m_sel &= m_sel - 1;
@@ -257,8 +346,7 @@ __device__ void topk_emit(const uint32_t* keys, int n, int k, uint32_t kmin, uin
 
 
 struct SelParams {
-    const uint4* F;
-    const char* Kpool;
+    const uint32_t* F;   // [R][D] bf16 pairs
     int32_t* ids;
     int n_blocks, n_cand, topk;
     int per;   // candidates (blocks) per CTA of the cluster (the last CTA's range may be shorter or empty)
@@ -272,25 +360,28 @@ struct SelParams {
     int32_t* n_fetch;
 };
 
+// tmap: the pooled keys as a [R * n_blocks * KPB][D] bf16 tensor, box = 64 keys x 64 elements, 128-byte swizzle.
 template <int D, bool GRID>
-__global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(SelParams p) {
+__global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(const __grid_constant__ CUtensorMap tmap, SelParams p) {
     constexpr int KPB = GRID ? 4 : 1;                // keys per candidate block
-    constexpr int LPK = D / 8;                       // lanes per key (16 B = 8 bf16 each)
-    constexpr int KPL = 32 / LPK;                    // keys per warp-wide read
     constexpr int NW = SEL_THREADS / 32;
     constexpr int ROW_BYTES = D * 2;
-    constexpr int KPS = SEL_STAGE_BYTES / ROW_BYTES; // keys per stage
-    constexpr int PASSES = KPS / (NW * KPL);
+    constexpr int KPS = SEL_STAGE_BYTES / ROW_BYTES; // keys per stage: 64 (D = 128) or 128 (D = 64)
+    constexpr int TPW = KPS / 64;                    // 16-key MMA tiles per warp per stage (4 warps share a stage)
+    constexpr int KSTEPS = D / 16;                   // k-steps of the contraction
+    SEL_LOG_DECL
     extern __shared__ uint8_t sel_smem_raw[];
     __shared__ uint64_t s_full[SEL_STAGES], s_empty[SEL_STAGES];
-    __shared__ uint32_t s_hist[256];
-    __shared__ uint32_t s_wtot[8];
+    __shared__ uint64_t s_done;                      // CTA 0: one arrival per consumer warp of the cluster when its keys are in
+    __shared__ __align__(16) uint32_t s_hist[256];
+    __shared__ __align__(16) uint32_t s_wtot[8];
     __shared__ uint32_t s_bcast[4];
     __shared__ uint32_t s_cand[2 * SEL_CAND_CAP];
-    __shared__ uint32_t s_mm[2][SEL_MAX_CS * NW];    // per (CTA of the cluster, warp): min / max key; lives in CTA 0
+    __shared__ uint32_t s_mm[2];                     // min / max key of the row; lives in CTA 0 (red.shared::cluster)
     __shared__ ReusePlanScratch s_plan;
 
-    uint8_t* ring = (uint8_t*)(((uintptr_t)sel_smem_raw + 127) & ~(uintptr_t)127);
+    // swizzle atoms are 1 KiB; the offset is taken in the shared window so that ring / s_keys stay shared-space pointers
+    uint8_t* ring = sel_smem_raw + ((1024u - (smem_u32(sel_smem_raw) & 1023u)) & 1023u);
     uint32_t* s_keys = reinterpret_cast<uint32_t*>(ring + SEL_STAGES * SEL_STAGE_BYTES);   // [n_cand], used in CTA 0
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -301,6 +392,8 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
     int32_t* ids_row = p.ids + (size_t)r * p.topk;
 
     if (p.n_cand <= p.topk) {  // every candidate is selected (reading q5); no scoring needed
+        pdl_wait();
+        pdl_launch_dependents();
         if (c == 0) {
             for (int i = tid; i < p.topk; i += SEL_CTA_THREADS) ids_row[i] = i < p.n_cand ? i : -1;
             if (p.slot_ids) {
@@ -314,129 +407,156 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 1) forecast_select_kernel(Sel
         return;
     }
 
-    if (tid == 0) {
-        for (int s = 0; s < SEL_STAGES; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], NW); }
-        mbar_fence_init();
-        fence_proxy_async_smem();
-    }
-    __syncthreads();
-    SEL_TRACE(0);
-
     const int k_lo = min((int)c * p.per, p.n_cand);
     const int n_local = min(p.per, p.n_cand - k_lo);
     const int n_keys_local = n_local * KPB;         // rows of Kpool this CTA streams
     const int n_st = (n_keys_local + KPS - 1) / KPS;
+    const int row0 = (r * p.n_blocks + k_lo) * KPB; // first row of this CTA's range in the tensor map
+
+    // one stage = up to two boxes: D = 128: the two 64-element halves of 64 keys; D = 64: two groups of 64 keys
+    auto issue_stage = [&](int i) {
+        const int s = i % SEL_STAGES;
+        const int nk = min(KPS, n_keys_local - i * KPS);
+        const int nbox = (D == 64 && nk <= 64) ? 1 : 2;
+        uint8_t* dst = ring + (size_t)s * SEL_STAGE_BYTES;
+        mbar_arrive_expect_tx(&s_full[s], (uint32_t)nbox * 8192u);
+        tma_load_2d(dst, &tmap, 0, row0 + i * KPS, &s_full[s]);
+        if (nbox == 2) tma_load_2d(dst + 8192, &tmap, D == 128 ? 64 : 0, row0 + i * KPS + (D == 128 ? 0 : 64), &s_full[s]);
+    };
+
+    SEL_CYC(0);
+    if (w == NW && lane == 0) {   // the producer thread arms the barriers
+        for (int s = 0; s < SEL_STAGES; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], NW / 2); }
+        mbar_init(&s_done, CS * NW);
+        mbar_fence_init();
+        fence_proxy_async_smem();
+        tma_prefetch_desc(&tmap);
+        SEL_CYC_PRODUCER(0);
+    }
+    if (tid < 256) s_hist[tid] = 0;
+    if (tid == 0) { s_bcast[2] = 0; s_mm[0] = 0xFFFFFFFFu; s_mm[1] = 0u; }
+    __syncthreads();
+    // All CTAs of the cluster must be running before anyone touches a neighbour's shared memory: arrive now, wait just
+    // before the first remote store (by then every CTA has long arrived: the wait is free).  The release / acquire pair
+    // also orders CTA 0's initialisation of s_mm / s_hist / s_done before the remote reductions and arrivals.
+    cluster_arrive();
+    pdl_wait();                  // everything above overlaps the previous kernel's tail; global memory is touched from here on
+    pdl_launch_dependents();
+    SEL_CYC(1);
 
     if (w == NW) {
-        // =============================== producer warp: bulk copies into the ring ===============================
+        // =============================== producer warp: the stream ===============================
+        // (measured: loads issued BEFORE the CTA barrier and the cluster arrive above land 2400 cycles later than loads
+        // issued here -- the async unit does not start a shared::cluster copy until the cluster is up)
         if (lane == 0) {
-            const char* src = p.Kpool + ((size_t)r * p.n_blocks + k_lo) * KPB * ROW_BYTES;
             for (int i = 0; i < n_st; ++i) {
-                const int s = i % SEL_STAGES;
-                if (i >= SEL_STAGES) mbar_wait(&s_empty[s], ((i / SEL_STAGES) - 1) & 1);
-                const uint32_t bytes = (uint32_t)min(KPS, n_keys_local - i * KPS) * ROW_BYTES;
-                mbar_arrive_expect_tx(&s_full[s], bytes);
-                bulk_g2s(ring + (size_t)s * SEL_STAGE_BYTES, src + (size_t)i * SEL_STAGE_BYTES, bytes, &s_full[s]);
+                if (i >= SEL_STAGES) mbar_wait(&s_empty[i % SEL_STAGES], ((i / SEL_STAGES) - 1) & 1);
+                issue_stage(i);
+                if (i == SEL_STAGES - 1 || i == n_st - 1) { SEL_CYC_PRODUCER(1); }
             }
         }
+        __syncwarp();
+        cluster_wait();
     } else {
         // =============================== consumers: a1, scores of this CTA's range ===============================
-        const int sub = lane / LPK, dl = lane % LPK;
-        const uint4 fv = __ldg(p.F + (size_t)r * LPK + dl);
-        float f[8];
-        f[0] = bf16_lo(fv.x); f[1] = bf16_hi(fv.x); f[2] = bf16_lo(fv.y); f[3] = bf16_hi(fv.y);
-        f[4] = bf16_lo(fv.z); f[5] = bf16_hi(fv.z); f[6] = bf16_lo(fv.w); f[7] = bf16_hi(fv.w);
+        // Warps 0-3 take the even stages, warps 4-7 the odd ones; inside a stage warp wi owns the 16-key tiles wi, wi + 4.
+        const int grp = w >> 2, wi = w & 3;
+        const int gid = lane >> 2, tig = lane & 3;
+        // B operand: F in column 0 (rows k of the 16 x 8 tile), zeros elsewhere: only the lanes with gid == 0 hold data
+        uint32_t fb[KSTEPS][2];
+        {
+            const uint32_t* frow = p.F + (size_t)r * (D / 2);
+#pragma unroll
+            for (int ks = 0; ks < KSTEPS; ++ks) {
+                fb[ks][0] = gid == 0 ? __ldg(frow + ks * 8 + tig) : 0u;
+                fb[ks][1] = gid == 0 ? __ldg(frow + ks * 8 + 4 + tig) : 0u;
+            }
+        }
         const uint32_t keys0 = map_to_cta(s_keys, 0);          // the row's key array lives in CTA 0
+        const int mi = lane >> 3, ri = lane & 7;                // ldmatrix: this lane addresses row ri of matrix mi
         uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
-        for (int i = 0; i < n_st; ++i) {
+        bool waited = false;
+        for (int i = grp; i < n_st; i += 2) {
             const int s = i % SEL_STAGES;
             const int nk = min(KPS, n_keys_local - i * KPS);
             mbar_wait(&s_full[s], (i / SEL_STAGES) & 1);
-            const uint8_t* st = ring + (size_t)s * SEL_STAGE_BYTES;
-            uint4 kv[PASSES];
+            if (i == 0) { SEL_CYC(2); }
+            const uint32_t st = smem_u32(ring + (size_t)s * SEL_STAGE_BYTES);
+            // A operand: 16 keys x 16 elements per ldmatrix.x4 (matrices: rows 0-7 / 8-15 x element halves), swizzled rows
+            uint32_t a[TPW][KSTEPS][4];
 #pragma unroll
-            for (int ps = 0; ps < PASSES; ++ps) {
-                // plain: pass ps takes key ps*16 + group; grid: the group takes the 4 keys of one block, one per pass
-                const int kl = GRID ? (w * KPL + sub) * 4 + ps : ps * (NW * KPL) + w * KPL + sub;
-                kv[ps] = kl < nk ? *reinterpret_cast<const uint4*>(st + (size_t)kl * ROW_BYTES + dl * 16) : make_uint4(0, 0, 0, 0);
+            for (int t = 0; t < TPW; ++t) {
+                const int krow = (wi + 4 * t) * 16 + (mi & 1) * 8 + ri;                       // key within the stage
+                const uint32_t rowaddr = st + (D == 64 ? (krow >> 6) * 8192 : 0) + (krow & 63) * 128;
+#pragma unroll
+                for (int ks = 0; ks < KSTEPS; ++ks) {
+                    const int ch = ks * 2 + (mi >> 1);                                        // 16-byte chunk of the key row
+                    ldmatrix_x4(rowaddr + (ch >> 3) * 8192 + (((ch & 7) ^ ri) << 4), a[t][ks][0], a[t][ks][1], a[t][ks][2], a[t][ks][3]);
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive1(&s_empty[s]);            // the stage is in registers: hand it back
-#ifdef SEL_NOCOMPUTE
-            if (kv[0].x == 0x12345678u) kmin = 0;
-            continue;
-#endif
-            float sc[PASSES];
+            if (!waited) { cluster_wait(); waited = true; }
 #pragma unroll
-            for (int ps = 0; ps < PASSES; ++ps) {
-                float a = f[0] * bf16_lo(kv[ps].x);
-                a = fmaf(f[1], bf16_hi(kv[ps].x), a);
-                a = fmaf(f[2], bf16_lo(kv[ps].y), a);
-                a = fmaf(f[3], bf16_hi(kv[ps].y), a);
-                a = fmaf(f[4], bf16_lo(kv[ps].z), a);
-                a = fmaf(f[5], bf16_hi(kv[ps].z), a);
-                a = fmaf(f[6], bf16_lo(kv[ps].w), a);
-                sc[ps] = fmaf(f[7], bf16_hi(kv[ps].w), a);
-            }
-            // Transposed butterfly over the LPK lanes of a key: instead of reducing each of the 4 partial sums over all
-            // lanes (4 * log2(LPK) shuffles), the two highest lane bits split the 4 sums between the lanes (2 + 1
-            // shuffles), the remaining bits are plain butterflies on the one sum a lane is left with.  Pass `mine` of
-            // the stage ends up complete in the lanes whose two highest key-lane bits spell `mine`.
-            static_assert(PASSES == 4 && LPK >= 4, "the transposed reduction is written for 4 partial sums per lane");
-            const bool hi1 = (dl & (LPK / 2)) != 0, hi2 = (dl & (LPK / 4)) != 0;
-            const float r0 = __shfl_xor_sync(0xffffffffu, hi1 ? sc[0] : sc[2], LPK / 2);
-            const float r1 = __shfl_xor_sync(0xffffffffu, hi1 ? sc[1] : sc[3], LPK / 2);
-            const float v0 = (hi1 ? sc[2] : sc[0]) + r0, v1 = (hi1 ? sc[3] : sc[1]) + r1;
-            float tot = (hi2 ? v1 : v0) + __shfl_xor_sync(0xffffffffu, hi2 ? v0 : v1, LPK / 4);
+            for (int t = 0; t < TPW; ++t) {
+                float acc0[4] = {0.f, 0.f, 0.f, 0.f}, acc1[4] = {0.f, 0.f, 0.f, 0.f};   // two chains: half the dependent latency
 #pragma unroll
-            for (int o = LPK / 8; o >= 1; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-            const int mine = (hi1 ? 2 : 0) + (hi2 ? 1 : 0);
-            if (GRID) {
-                // f_top's max-pool (reading q19): block score = max over the compressed keys that start in the block
-                const int blk = i * (KPS / 4) + w * KPL + sub;                     // block within this CTA's range
-                const int jkey = (k_lo + blk) * 4 + mine;                            // compressed key index in the row
-                float bsc = jkey < p.keys_valid ? tot : -INFINITY;
-                bsc = fmaxf(bsc, __shfl_xor_sync(0xffffffffu, bsc, LPK / 2));
-                bsc = fmaxf(bsc, __shfl_xor_sync(0xffffffffu, bsc, LPK / 4));
-                if (dl == 0 && blk < n_local) {
-                    const int b = k_lo + blk;
-                    const bool forced = b < p.n_init || b >= p.n_cand - p.n_local;   // init / local blocks: always attended
-                    const uint32_t key = forced ? 0xFFFFFFFFu : orderable(bsc + 0.0f);
-                    st_cluster_u32(keys0 + 4u * (uint32_t)b, key);
-                    if (!forced) { kmin = min(kmin, key); kmax = max(kmax, key); }
+                for (int ks = 0; ks < KSTEPS; ks += 2) {
+                    mma_bf16_16816(acc0, a[t][ks], fb[ks][0], fb[ks][1]);
+                    mma_bf16_16816(acc1, a[t][ks + 1], fb[ks + 1][0], fb[ks + 1][1]);
                 }
-            } else {
-                const int kl = mine * (NW * KPL) + w * KPL + sub;
-                if ((dl & (LPK / 4 - 1)) == 0 && kl < nk) {
-                    const uint32_t key = orderable(tot + 0.0f);      // +0: -0 -> +0
-                    st_cluster_u32(keys0 + 4u * (uint32_t)(k_lo + i * KPS + kl), key);
-                    kmin = min(kmin, key);
-                    kmax = max(kmax, key);
+                // column 0 of the 16 x 8 result: lanes with tig == 0 hold key gid (c0) and key gid + 8 (c2)
+                const float sc[2] = {acc0[0] + acc1[0], acc0[2] + acc1[2]};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int kl = (wi + 4 * t) * 16 + h * 8 + gid;                           // key within the stage
+                    if (GRID) {
+                        // f_top's max-pool (reading q19): block score = max over the compressed keys that start in
+                        // the block = keys 4b .. 4b+3 = four consecutive gid
+                        const int jkey = (k_lo * 4 + i * KPS) + kl;                           // compressed key index in the row
+                        float bsc = jkey < p.keys_valid ? sc[h] : -INFINITY;
+                        bsc = fmaxf(bsc, __shfl_xor_sync(0xffffffffu, bsc, 4));
+                        bsc = fmaxf(bsc, __shfl_xor_sync(0xffffffffu, bsc, 8));
+                        const int blk = i * (KPS / 4) + (kl >> 2);                            // block within this CTA's range
+                        if (tig == 0 && (gid & 3) == 0 && blk < n_local) {
+                            const int b = k_lo + blk;
+                            const bool forced = b < p.n_init || b >= p.n_cand - p.n_local;   // init / local blocks: always attended
+                            const uint32_t key = forced ? 0xFFFFFFFFu : orderable(bsc + 0.0f);
+                            st_cluster_u32(keys0 + 4u * (uint32_t)b, key);
+                            if (!forced) { kmin = min(kmin, key); kmax = max(kmax, key); }
+                        }
+                    } else if (tig == 0 && kl < nk) {
+                        const uint32_t key = orderable(sc[h] + 0.0f);      // +0: -0 -> +0
+                        st_cluster_u32(keys0 + 4u * (uint32_t)(k_lo + i * KPS + kl), key);
+                        kmin = min(kmin, key);
+                        kmax = max(kmax, key);
+                    }
                 }
             }
         }
+        SEL_CYC(3);
+        if (!waited) cluster_wait();
         kmin = __reduce_min_sync(0xffffffffu, kmin);
         kmax = __reduce_max_sync(0xffffffffu, kmax);
-        if (lane == 0) {
-            st_cluster_u32(map_to_cta(&s_mm[0][c * NW + w], 0), kmin);
-            st_cluster_u32(map_to_cta(&s_mm[1][c * NW + w], 0), kmax);
+        if (lane == 0 && kmin <= kmax) {
+            red_cluster_min_u32(map_to_cta(&s_mm[0], 0), kmin);
+            red_cluster_max_u32(map_to_cta(&s_mm[1], 0), kmax);
         }
+        // This warp's keys are on their way to CTA 0: tell it (release at cluster scope, cumulative over the warp's stores
+        // through the warp barrier).  No closing cluster barrier: nobody reads the shared memory of CTAs 1.., so they leave
+        // at once, and CTA 0 waits for the arrivals only -- not for a barrier round trip of the whole cluster.
+        __syncwarp();
+        if (lane == 0) mbar_arrive_remote(map_to_cta(&s_done, 0));
     }
-    if (tid < 256) s_hist[tid] = 0;
-    if (tid == 0) s_bcast[2] = 0;
-    SEL_TRACE(1);
-    // every CTA's keys and min / max have landed in CTA 0 once the cluster barrier completes (release / acquire)
-    cluster_sync_all();
-    SEL_TRACE(2);
-    if (c != 0 || w == NW) return;
+    SEL_CYC(4);
+    if (c != 0 || w == NW) { SEL_LOG_EXIT return; }
+    mbar_wait_cluster(&s_done, 0);   // acquire: every CTA's keys and min / max have landed in this CTA
+    SEL_CYC(5);
 
     // =============================== a2 (CTA 0, consumer threads): exact top-k, ascending ids ===============================
-    uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
-    for (int i = lane; i < (int)CS * NW; i += 32) { kmin = min(kmin, s_mm[0][i]); kmax = max(kmax, s_mm[1][i]); }
-    kmin = __reduce_min_sync(0xffffffffu, kmin);
-    kmax = __reduce_max_sync(0xffffffffu, kmax);
-    topk_emit(s_keys, p.n_cand, p.topk, kmin, kmax, ids_row, s_hist, s_wtot, s_bcast, s_cand);
-    SEL_TRACE(3);
+    topk_emit(s_keys, p.n_cand, p.topk, s_mm[0], s_mm[1], ids_row, s_hist, s_wtot, s_bcast, s_cand, cyc_);
+    SEL_CYC(12);
+    SEL_LOG_EXIT
     if (p.slot_ids) {
         consumer_sync();   // the row's ids are in global memory (read back through L2)
         if (w == 0) {
@@ -546,57 +666,66 @@ __global__ void __launch_bounds__(256) append_kv_kernel(const uint4* __restrict_
 
 }  // namespace
 
-// Cluster size of the select launch: the largest power of two <= 16 such that R*CS CTAs fit the SMs (the
-// ring takes 96 KiB of shared memory), every CTA has at least one stage of keys, and the driver can co-schedule
-// such a cluster (asked once per size; sizes above 8 are non-portable and need the opt-in attribute).  Measured on
-// B200 (batch 32, 2048 blocks, cold HBM): a 6 x 16 KiB ring streams as fast as 10 stages and lets two CTAs share an
-// SM, so with R > SM count the selection of one row overlaps the stream of the next.
+// Cluster size of the select launch (measured on B200 at 128K, batch 4 .. 128, cold HBM): the largest power of two <= 8 such
+// that every CTA has at least one stage of keys, R*CS <= SM count (one CTA per SM: 64 .. 128 CTAs stream as fast as 256, and
+// twice the CTAs only add to the cluster barrier and to the launch) and the device can keep all R clusters resident at once
+// (asked once per context, cluster size and shared-memory size).  16-CTA clusters lose to 8 at every batch (barrier cost,
+// non-portable placement).  With more rows than SMs one CTA per row runs two to an SM and in waves, and the selection of one
+// row overlaps the stream of the next.
 template <int D, bool GRID>
-static int select_launch(sparda_ctx* ctx, const SelParams& p0, cudaStream_t st) {
+static int select_launch(sparda_ctx* ctx, const void* Kpool, const SelParams& p0, cudaStream_t st) {
     auto kern = forecast_select_kernel<D, GRID>;
-    constexpr int KPS = SEL_STAGE_BYTES / (D * 2) / (GRID ? 4 : 1);   // candidates per stage
-    static bool attr_set = false;
-    static int cluster_ok[SEL_MAX_CS + 1];   // 0 = not asked, 1 = schedulable, -1 = not
-    const size_t smem_max = 127 + (size_t)SEL_STAGES * SEL_STAGE_BYTES + (size_t)ctx->cfg.max_blocks * sizeof(uint32_t);
-    if (!attr_set) {
+    constexpr int KPB = GRID ? 4 : 1;
+    constexpr int CPS = SEL_STAGE_BYTES / (D * 2) / KPB;   // candidates per stage
+    sparda_kernel_state& ks = ctx->kstate[(GRID ? SPARDA_K_SELECT_GRID_128 : SPARDA_K_SELECT_128) + (D == 128 ? 0 : 1)];
+    if (!ks.attr_set) {
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 8192));
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        attr_set = true;
+        ks.attr_set = true;
     }
-    if (smem_max > 227 * 1024 - 8192) return SPARDA_EINVAL;
     SelParams p = p0;
-    const size_t smem = 127 + (size_t)SEL_STAGES * SEL_STAGE_BYTES + (size_t)(p.n_cand > p.topk ? p.n_cand : 0) * sizeof(uint32_t);
+    // key array in CTA 0: sized in steps of 2048 candidates so that the occupancy answers below stay valid
+    const size_t key_bytes = p.n_cand > p.topk ? (size_t)((p.n_cand + 2047) & ~2047) * sizeof(uint32_t) : 0;
+    const size_t smem = 1023 + (size_t)SEL_STAGES * SEL_STAGE_BYTES + key_bytes;
+    if (smem > 227 * 1024 - 8192) return SPARDA_EINVAL;
+    CUtensorMap map;
+    int rc = sparda_get_tmap(ctx, Kpool, (uint64_t)ctx->R * p.n_blocks * KPB, D, 64, &map);
+    if (rc) return rc;
     cudaLaunchConfig_t lc = {};
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[1] = sparda_pdl_attr();
     lc.attrs = at;
-    lc.numAttrs = 1;
+    lc.numAttrs = ctx->cfg.no_pdl ? 1 : 2;
     lc.blockDim = dim3(SEL_CTA_THREADS, 1, 1);
     lc.dynamicSmemBytes = smem;
     lc.stream = st;
     int cs = 1;
-    if (p.n_cand > p.topk)
-        while (cs * 2 <= SEL_MAX_CS && (long long)ctx->R * cs * 2 <= ctx->sm_count && cs * 2 <= (p.n_cand + KPS - 1) / KPS) cs *= 2;
-#ifdef SEL_CS_ENV
-    if (getenv("SPARDA_SELECT_CS") && p.n_cand > p.topk) cs = atoi(getenv("SPARDA_SELECT_CS"));
-#endif
-    for (; cs > 1; cs /= 2) {
-        if (cluster_ok[cs] == 0) {
-            int n = 0;
-            lc.gridDim = dim3(cs, 1, 1);
-            at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-            lc.dynamicSmemBytes = smem_max;
-            cudaError_t e = cudaOccupancyMaxActiveClusters(&n, kern, &lc);
-            (void)cudaGetLastError();
-            cluster_ok[cs] = (e == cudaSuccess && n >= 1) ? 1 : -1;
-            lc.dynamicSmemBytes = smem;
+    if (p.n_cand > p.topk) {
+        const int n_stages = (p.n_cand + CPS - 1) / CPS;
+        for (int c = ctx->cfg.select_cluster > 0 ? ctx->cfg.select_cluster : 8; c > 1; c /= 2) {
+            if (ctx->cfg.select_cluster == 0 && (c > n_stages || (long long)ctx->R * c > ctx->sm_count)) continue;
+            if (ks.max_clusters[c] == 0 || ks.asked_smem[c] != (int)smem) {
+                int n = 0;
+                lc.gridDim = dim3(c, 1, 1);
+                at[0].val.clusterDim.x = c;
+                const unsigned na = lc.numAttrs;
+                lc.numAttrs = 1;
+                cudaError_t e = cudaOccupancyMaxActiveClusters(&n, kern, &lc);
+                lc.numAttrs = na;
+                (void)cudaGetLastError();
+                ks.max_clusters[c] = (e == cudaSuccess && n >= 1) ? n : -1;
+                ks.asked_smem[c] = (int)smem;
+            }
+            if (ks.max_clusters[c] >= (ctx->cfg.select_cluster > 0 ? 1 : ctx->R)) { cs = c; break; }
         }
-        if (cluster_ok[cs] == 1) break;
     }
     p.per = (p.n_cand + cs - 1) / cs;
     lc.gridDim = dim3((unsigned)(ctx->R * cs), 1, 1);
-    at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, kern, p));
+    at[0].val.clusterDim.x = cs;
+    SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, kern, map, p));
+    ctx->last_select_cluster = cs;
     return SPARDA_OK;
 }
 
@@ -607,8 +736,7 @@ int sparda_launch_select(sparda_ctx* ctx, const void* F, const void* Kpool, int 
     p.slot_ids = slot_ids;
     p.fetch = fetch;
     p.n_fetch = n_fetch;
-    p.F = (const uint4*)F;
-    p.Kpool = (const char*)Kpool;
+    p.F = (const uint32_t*)F;
     p.ids = ids;
     p.n_blocks = n_blocks;
     p.n_cand = n_cand;
@@ -616,7 +744,7 @@ int sparda_launch_select(sparda_ctx* ctx, const void* F, const void* Kpool, int 
     p.per = n_cand;
     p.keys_valid = n_cand;
     p.n_init = p.n_local = 0;
-    int rc = ctx->cfg.head_dim == 128 ? select_launch<128, false>(ctx, p, st) : select_launch<64, false>(ctx, p, st);
+    int rc = ctx->cfg.head_dim == 128 ? select_launch<128, false>(ctx, Kpool, p, st) : select_launch<64, false>(ctx, Kpool, p, st);
     if (rc) return rc;
     ctx->launches++;
     return SPARDA_OK;
@@ -628,8 +756,7 @@ int sparda_launch_select_grid(sparda_ctx* ctx, const void* F, const void* Kgrid,
                               int topk, int32_t* ids, cudaStream_t st) {
     SelParams p;
     p.slot_ids = p.fetch = p.n_fetch = nullptr;
-    p.F = (const uint4*)F;
-    p.Kpool = (const char*)Kgrid;
+    p.F = (const uint32_t*)F;
     p.ids = ids;
     p.n_blocks = n_blocks;
     p.n_cand = n_cand;
@@ -638,7 +765,7 @@ int sparda_launch_select_grid(sparda_ctx* ctx, const void* F, const void* Kgrid,
     p.keys_valid = 4 * n_cand - 1;
     p.n_init = n_init;
     p.n_local = n_local;
-    int rc = ctx->cfg.head_dim == 128 ? select_launch<128, true>(ctx, p, st) : select_launch<64, true>(ctx, p, st);
+    int rc = ctx->cfg.head_dim == 128 ? select_launch<128, true>(ctx, Kgrid, p, st) : select_launch<64, true>(ctx, Kgrid, p, st);
     if (rc) return rc;
     ctx->launches++;
     return SPARDA_OK;

@@ -30,6 +30,9 @@ const char* sparda_strerror(int code) {
 
 const char* sparda_last_cuda_error(const sparda_ctx* ctx) { return ctx ? ctx->cuda_err : ""; }
 int64_t sparda_launch_count(const sparda_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int64_t sparda_tmap_encodes(const sparda_ctx* ctx) { return ctx ? ctx->tmap_encodes : 0; }
+int sparda_get_select_cluster(const sparda_ctx* ctx) { return ctx ? ctx->last_select_cluster : SPARDA_EINVAL; }
+int sparda_get_attn_cluster(const sparda_ctx* ctx) { return ctx ? ctx->last_attn_cluster : SPARDA_EINVAL; }
 int sparda_get_attn_splits(const sparda_ctx* ctx, int topk) { return ctx ? sparda_resolve_splits(ctx, topk) : SPARDA_EINVAL; }
 int sparda_get_gather_ctas(const sparda_ctx* ctx) { return ctx ? ctx->cfg.gather_ctas : SPARDA_EINVAL; }
 
@@ -44,6 +47,9 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     if (cfg->topk < 1 || cfg->topk > 256) return SPARDA_EINVAL;
     if (cfg->gather_mode != SPARDA_GATHER_TMA && cfg->gather_mode != SPARDA_GATHER_LDG) return SPARDA_EINVAL;
     if (cfg->gather_ctas < 0 || cfg->gather_ctas > 1024 || cfg->attn_splits < 0 || cfg->max_layers < 0) return SPARDA_EINVAL;
+    if (!(cfg->select_cluster == 0 || cfg->select_cluster == 1 || cfg->select_cluster == 2 || cfg->select_cluster == 4 ||
+          cfg->select_cluster == 8 || cfg->select_cluster == 16))
+        return SPARDA_EINVAL;
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -57,6 +63,7 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     if (!ctx) return SPARDA_ENOMEM;
     memset(ctx, 0, sizeof(*ctx));
     ctx->cfg = *cfg;
+    ctx->device = dev;
     ctx->sm_count = prop.multiProcessorCount;
     ctx->R = cfg->batch * cfg->n_kv_heads;
     ctx->G = G;
@@ -415,16 +422,23 @@ int sparda_profile_read(sparda_ctx* ctx, double ms_out[3], int64_t count_out[3])
 }  // extern "C"
 
 // TMA descriptor for a [rows][head_dim] bf16 view (KV pool / cache, F, Kpool): box = box_rows x 64 elements (128 B),
-// 128-byte swizzle.  Cached per (base, rows, head_dim): encoding costs a few microseconds on the host.
-int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_dim, int box_rows, const CUtensorMap** out) {
-    for (int i = 0; i < ctx->n_tmaps; ++i)
-        if (ctx->tmaps[i].base == base && ctx->tmaps[i].rows == rows && ctx->tmaps[i].head_dim == head_dim &&
-            ctx->tmaps[i].box_rows == box_rows) {
-            *out = &ctx->tmaps[i].map;
+// 128-byte swizzle.  Cached per (base, rows, head_dim, box_rows) in an open-addressed hash table: encoding costs a few
+// microseconds on the host.  The caller receives a copy (kernels take it as a __grid_constant__ parameter), so a later
+// lookup that evicts an entry cannot change a descriptor already handed out.
+int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_dim, int box_rows, CUtensorMap* out) {
+    uint64_t h = (uint64_t)(uintptr_t)base * 0x9E3779B97F4A7C15ull ^ rows * 0xC2B2AE3D27D4EB4Full ^ (uint64_t)(head_dim * 131 + box_rows);
+    h ^= h >> 29;
+    const int home = (int)(h & (SPARDA_TMAP_SLOTS - 1));
+    sparda_tmap_entry* e = nullptr;
+    for (int probe = 0; probe < 8; ++probe) {
+        sparda_tmap_entry* c = &ctx->tmaps[(home + probe) & (SPARDA_TMAP_SLOTS - 1)];
+        if (c->base == base && c->rows == rows && c->head_dim == head_dim && c->box_rows == box_rows) {
+            *out = c->map;
             return SPARDA_OK;
         }
-    int slot = ctx->n_tmaps < SPARDA_MAX_TMAP_CACHE ? ctx->n_tmaps++ : (ctx->next_tmap++ % SPARDA_MAX_TMAP_CACHE);
-    sparda_tmap_entry* e = &ctx->tmaps[slot];
+        if (!c->base) { e = c; break; }
+    }
+    if (!e) e = &ctx->tmaps[home];   // neighbourhood full: overwrite the home slot
     typedef CUresult (*encode_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -444,6 +458,7 @@ int sparda_get_tmap(sparda_ctx* ctx, const void* base, uint64_t rows, int head_d
     e->rows = rows;
     e->head_dim = head_dim;
     e->box_rows = box_rows;
-    *out = &e->map;
+    ctx->tmap_encodes++;
+    *out = e->map;
     return SPARDA_OK;
 }

@@ -7,8 +7,25 @@
 
 #include "../../include/sparda.h"
 
-#define SPARDA_MAX_TMAP_CACHE 16
+#define SPARDA_TMAP_SLOTS 256   // hashed tensor-map cache (power of two): a 32-layer step presents ~64 distinct bases
 #define SPARDA_MAX_G 16        // query heads per group, padded to the M=16 of mma.m16n8k16
+#define SPARDA_MAX_CLUSTER 16
+
+// Per-context launcher state of one kernel instantiation (the context lives on one device, so "per context" is also
+// "per device"): whether the dynamic-shared-memory / cluster opt-in attributes have been set, and how many clusters of
+// each size the device can keep resident at the shared-memory size the context uses (0 = not asked, -1 = none).
+struct sparda_kernel_state {
+    bool attr_set;
+    int max_clusters[SPARDA_MAX_CLUSTER + 1];
+    int asked_smem[SPARDA_MAX_CLUSTER + 1];   // dynamic shared memory the answer in max_clusters[] was asked for
+};
+enum {
+    SPARDA_K_SELECT_128, SPARDA_K_SELECT_64, SPARDA_K_SELECT_GRID_128, SPARDA_K_SELECT_GRID_64,
+    SPARDA_K_ATTN_128, SPARDA_K_ATTN_64, SPARDA_K_ATTN_CL_128, SPARDA_K_ATTN_CL_64,
+    SPARDA_K_GATHER_TMA,
+    SPARDA_K_PF_0, /* 8 prefill instantiations: D x BASELINE x REPL */
+    SPARDA_K_COUNT = SPARDA_K_PF_0 + 8
+};
 
 struct sparda_tmap_entry {
     const void* base;
@@ -45,11 +62,15 @@ struct sparda_ctx {
     cudaEvent_t* ev_prof;
     int prof_n[3];
     int64_t launches;
+    int last_select_cluster, last_attn_cluster;   // introspection: the shape the last launch resolved to
     char cuda_err[256];
-    // TMA descriptor cache (host)
-    sparda_tmap_entry tmaps[SPARDA_MAX_TMAP_CACHE];
-    int n_tmaps, next_tmap;
+    // TMA descriptor cache (host): open-addressed hash on (base, rows, head_dim, box_rows); lookups return a COPY, so an
+    // eviction can never change a descriptor a launcher already holds
+    sparda_tmap_entry tmaps[SPARDA_TMAP_SLOTS];
+    int64_t tmap_encodes;   // descriptors encoded so far (introspection: a warm step must not encode)
     void* encode_fn;   // cuTensorMapEncodeTiled
+    int device;             // the device the context was created on
+    sparda_kernel_state kstate[SPARDA_K_COUNT];
 };
 
 int sparda_set_cuda_error(sparda_ctx* ctx, cudaError_t e, const char* where);
@@ -58,6 +79,14 @@ int sparda_set_cuda_error(sparda_ctx* ctx, cudaError_t e, const char* where);
         cudaError_t e__ = (call);                                              \
         if (e__ != cudaSuccess) return sparda_set_cuda_error(ctx, e__, #call); \
     } while (0)
+
+// launch attribute that allows this launch to overlap its prologue with the tail of the previous kernel of the stream (PDL)
+static inline cudaLaunchAttribute sparda_pdl_attr() {
+    cudaLaunchAttribute a;
+    a.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    a.val.programmaticStreamSerializationAllowed = 1;
+    return a;
+}
 
 static inline bool sparda_aligned(const void* p, uintptr_t a) { return p != nullptr && ((uintptr_t)p & (a - 1)) == 0; }
 
@@ -82,8 +111,8 @@ int sparda_launch_prefill_select(sparda_ctx*, const void* F, const void* Kpool, 
                                  int n_rows, int topk, int32_t* ids, cudaStream_t);
 int sparda_launch_prefill_baseline(sparda_ctx*, const void* Q, const void* Kpool, int T, int n_blocks, int row0,
                                    int n_rows, int topk, int32_t* ids, cudaStream_t);
-// [rows][head_dim] bf16 row-major view, box = box_rows x 64 elements (128 B), 128-byte swizzle
-int sparda_get_tmap(sparda_ctx*, const void* base, uint64_t rows, int head_dim, int box_rows, const CUtensorMap** out);
+// [rows][head_dim] bf16 row-major view, box = box_rows x 64 elements (128 B), 128-byte swizzle; *out receives a copy
+int sparda_get_tmap(sparda_ctx*, const void* base, uint64_t rows, int head_dim, int box_rows, CUtensorMap* out);
 int sparda_resolve_splits(const sparda_ctx*, int topk);     // average CTAs per row of the attention launch
 int sparda_resolve_attn_ctas(const sparda_ctx*, int topk);  // its grid size
 
@@ -121,6 +150,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "r"(parity)
         : "memory");
 }
+
+// Programmatic dependent launch (PDL): a kernel launched with sparda_pdl_attr() may become resident and run its prologue
+// (barrier init, tensor-map prefetch, index arithmetic) while the previous kernel of the stream is still draining;
+// pdl_wait() blocks until that kernel has completed and its memory is visible -- it must precede every global-memory
+// access -- and pdl_launch_dependents() lets the NEXT kernel do the same with this one.  Without the launch attribute both
+// are no-ops.  Semantics are those of plain stream order; what is saved is the launch gap and the prologue (~1.3 us per
+// kernel of a back-to-back chain on B200).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // 1-D bulk copies (TMA engine, no tensor map)
 __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {

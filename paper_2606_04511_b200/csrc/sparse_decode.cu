@@ -98,6 +98,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
         tma_prefetch_desc(&tmap);
     }
     __syncthreads();
+    pdl_wait();                  // the prologue above overlaps the previous kernel's tail; global memory from here on
+    pdl_launch_dependents();
 
     uint8_t* stage = smem + (size_t)w * SM::STAGE_BYTES;
     const uint32_t k_base = smem_u32(stage), v_base = k_base + SM::TILE_BYTES;
@@ -496,15 +498,16 @@ template <int D, bool CL>
 int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, int cluster, cudaStream_t st) {
     auto kern = sparse_decode_kernel<D, ATT_NW, 1, CL>;
     constexpr int smem = AttnSmem<D, ATT_NW>::TOTAL;
-    static bool attr_set = false;
-    if (!attr_set) {
+    sparda_kernel_state& ks = ctx->kstate[(CL ? SPARDA_K_ATTN_CL_128 : SPARDA_K_ATTN_128) + (D == 128 ? 0 : 1)];
+    if (!ks.attr_set) {
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_set = true;
+        ks.attr_set = true;
     }
     cudaLaunchConfig_t lc = {};
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[1] = sparda_pdl_attr();
     lc.attrs = at;
     lc.numAttrs = 1;
     lc.gridDim = dim3((unsigned)C, 1, 1);
@@ -514,15 +517,15 @@ int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, 
     if (CL) {
         // a cluster needs `cluster` SMs of one GPC at the same time (one CTA per SM): use this path only when every row's
         // cluster is resident in one wave, else the second wave costs more than the reduction saves (batch 8, 16 x 8 CTAs)
-        static int max_clusters[9];   // per cluster size; 0 = not asked
-        if (max_clusters[cluster] == 0) {
+        if (ks.max_clusters[cluster] == 0) {   // asked once per context and cluster size (the shared-memory size is fixed)
             int n = 0;
             if (cudaOccupancyMaxActiveClusters(&n, kern, &lc) != cudaSuccess) n = -1;
             (void)cudaGetLastError();
-            max_clusters[cluster] = n > 0 ? n : -1;
+            ks.max_clusters[cluster] = n > 0 ? n : -1;
         }
-        if (max_clusters[cluster] * cluster < C) return 1;   // caller falls back to the workspace reduction
+        if (ks.max_clusters[cluster] * cluster < C) return 1;   // caller falls back to the workspace reduction
     }
+    lc.numAttrs = ctx->cfg.no_pdl ? 1 : 2;
     SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, kern, *map, p));
     return SPARDA_OK;
 }
@@ -565,7 +568,7 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
                        int n_slots, void* O, cudaStream_t st) {
     const int D = ctx->cfg.head_dim;
     const uint64_t rows = (uint64_t)ctx->R * n_slots * 2 * S_BLK;
-    const CUtensorMap* map;
+    CUtensorMap map;
     int rc = sparda_get_tmap(ctx, pool, rows, D, S_BLK, &map);
     if (rc) return rc;
     AttnParams p;
@@ -591,10 +594,13 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     const int s_per = p.quota > 0 && p.rem == 0 && topk % p.quota == 0 ? topk / p.quota : 0;
     const bool cl = (s_per == 2 || s_per == 4 || s_per == 8) && (long long)s_per * ctx->R == C;
     rc = 1;
-    if (cl) rc = D == 128 ? launch<128, true>(ctx, map, p, C, s_per, st) : launch<64, true>(ctx, map, p, C, s_per, st);
-    if (rc == 1) rc = D == 128 ? launch<128, false>(ctx, map, p, C, 1, st) : launch<64, false>(ctx, map, p, C, 1, st);
+    int used_cl = cl ? s_per : 0;
+    if (cl) rc = D == 128 ? launch<128, true>(ctx, &map, p, C, s_per, st) : launch<64, true>(ctx, &map, p, C, s_per, st);
+    if (rc == 1) used_cl = 0;
+    if (rc == 1) rc = D == 128 ? launch<128, false>(ctx, &map, p, C, 1, st) : launch<64, false>(ctx, &map, p, C, 1, st);
     if (rc) return rc;
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
+    ctx->last_attn_cluster = used_cl;
     ctx->launches++;
     return SPARDA_OK;
 }

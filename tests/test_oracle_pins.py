@@ -574,7 +574,7 @@ def test_paper_closed_forms_golden():
     hidden = 4096
     n_proj = c.n_layers                 # 31 lookahead projections + the layer-0 same-layer one
     params = hidden * c.n_kv_heads * c.head_dim * n_proj
-    assert round(params / 1e6, 1) == vals["forecast_params_millions"]
+    assert abs(params / 1e6 - vals["forecast_params_millions"]) < 0.1          # P:L95 prints 33.5M
     assert 7.9e9 < params / (vals["forecast_params_percent_of_8b"] / 100) < 8.4e9      # "of the 8B total"
     per_seq = c.n_layers * c.kv_bytes_per_layer / c.batch
     assert round(per_seq / 1e9, 1) == vals["kv_gb_per_sequence_128k"]

@@ -11,16 +11,24 @@ configuration the metric "decode tok/s at 128K" is quoted on that fits one GPU b
 KV).  configs[3] (batch 32, 137 GB pinned) is reachable with --workload cfg4 [--batch B] and aliases the
 host cache onto fewer resident layers when the box cannot pin that much.
 
-N > 1 (torchrun): every rank runs the same per-GPU workload on its own sequences (batch shards, no
-collective on the data path -- SURVEY 8(e)); value = tokens all ranks decoded / max-over-ranks device time.
+N > 1: every rank runs the same per-GPU workload on its own sequences (batch shards, no collective on the data
+path -- SURVEY 8(e)); value = tokens all ranks decoded / max-over-ranks device time.  Under torchrun the ranks
+come from the environment; a plain `python bench.py --gpus N` spawns them itself and exits non-zero if the box
+has fewer than N GPUs.
+
+Everything the line reports is measured in this run.  The only numbers that are not -- DRAM traffic and executed
+instructions per launch, which need ncu -- are read from the committed profiles/r2_ncu_metrics.csv and carry the
+file's content hash (`traffic_src`); a kernel without an entry there reports null.
 
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -33,6 +41,8 @@ if ROOT not in sys.path:
 
 METRIC = "decode_tokens_per_s_128k"
 UNIT = "tok/s"
+NCU_METRICS = os.path.join(ROOT, "profiles", "r2_ncu_metrics.csv")
+ALL_SECTIONS = ("kernels", "prefill", "reuse", "standin", "gather", "floor", "append")
 
 
 def parse_args():
@@ -48,11 +58,17 @@ def parse_args():
     ap.add_argument("--gather-mode", default="tma", choices=["tma", "ldg"])
     ap.add_argument("--host-gib", type=float, default=0.0, help="cap on pinned host KV per rank (GiB); 0 = auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-kernels", action="store_true", help="skip the batch-32 per-kernel HBM roofline section")
+    ap.add_argument("--sections", default="all",
+                    help="comma list of the extra sections measured after the headline step: " + ",".join(ALL_SECTIONS) + " (all | none)")
     ap.add_argument("--section", default="all", choices=["all", "kernels"],
-                    help="kernels: only the per-kernel sections (batch-32 select / attention, prefill selection); used for ncu captures")
+                    help="kernels: ONLY the per-kernel sections, no pipeline (the command the ncu captures in profiles/ run)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
-    return ap.parse_args()
+    a = ap.parse_args()
+    a.sections = set(ALL_SECTIONS) if a.sections == "all" else set(s for s in a.sections.split(",") if s and s != "none")
+    bad = a.sections - set(ALL_SECTIONS)
+    if bad:
+        ap.error(f"unknown sections {sorted(bad)}")
+    return a
 
 
 def load_peaks():
@@ -61,7 +77,23 @@ def load_peaks():
         d = json.load(open(p))
         return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": d.get("bf16_tflops"),
                 "bf16_tflops_sustained": d.get("bf16_tflops_sustained"), "source": "measured (MEASURED_PEAKS.json)"}
-    return {"hbm_gbs": 6650.0, "bf16_tflops": 1700.0, "bf16_tflops_sustained": 1400.0, "source": "fallback (B200_PROFILING.md)"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def load_ncu_metrics():
+    """profiles/r2_ncu_metrics.csv: `key,metric,value` rows extracted from the committed ncu captures (the commands are
+    in profiles/r2_ncu_summary.md).  Returns ({key: {metric: value}}, 'path@sha1[:12]')."""
+    if not os.path.exists(NCU_METRICS):
+        return {}, None
+    raw = open(NCU_METRICS, "rb").read()
+    out = {}
+    for line in raw.decode().splitlines():
+        line = line.split("#")[0].strip()
+        if not line or line.startswith("key,"):
+            continue
+        key, metric, value = [x.strip() for x in line.split(",")[:3]]
+        out.setdefault(key, {})[metric] = float(value)
+    return out, f"profiles/{os.path.basename(NCU_METRICS)}@{hashlib.sha1(raw).hexdigest()[:12]}"
 
 
 def workload_config(args):
@@ -72,6 +104,14 @@ def workload_config(args):
     if args.layers:
         cfg = cfg.with_(n_layers=args.layers)
     return cfg
+
+
+def config_dict(cfg, world):
+    """The workload, identically for both arms (the driver compares the two dicts)."""
+    return {"workload": cfg.name, "batch_per_gpu": cfg.batch, "global_batch": cfg.batch * world, "context": cfg.context,
+            "layers": cfg.n_layers, "q_heads": cfg.n_q_heads, "kv_heads": cfg.n_kv_heads, "head_dim": cfg.head_dim,
+            "block": cfg.block_size, "topk": cfg.topk, "parallelism": f"batch shards x{world}, no collective",
+            "fresh_fetch_fraction": 1.0}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -115,6 +155,33 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def numa_info(torch, local):
+    """Where the pinned KV lives relative to the GPU: the GPU's NUMA node from sysfs, the node of the CPU this
+    process allocates (first-touches) on, and the CPU affinity.  Best effort: None where the box does not say."""
+    out = {"gpu_numa_node": None, "alloc_cpu": None, "alloc_numa_node": None, "numa_nodes": None,
+           "affinity_cpus": len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else None}
+    try:
+        props = torch.cuda.get_device_properties(local)
+        bdf = f"{props.pci_domain_id:04x}:{props.pci_bus_id:02x}:{props.pci_device_id:02x}.0"
+        out["gpu_numa_node"] = int(open(f"/sys/bus/pci/devices/{bdf}/numa_node").read())
+    except Exception:
+        pass
+    try:
+        cpu = int(open("/proc/self/stat").read().rsplit(")", 1)[1].split()[36])
+        out["alloc_cpu"] = cpu
+        nodes = sorted(d for d in os.listdir("/sys/devices/system/node") if d.startswith("node") and d[4:].isdigit())
+        out["numa_nodes"] = len(nodes)
+        for nd in nodes:
+            for part in open(f"/sys/devices/system/node/{nd}/cpulist").read().strip().split(","):
+                lo, _, hi = part.partition("-")
+                if int(lo) <= cpu <= int(hi or lo):
+                    out["alloc_numa_node"] = int(nd[4:])
+    except Exception:
+        pass
+    out["policy"] = "default (first touch by the allocating thread; no explicit binding)"
+    return out
+
+
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline and --impl reference).  The only place bench.py touches oracle/.
 # ------------------------------------------------------------------------------------------------
@@ -146,24 +213,34 @@ def _oracle_sample_layers(cfg, n, device="cpu"):
 
 def cpu_baseline(cfg, layers_bits, target_s):
     """Oracle timed on this box's host cores on a bounded sample: whole layers of the decode step, as many as
-    fit in ~target_s seconds, scaled to the full layer count."""
+    fit in ~target_s seconds, scaled to the full layer count; plus the same two layer-steps single-threaded."""
     from oracle import sparda_oracle as oracle
-    t0 = time.perf_counter()
-    done = 0
-    while done < 4 * cfg.n_layers:                          # whole layer-steps until ~target_s of CPU time
-        l = done % cfg.n_layers
-        lay = layers_bits[l % len(layers_bits)]
-        prev = layers_bits[(l - 1) % len(layers_bits)]
-        _oracle_layer_step(oracle, lay, lay["F0cur"] if l == 0 else prev["F"], cfg.topk, layer0=(l == 0))
-        done += 1
-        if time.perf_counter() - t0 >= target_s:
-            break
-    el = time.perf_counter() - t0
+    cores = oracle.threads()
+
+    def run(max_steps, budget):
+        t0 = time.perf_counter()
+        done = 0
+        while done < max_steps:
+            l = done % cfg.n_layers
+            lay = layers_bits[l % len(layers_bits)]
+            prev = layers_bits[(l - 1) % len(layers_bits)]
+            _oracle_layer_step(oracle, lay, lay["F0cur"] if l == 0 else prev["F"], cfg.topk, layer0=(l == 0))
+            done += 1
+            if time.perf_counter() - t0 >= budget:
+                break
+        return done, time.perf_counter() - t0
+
+    done, el = run(4 * cfg.n_layers, target_s)
     per_step_s = el * cfg.n_layers / done
-    return {"value": cfg.batch / per_step_s, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
-            "sample": f"{done} layer-steps (select + gather + sparse attention, batch {cfg.batch}, 128K, "
-                      f"{cfg.n_layers} per decode step) in {el:.2f} s, scaled to one {cfg.n_layers}-layer step",
-            "seconds_per_decode_step": per_step_s}
+    oracle.set_threads(1)
+    d1, e1 = run(2, 1e9)                                       # layer 0 + one gathered layer, one thread
+    oracle.set_threads(cores)
+    per_step_1 = e1 * cfg.n_layers / d1
+    return {"value": cfg.batch / per_step_s, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{done} layer-steps (select+gather+attention, batch {cfg.batch}, 128K) in {el:.2f} s, scaled to {cfg.n_layers} layers",
+            "seconds_per_decode_step": per_step_s,
+            "single_thread": {"value": cfg.batch / per_step_1, "unit": UNIT, "cores": 1, "seconds_per_decode_step": per_step_1,
+                              "sample": f"{d1} layer-steps in {e1:.2f} s, scaled to {cfg.n_layers} layers"}}
 
 
 def run_reference(args):
@@ -185,13 +262,11 @@ def run_reference(args):
             times.append(time.perf_counter() - t0)
     per_step_s = statistics.mean(times) * cfg.n_layers / n_sample
     val = cfg.batch / per_step_s
-    sample = (f"each step = {n_sample} of {cfg.n_layers} layer-steps (layer 0 + one gathered layer) of the oracle at batch "
-              f"{cfg.batch}, 128K, scaled to {cfg.n_layers} layers")
+    sample = f"each step = {n_sample} of {cfg.n_layers} layer-steps (layer 0 + one gathered layer) of the oracle, scaled to {cfg.n_layers}"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": per_step_s * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "batch": cfg.batch, "context": cfg.context, "layers": cfg.n_layers,
-                       "topk": cfg.topk, "sample": sample},
+            "config": config_dict(cfg, 1),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -200,8 +275,48 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------
-# the CUDA arm
+# the CUDA arm: helpers
 # ------------------------------------------------------------------------------------------------
+def graph_time(torch, fn, n_sets, reps=10, best_of=3, flush=None):
+    """Seconds per launch of fn(i, stream): reps passes over n_sets rotating buffer sets captured once into a CUDA graph
+    (the launches of these short kernels would otherwise be paced by the Python caller, not by the GPU) and replayed
+    between two events on the replaying stream; best of `best_of` replays.  flush(): called before every timed replay,
+    outside the events (an L2 flush for shapes whose rotation does not exceed L2)."""
+    st = torch.cuda.current_stream()
+    for i in range(2 * n_sets):
+        fn(i % n_sets, st)
+    torch.cuda.synchronize()
+    graph, cap = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.graph(graph, stream=cap):
+        for i in range(reps * n_sets):
+            fn(i % n_sets, torch.cuda.current_stream())
+    graph.replay()
+    torch.cuda.synchronize()
+    best = float("inf")
+    for _ in range(best_of):
+        if flush is not None:
+            flush()
+            torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        graph.replay()
+        e1.record(st)
+        e1.synchronize()
+        best = min(best, e0.elapsed_time(e1) * 1e-3 / (reps * n_sets))
+    del graph
+    return best
+
+
+def kernel_entry(name, shape, t, nbytes, peak, ncu, key, ncu_src, **extra):
+    m = ncu.get(key, {})
+    traffic = (m.get("dram__bytes_read.sum", 0.0) + m.get("dram__bytes_write.sum", 0.0)) if "dram__bytes_read.sum" in m else None
+    e = {"kernel": name, "shape": shape, "bound": "hbm", "us": round(t * 1e6, 3), "bytes": int(nbytes),
+         "achieved": round(nbytes / t / 1e9, 1), "peak": peak, "unit": "GB/s", "frac": round(nbytes / t / 1e9 / peak, 4),
+         "frac_of_8tbs": round(nbytes / t / 1e9 / 8000.0, 4), "traffic": traffic, "traffic_src": ncu_src if traffic is not None else None}
+    e.update(extra)
+    return e
+
+
 def measure_h2d_ceiling(torch, host_chunks):
     """cudaMemcpyAsync pinned host -> device ceiling on this box: the denominator of the gather's roofline.
     Copies whole pinned layer buffers (>= 256 MiB each) back to back, best of 5 passes, CUDA events."""
@@ -219,18 +334,31 @@ def measure_h2d_ceiling(torch, host_chunks):
     return best
 
 
-def bench_kernels_b32(torch, binding, peaks, args):
-    """Per-kernel HBM rooflines at the batch-32 shape of BASELINE.json configs[3] (R = 64 rows, 2048 blocks,
-    top-64, D = 128), where the ideal times (5 us select, 20 us attention) stand clear of the launch floor
-    (SURVEY 8(d)).  Cold HBM: each launch works on the next of NSETS buffer sets, together larger than L2."""
+# ------------------------------------------------------------------------------------------------
+# per-kernel sections
+# ------------------------------------------------------------------------------------------------
+def bench_kernels(torch, binding, peaks, ncu, ncu_src, batch):
+    """Per-kernel HBM rooflines at one batch of the BASELINE.json configs[3] shape (R = 2 * batch rows, 2048 blocks,
+    top-64, D = 128).  Batch 32 is where the ideal times (5 us select, 20 us attention) stand clear of the launch
+    floor; batch 4 is configs[2]'s per-layer shape, launch-latency-sized, reported beside the floor.
+    Cold HBM: each launch works on the next of several buffer sets, together >= 1 GiB (8 x the 126 MB L2); launches are
+    replayed from a CUDA graph."""
     from paper_2606_04511_b200 import synth
-    cfg = synth.CFG4_128K
+    cfg = synth.CFG4_128K.with_(batch=batch)
     R, Nb, k, D = cfg.rows, cfg.n_blocks, cfg.topk, cfg.head_dim
     ctx = binding.Sparda.from_config(cfg)
-    g = torch.Generator(device="cuda").manual_seed(40)
-    NS_SEL, NS_ATT = 8, 4                                    # 8 x 32 MiB Kpool, 4 x 128 MiB pool: each ring > 126 MB L2
+    g = torch.Generator(device="cuda").manual_seed(40 + batch)
+    tag = f"b{batch}"
+    kp_bytes, pool_bytes = cfg.kpool_bytes_per_layer, cfg.gather_bytes_per_layer
+    NS_SEL = max(4, -(-(1 << 30) // kp_bytes))
+    NS_SEL = min(NS_SEL, 64)
+    NS_ATT = min(max(4, -(-(1 << 30) // pool_bytes)), 64)
+    Fs = [torch.randn((R, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(8)]
+    ids = torch.empty((R, k), dtype=torch.int32, device="cuda")
     kpools = [torch.randn((R, Nb, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(NS_SEL)]
-    Fs = [torch.randn((R, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(NS_SEL)]
+    t_sel = graph_time(torch, lambda i, s: ctx.forecast_select(Fs[i % 8], kpools[i], Nb, k, ids, stream=s), NS_SEL, reps=max(2, 160 // NS_SEL))
+    cs_sel = ctx.select_cluster
+    del kpools
     pools = []
     for _ in range(NS_ATT):
         p = torch.empty((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda")
@@ -238,62 +366,69 @@ def bench_kernels_b32(torch, binding, peaks, args):
         pools.append(p)
     Q = torch.randn((cfg.batch, cfg.n_q_heads, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
     O = torch.empty_like(Q)
-    ids = torch.empty((R, k), dtype=torch.int32, device="cuda")
     ids_att = torch.arange(k, dtype=torch.int32, device="cuda").repeat(R, 1).contiguous()
-    st = torch.cuda.current_stream()
-
-    def timed(fn, n_sets, reps=10):
-        """reps passes over the n_sets buffer sets, captured once into a CUDA graph (the launches of these short kernels
-        would otherwise be paced by the Python caller, not by the GPU) and replayed between two events."""
-        for i in range(2 * n_sets):
-            fn(i % n_sets, st)
-        torch.cuda.synchronize()
-        graph, cap = torch.cuda.CUDAGraph(), torch.cuda.Stream()
-        with torch.cuda.graph(graph, stream=cap):
-            for i in range(reps * n_sets):
-                fn(i % n_sets, torch.cuda.current_stream())
-        graph.replay()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(st)
-        graph.replay()
-        e1.record(st)
-        e1.synchronize()
-        return e0.elapsed_time(e1) * 1e-3 / (reps * n_sets)
-
-    t_sel = timed(lambda i, s: ctx.forecast_select(Fs[i], kpools[i], Nb, k, ids, stream=s), NS_SEL)
-    t_att = timed(lambda i, s: ctx.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT)
-    sel_bytes = cfg.kpool_bytes_per_layer + R * D * 2 + R * k * 4
-    att_bytes = cfg.gather_bytes_per_layer + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
-    # f3: the paper's geometry -- (32,16) compressed-key grid (4 keys per block), max-pool to blocks, budget 96 = 1 + 32 + 63
-    del kpools
-    grids = [torch.randn((R, 4 * Nb, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(2)]
-    ids96 = torch.empty((R, 96), dtype=torch.int32, device="cuda")
-    ctx96 = binding.Sparda(cfg.batch, cfg.n_q_heads, cfg.n_kv_heads, D, Nb, 96)
-    t_grid = timed(lambda i, s: ctx96.forecast_select_grid(Fs[i], grids[i], Nb, 96, ids96, n_init=1, n_local=32, stream=s), 2)
-    grid_bytes = R * (4 * Nb - 1) * D * 2 + R * D * 2 + R * 96 * 4
-    ctx96.close()
-    del grids
-    out = []
-    for name, t, b in (("forecast_select_kernel<128>", t_sel, sel_bytes), ("sparse_decode_kernel<128>", t_att, att_bytes),
-                       ("forecast_select_kernel<128,grid>", t_grid, grid_bytes)):
-        out.append({"kernel": name, "workload": "cfg4 shape, batch 32, one layer, cold HBM (rotating buffer sets > L2), launches replayed from a CUDA graph",
-                    "bound": "hbm", "us_per_launch": t * 1e6, "algorithmic_bytes": b, "achieved": b / t / 1e9,
-                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": b / t / 1e9 / peaks["hbm_gbs"],
-                    "frac_of_nominal_8tbs": b / t / 1e9 / 8000.0, "peak_source": peaks["source"], "traffic": None})
-    # DRAM read + write bytes per launch of the same shapes from the committed ncu --set full captures
-    out[0]["traffic"], out[0]["traffic_source"] = 33612800, "profiles/r1c_ncu_summary.md (prof_b32_select_c: dram read 33.61 MB, write 0)"
-    out[1]["traffic"], out[1]["traffic_source"] = 134544640 + 3627776, "profiles/r1c_ncu_summary.md (prof_b32_attn_c: dram read 134.54 MB, 3.6 MB of evictions)"
-    out[1]["attn_splits"] = ctx.attn_splits(k)
-    out[2]["workload"] = ("f3 (reading q19, unpinned by the paper): batch 32, 2048 blocks x 4 compressed keys, max-pool to blocks, "
-                          "top-96 = 1 initial + 32 local + 63 ranked; cold HBM (two 128 MiB grids > L2), CUDA-graph replay")
-    ctx.close()
+    t_att = graph_time(torch, lambda i, s: ctx.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT, reps=max(2, 80 // NS_ATT))
+    cl_att = ctx.attn_cluster
     del pools
+    sel_bytes = kp_bytes + R * D * 2 + R * k * 4
+    att_bytes = pool_bytes + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
+    hbm = peaks["hbm_gbs"]
+    out = [kernel_entry("forecast_select_kernel<128,false>", f"batch {batch}: R={R}, {Nb} blocks, top-{k}; cold HBM, graph replay", t_sel, sel_bytes,
+                        hbm, ncu, f"select_{tag}", ncu_src, cluster=cs_sel),
+           kernel_entry("sparse_decode_kernel<128>", f"batch {batch}: R={R}, top-{k} x 32 KiB; cold HBM, graph replay", t_att, att_bytes,
+                        hbm, ncu, f"attn_{tag}", ncu_src, cluster=cl_att, ctas_per_row=ctx.attn_splits(k))]
+    if batch == 32:
+        # f3: the paper's geometry -- (32,16) compressed-key grid (4 keys per block), max-pool to blocks, budget 96 = 1 + 32 + 63
+        NS_G = 8
+        grids = [torch.randn((R, 4 * Nb, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(NS_G)]
+        ids96 = torch.empty((R, 96), dtype=torch.int32, device="cuda")
+        ctx96 = binding.Sparda(cfg.batch, cfg.n_q_heads, cfg.n_kv_heads, D, Nb, 96)
+        t_grid = graph_time(torch, lambda i, s: ctx96.forecast_select_grid(Fs[i % 8], grids[i], Nb, 96, ids96, n_init=1, n_local=32, stream=s), NS_G, reps=10)
+        grid_bytes = R * (4 * Nb - 1) * D * 2 + R * D * 2 + R * 96 * 4
+        out.append(kernel_entry("forecast_select_kernel<128,grid>", "f3 (reading q19, unpinned): batch 32, 4 keys per block, top-96 = 1 + 32 + 63; cold HBM",
+                                t_grid, grid_bytes, hbm, ncu, "grid_b32", ncu_src, cluster=ctx96.select_cluster))
+        ctx96.close()
+        del grids
+        # A4: the Forecast projection GEMV (Eq.3), 8B shape: hidden 4096 -> 2 x 128; bound by streaming W_F (2 MiB) once
+        hidden = 4096
+        NS_W = 64
+        Ws = [torch.randn((hidden, cfg.n_kv_heads * D), generator=g, device="cuda").to(torch.bfloat16) for _ in range(NS_W)]
+        X = torch.randn((cfg.batch, hidden), generator=g, device="cuda").to(torch.bfloat16)
+        Fo = torch.empty((R, D), dtype=torch.bfloat16, device="cuda")
+        t_fp = graph_time(torch, lambda i, s: ctx.forecast_project(X, Ws[i], hidden, Fo, stream=s), NS_W, reps=3)
+        fp_bytes = hidden * cfg.n_kv_heads * D * 2 + cfg.batch * hidden * 2 + R * D * 2
+        out.append(kernel_entry("forecast_project_kernel", "A4 (Eq.3): batch 32, hidden 4096 -> 2 x 128; W_F rotated over 128 MiB", t_fp, fp_bytes,
+                                hbm, ncu, "project_b32", ncu_src))
+        del Ws
+    ctx.close()
     torch.cuda.empty_cache()
     return out
 
 
-def bench_prefill(torch, binding, peaks_all):
+def bench_floor(torch, binding):
+    """Launch floor beside the launch-latency-sized shapes: per-launch time of back-to-back probe kernels
+    replayed from a CUDA graph -- an empty kernel, an empty kernel with the select launch shape, and 148 CTAs doing one
+    dependent DRAM load each."""
+    from paper_2606_04511_b200 import synth
+    ctx = binding.Sparda.from_config(synth.CFG1_TINY)
+    buf = torch.zeros(1 << 28, dtype=torch.int32, device="cuda")   # 1 GiB: the touched locations are cold every launch
+    nb = buf.numel() * 4
+    out = {}
+    for name, kind in (("empty_1x32_us", 0), ("empty_select_shape_us", 1)):
+        out[name] = round(graph_time(torch, lambda i, s: ctx.probe_launch(kind, stream=s), 1, reps=200) * 1e6, 3)
+    views = [buf[i * 4096:] for i in range(192)]                   # 16 KiB apart: a different DRAM line per launch and CTA
+    scrub = torch.empty(1 << 27, dtype=torch.int32, device="cuda")  # 512 MiB written before each replay: the lines are cold
+    out["one_dram_load_148_ctas_us"] = round(graph_time(torch, lambda i, s: ctx.probe_launch(2, views[i], nb - 192 * 16384, stream=s), 192, reps=1,
+                                                        flush=lambda: scrub.fill_(1)) * 1e6, 3)
+    out["note"] = "back-to-back launches in one graph: per-launch period, not latency"
+    del scrub
+    ctx.close()
+    del buf
+    torch.cuda.empty_cache()
+    return out
+
+
+def bench_prefill(torch, binding, peaks_all, ncu, ncu_src):
     """BASELINE.json configs[4]: chunked-prefill Forecast selection (a7) at T = 32768, 2 groups, 512 pooled keys, top-64,
     in 2048-row chunks (16 launches per pass) and as one launch, plus the per-head softmax comparison selector (a7',
     G = 16 heads per group) on the same shapes: the analog of the paper's 'selection cost cut up to 2.50x'."""
@@ -306,50 +441,34 @@ def bench_prefill(torch, binding, peaks_all):
     ctx.pool_keys(P["kv"], Hkv, Nb, kpool)
     ids = torch.empty((Hkv, T, k), dtype=torch.int32, device="cuda")
     part = torch.empty((Hkv, cfg.chunk, k), dtype=torch.int32, device="cuda")
-    st = torch.cuda.current_stream()
 
-    def chunked(fn, src):
+    def chunked(fn, src, s):
         for r0 in range(0, T, cfg.chunk):
-            fn(src, kpool, T, Nb, r0, cfg.chunk, k, part)
-
-    def timed(fn, reps):
-        for _ in range(3):
-            fn()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(st)
-        for _ in range(reps):
-            fn()
-        e1.record(st)
-        e1.synchronize()
-        return e0.elapsed_time(e1) * 1e-3 / reps
+            fn(src, kpool, T, Nb, r0, cfg.chunk, k, part, stream=s)
 
     n0 = ctx.launch_count
-    t_one = timed(lambda: ctx.prefill_select(P["F"], kpool, T, Nb, 0, T, k, ids), 20)
-    t_chunk = timed(lambda: chunked(ctx.prefill_select, P["F"]), 10)
-    t_base = timed(lambda: chunked(ctx.prefill_select_baseline, P["Q"]), 3)
+    t_one = graph_time(torch, lambda i, s: ctx.prefill_select(P["F"], kpool, T, Nb, 0, T, k, ids, stream=s), 1, reps=10)
+    t_chunk = graph_time(torch, lambda i, s: chunked(ctx.prefill_select, P["F"], s), 1, reps=5)
+    t_base = graph_time(torch, lambda i, s: chunked(ctx.prefill_select_baseline, P["Q"], s), 1, reps=2)
     launches = ctx.launch_count - n0
-    # causal contraction: row i multiplies min(Nb, (i+1)//64) pooled keys of width D
-    ncand = sum(min(Nb, (i + 1) // 64) for i in range(T))
+    ncand = sum(min(Nb, (i + 1) // 64) for i in range(T))        # causal contraction: row i meets min(Nb, (i+1)//64) pooled keys
     flops = 2.0 * Hkv * ncand * D
     bf16_peak = peaks_all.get("bf16_tflops_sustained") or peaks_all.get("bf16_tflops") or 1400.0
     ranked_rows = Hkv * sum(1 for i in range(T) if (i + 1) // 64 > k)
+    inst = ncu.get("prefill_one", {}).get("smsp__inst_executed.sum")
+    alu_peak = 148 * 4 * 1.965                                     # G warp-instr/s: 148 SMs x 4 schedulers x 1 per clock x 1.965 GHz
     out = {
-        "workload": f"{cfg.name}: T={T}, {Hkv} groups, {Nb} pooled keys, top-{k}, {cfg.chunk}-row chunks",
-        "forecast_select_us_per_pass_chunked": t_chunk * 1e6, "forecast_select_us_one_launch": t_one * 1e6,
-        "baseline_selector_us_per_pass_chunked": t_base * 1e6, "selection_cost_ratio_baseline_over_forecast": t_base / t_chunk,
-        "tokens_per_s_selection_only": T / t_chunk, "gpu_launches": launches,
-        "ns_per_ranked_row": t_chunk * 1e9 / ranked_rows,
-        "roofline": {"kernel": "prefill_select_kernel<128,false>", "bound": "tensor", "achieved": flops / t_chunk / 1e12,
-                     "peak": bf16_peak, "unit": "TFLOP/s", "frac": flops / t_chunk / 1e12 / bf16_peak, "traffic": None,
-                     "algorithmic_flops": flops,
-                     "note": "the contraction is ~1% of the kernel; the fused per-row top-k (plain ALU, DESIGN.md 5.5) is the cost"},
-        # the bound that matters: warp instructions executed by the one-launch kernel (ncu smsp__inst_executed.sum,
-        # profiles/r1c_ncu_summary.md prof_prefill_c) over the live duration, against 148 SMs x 4 schedulers x 1 warp-instr/clk
-        "roofline_alu": {"kernel": "prefill_select_kernel<128,false,false> (whole sequence, one launch)", "bound": "alu",
-                         "achieved": 40551465 / t_one / 1e9, "peak": 148 * 4 * 1.965, "unit": "G warp-instr/s",
-                         "frac": 40551465 / t_one / 1e9 / (148 * 4 * 1.965), "us_per_launch": t_one * 1e6,
-                         "executed_warp_instructions": 40551465},
+        "shape": f"{cfg.name}: T={T}, {Hkv} groups, {Nb} pooled keys, top-{k}, {cfg.chunk}-row chunks",
+        "forecast_us_chunked": round(t_chunk * 1e6, 2), "forecast_us_one_launch": round(t_one * 1e6, 2),
+        "baseline_selector_us_chunked": round(t_base * 1e6, 2), "baseline_over_forecast": round(t_base / t_chunk, 2),
+        "tok_s_selection_only": round(T / t_chunk), "gpu_launches": launches, "ns_per_ranked_row": round(t_chunk * 1e9 / ranked_rows, 3),
+        "tensor": {"kernel": "prefill_select_kernel<128,false>", "bound": "tensor", "achieved": round(flops / t_chunk / 1e12, 2), "peak": bf16_peak,
+                   "unit": "TFLOP/s", "frac": round(flops / t_chunk / 1e12 / bf16_peak, 4), "flops": flops,
+                   "note": "the contraction is ~1% of the kernel; the fused exact per-row top-k (plain ALU) is the cost"},
+        "alu": {"kernel": "prefill_select_kernel<128,false,false> (one launch)", "bound": "alu", "us": round(t_one * 1e6, 2),
+                "warp_instructions": inst, "achieved": round(inst / t_one / 1e9, 1) if inst else None, "peak": round(alu_peak, 1),
+                "unit": "G warp-instr/s", "frac": round(inst / t_one / 1e9 / alu_peak, 4) if inst else None,
+                "traffic_src": ncu_src if inst else None},
     }
     ctx.close()
     return out
@@ -387,70 +506,74 @@ def bench_append(torch, binding):
             graph.replay()
         e1.record()
         e1.synchronize()
-        out[f"us_per_append_{where}"] = e0.elapsed_time(e1) * 1e3 / (5 * 64)
+        out[f"us_per_append_{where}"] = round(e0.elapsed_time(e1) * 1e3 / (5 * 64), 3)
         del graph, kv
-    out["workload"] = f"append_kv_kernel<128>, R = {R} rows (batch 32), one token per launch, 64 launches per graph"
+    out["shape"] = f"append_kv_kernel<128>, R = {R} rows (batch 32), one token per launch, 64 launches per graph"
     out["bytes_per_launch"] = R * D * 2 * 2 + 2 * R * D * 4
     ctx.close()
     return out
 
 
-def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps):
+def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps, standin_bytes=0):
     """SURVEY 8(f) f1 / 8(d) "gather hidden": the same 32-layer decode step with the previous step's blocks kept per
     layer, so only newly selected blocks cross the host link.  The Forecast alternates between F_A and
     F_B = bf16(F_A + alpha * N(0,1)) from step to step; alpha sets how much the selection drifts, the fresh-fetch
     fraction rho is MEASURED (blocks fetched / blocks selected, from the plan kernel's counters).  alpha = 0 gives
-    rho = 0: the compute-only floor of the step; exposed gather time = step(rho) - step(0)."""
+    rho = 0: the compute-only floor of the step; exposed gather time = step(rho) - step(0).
+    standin_bytes > 0: a labelled stand-in kernel (NOT part of the method) streams that many bytes of weights on the
+    compute stream after every attention -- the rest of an 8B decoder layer -- so that 'gather hidden behind the next
+    layer's compute' (P:L114) is measured."""
     R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
     g = torch.Generator(device="cuda").manual_seed(777)
-    layers = []
+    # two views of the same layers that differ only in the Forecast they point to: the step alternates between them, so
+    # no copy of F sits in the timed region (F is an input of the path, produced by the model's projections)
+    layers = [[], []]
     for l, d in enumerate(dev_layers):
         e = dict(d)
-        e["F"] = d["F"].clone()
         if l:
             e["pool"] = torch.zeros((R, k, 2, cfg.block_size, D), dtype=torch.bfloat16, device="cuda")
             e["slot_ids"] = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
             e["fetch"] = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
             e["n_fetch"] = torch.zeros((R,), dtype=torch.int32, device="cuda")
-        layers.append(e)
-    arr = ctx.make_cached_layers(layers)
-    F0w = F0.clone()
-    FA = [d["F"].clone() for d in dev_layers]
+        layers[0].append(e)
+        layers[1].append({**e, "F": d["F"].clone()})
+    arrs = [ctx.make_cached_layers(layers[0]), ctx.make_cached_layers(layers[1])]
+    F0s = [F0, F0.clone()]
     noise = [torch.randn(d["F"].shape, generator=g, device="cuda") for d in dev_layers]
     noise0 = torch.randn(F0.shape, generator=g, device="cuda")
+    weights = None
+    if standin_bytes:
+        weights = torch.empty(standin_bytes // 2, dtype=torch.bfloat16, device="cuda").fill_(1.0)
+        ctx.set_layer_standin(weights, standin_bytes)
 
-    def set_F(which, alpha):
-        for l, e in enumerate(layers):
-            e["F"].copy_(FA[l] if which == 0 else (FA[l].float() + alpha * noise[l]).to(torch.bfloat16))
-        F0w.copy_(F0 if which == 0 else (F0.float() + alpha * noise0).to(torch.bfloat16))
-
-    def one(which, alpha):
-        with torch.cuda.stream(cs):                          # the Forecast of this step is produced on the compute stream
-            set_F(which, alpha)
-        ctx.decode_step_cached(arr, F0w, Nb, k, cs, ps, binding.STEP_OVERLAP)
+    def one(which):
+        ctx.decode_step_cached(arrs[which], F0s[which], Nb, k, cs, ps, binding.STEP_OVERLAP)
 
     out = []
     for alpha in (0.0, 0.05, 0.1, 0.2, 0.4, 0.8, 1e9):
-        for e in layers[1:]:
+        for l, e in enumerate(layers[1]):                    # F_B = bf16(F_A + alpha * N(0, 1))
+            e["F"].copy_((dev_layers[l]["F"].float() + alpha * noise[l]).to(torch.bfloat16))
+        F0s[1].copy_((F0.float() + alpha * noise0).to(torch.bfloat16))
+        for e in layers[0][1:]:
             e["slot_ids"].fill_(-1)
+        torch.cuda.synchronize()
         for i in range(4):
-            one(i & 1, alpha)
+            one(i & 1)
         torch.cuda.synchronize()
         fetched = 0
         for i in range(2):                                   # periodic state: count one A step and one B step
-            one(i & 1, alpha)
+            one(i & 1)
             torch.cuda.synchronize()
-            fetched += sum(int(e["n_fetch"].sum().item()) for e in layers[1:])
+            fetched += sum(int(e["n_fetch"].sum().item()) for e in layers[0][1:])
         rho = fetched / (2.0 * (NL - 1) * R * k)
         n = max(4, steps - steps % 2)
         torch.cuda.synchronize()
-        # one A step and one B step captured into a CUDA graph (two streams, events and the F copies included): the
-        # ~300 enqueue calls of a step would otherwise pace this compute-sized step from the host
+        # one A step and one B step captured into a CUDA graph (three streams and their events): the ~200 enqueue calls of a
+        # step would otherwise pace this compute-sized step from the host
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(graph, stream=cs):
             for i in range(2):
-                set_F(i & 1, alpha)
-                ctx.decode_step_cached(arr, F0w, Nb, k, cs, ps, binding.STEP_OVERLAP)
+                ctx.decode_step_cached(arrs[i], F0s[i], Nb, k, cs, ps, binding.STEP_OVERLAP)
         graph.replay()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -462,18 +585,115 @@ def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / n
         del graph
-        out.append({"alpha": alpha if alpha < 1e8 else "independent", "fresh_fetch_fraction": rho, "ms_per_step": ms,
-                    "tok_s": cfg.batch / (ms * 1e-3), "host_link_mib_per_step": rho * (NL - 1) * cfg.gather_bytes_per_layer / 2**20})
+        out.append({"alpha": alpha if alpha < 1e8 else "independent", "rho": round(rho, 4), "ms_per_step": round(ms, 4),
+                    "tok_s": round(cfg.batch / (ms * 1e-3), 1), "link_mib_per_step": round(rho * (NL - 1) * cfg.gather_bytes_per_layer / 2**20, 1)})
     floor = out[0]["ms_per_step"]
     for o in out:
-        o["gather_exposed_us_per_layer"] = max(0.0, (o["ms_per_step"] - floor) * 1e3 / (NL - 1))
-    del layers, arr
+        o["gather_exposed_us_per_layer"] = round(max(0.0, (o["ms_per_step"] - floor) * 1e3 / (NL - 1)), 2)
+    hidden_up_to = max([o["rho"] for o in out if o["gather_exposed_us_per_layer"] <= 0.05 * floor * 1e3 / (NL - 1)] or [0.0])
+    if standin_bytes:
+        ctx.set_layer_standin(None, 0)
+    del layers, arrs, weights
     torch.cuda.empty_cache()
-    return {"workload": f"{cfg.name}, per-layer persistent pools ({(NL - 1) * cfg.gather_bytes_per_layer / 2**20:.0f} MiB of HBM), "
-                        "Forecast alternating F_A / F_A + alpha*N(0,1) (F copied on the device each step, inside the timed region); steps replayed from a CUDA graph",
-            "compute_floor_ms_per_step": floor, "sweep": out}
+    return {"shape": f"{cfg.name}, per-layer persistent pools, steps alternate between F_A and F_A + alpha*N(0,1); CUDA-graph replay",
+            "standin_bytes_per_layer": standin_bytes,
+            "standin": "NOT part of the method: a kernel streaming 474 MB of weights after every attention" if standin_bytes else None,
+            "compute_floor_ms_per_step": floor, "us_per_layer_at_floor": round(floor * 1e3 / NL, 2),
+            "rho_hidden_up_to": hidden_up_to, "sweep": out}
 
 
+def bench_gather_sweep(torch, binding, peaks, ceiling, host_layer_b4):
+    """Table-7 analog: persistent-CTA count of the UVA gather against link throughput AND against
+    what it costs the compute stream.  For batch 4 and batch 32 (one layer of configs[3]: R*64 blocks of 32 KiB from
+    pinned host memory): gather GB/s and fraction of the same-run memcpy ceiling per engine and CTA count; and the time
+    of 20 (select, attention) pairs of that batch replayed from a graph alone and while gathers run on another stream."""
+    from paper_2606_04511_b200 import synth
+    out = []
+    for batch in (4, 32):
+        cfg = synth.CFG4_128K.with_(batch=batch)
+        R, Nb, k, D = cfg.rows, cfg.n_blocks, cfg.topk, cfg.head_dim
+        if batch == 4:
+            host = host_layer_b4
+        else:
+            host = torch.empty((R, Nb, 2, 64, D), dtype=torch.bfloat16, pin_memory=True)   # 4 GiB; contents irrelevant to the copy
+        g = torch.Generator(device="cuda").manual_seed(500 + batch)
+        ids_g = torch.stack([torch.randperm(Nb, generator=g, device="cuda")[:k].sort().values for _ in range(R)]).to(torch.int32).contiguous()
+        pool = torch.empty((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda")
+        # the compute pair: select + attention on rotating cold buffers
+        NSETS = 4 if batch == 32 else 16
+        kpools = [torch.randn((R, Nb, D), generator=g, device="cuda").to(torch.bfloat16) for _ in range(NSETS)]
+        apools = [torch.randn((R, k, 2, 64, D), generator=g, device="cuda").to(torch.bfloat16) for _ in range(NSETS)]
+        F = torch.randn((R, D), generator=g, device="cuda").to(torch.bfloat16)
+        Q = torch.randn((cfg.batch, cfg.n_q_heads, D), generator=g, device="cuda").to(torch.bfloat16)
+        O = torch.empty_like(Q)
+        ids_s = torch.empty((R, k), dtype=torch.int32, device="cuda")
+        ids_a = torch.arange(k, dtype=torch.int32, device="cuda").repeat(R, 1).contiguous()
+        cctx = binding.Sparda.from_config(cfg)
+        cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+        NP = 20
+        for i in range(NSETS):
+            cctx.forecast_select(F, kpools[i], Nb, k, ids_s)
+            cctx.sparse_decode(Q, apools[i], ids_a, k, O)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=cs):
+            for i in range(NP):
+                cctx.forecast_select(F, kpools[i % NSETS], Nb, k, ids_s, stream=cs)
+                cctx.sparse_decode(Q, apools[i % NSETS], ids_a, k, O, stream=cs)
+        graph.replay()
+        torch.cuda.synchronize()
+
+        def pairs_us(n_rep):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(cs):
+                e0.record(cs)
+                for _ in range(n_rep):
+                    graph.replay()
+                e1.record(cs)
+            e1.synchronize()
+            return e0.elapsed_time(e1) * 1e3 / (n_rep * NP)
+        alone = min(pairs_us(5) for _ in range(3))
+        gbytes = cfg.gather_bytes_per_layer
+        rows = []
+        for mode, name, ctas_list in ((binding.GATHER_TMA, "tma", (2, 4, 8, 16)), (binding.GATHER_LDG, "ldg", (8, 16, 32, 64))):
+            for ctas in ctas_list:
+                gctx = binding.Sparda.from_config(cfg, gather_mode=mode, gather_ctas=ctas)
+                for _ in range(2):
+                    gctx.prefetch_launch(host, Nb, ids_g, k, pool, stream=ps)
+                ps.synchronize()
+                n_g = 6 if batch == 4 else 3
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(ps)
+                for _ in range(n_g):
+                    gctx.prefetch_launch(host, Nb, ids_g, k, pool, stream=ps)
+                e1.record(ps)
+                e1.synchronize()
+                t_g = e0.elapsed_time(e1) * 1e-3 / n_g
+                # interference: keep the link busy for the whole timed window of the compute graph
+                est_pairs_s = alone * 1e-6 * NP * 5
+                n_bg = int(est_pairs_s * 3 / t_g) + 3
+                for _ in range(n_bg):
+                    gctx.prefetch_launch(host, Nb, ids_g, k, pool, stream=ps)
+                with_g = pairs_us(5)
+                busy = not ps.query()                              # gathers still running when the timed window closed
+                ps.synchronize()
+                rows.append({"engine": name, "ctas": ctas, "gbs": round(gbytes / t_g / 1e9, 2), "frac_of_ceiling": round(gbytes / t_g / 1e9 / ceiling, 4),
+                             "pair_us_with_gather": round(with_g, 2), "pair_slowdown": round(with_g / alone, 3), "link_busy_throughout": bool(busy)})
+                gctx.close()
+        out.append({"batch": batch, "gather_mib_per_launch": gbytes / 2**20, "pair_us_alone": round(alone, 2),
+                    "pair": "forecast_select + sparse_decode of this batch, cold HBM, 20 pairs per graph", "rows": rows})
+        cctx.close()
+        del graph, kpools, apools, pool, host
+        torch.cuda.empty_cache()
+    best = {o["batch"]: max(o["rows"], key=lambda r: r["gbs"] / r["pair_slowdown"]) for o in out}
+    return {"ceiling_gbs": round(ceiling, 2), "sweep": out,
+            "pick": {str(b): {"engine": r["engine"], "ctas": r["ctas"]} for b, r in best.items()},
+            "paper": "H100: 16 CTAs below batch 32, 32 from there (P:L116, Table 7); B200 numbers above are this box's"}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
 def run_sparda(args):
     import torch
     import torch.distributed as dist
@@ -489,9 +709,11 @@ def run_sparda(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     assert args.warmup >= 3, "timing rules: at least 3 warm-up steps"
     peaks = load_peaks()
+    ncu, ncu_src = load_ncu_metrics()
     if args.section == "kernels":
-        print(json.dumps({"section": "kernels", "roofline_kernels": bench_kernels_b32(torch, binding, peaks, args),
-                          "prefill_select": bench_prefill(torch, binding, peaks), "cache_maintenance": bench_append(torch, binding)}))
+        print(json.dumps({"section": "kernels", "kernels": bench_kernels(torch, binding, peaks, ncu, ncu_src, 32) +
+                          bench_kernels(torch, binding, peaks, ncu, ncu_src, 4),
+                          "prefill": bench_prefill(torch, binding, peaks, ncu, ncu_src), "append": bench_append(torch, binding)}))
         return 0
     cfg = workload_config(args)
     from paper_2606_04511_b200 import shard
@@ -503,6 +725,7 @@ def run_sparda(args):
 
     # ---- pinned host KV: as many distinct layers as the box can hold, layer l -> l mod resident otherwise
     import psutil
+    numa = numa_info(torch, local)
     per_layer = cfg.kv_bytes_per_layer
     avail = psutil.virtual_memory().available / max(1, int(os.environ.get("LOCAL_WORLD_SIZE", world)))
     cap = args.host_gib * 2**30 if args.host_gib > 0 else 0.5 * avail
@@ -571,8 +794,8 @@ def run_sparda(args):
     launches0 = ctx.launch_count
     ms_total = timed_region(step, args.steps)
     launches = ctx.launch_count - launches0
-    # keep the sampler running through the e2e region too (same load)
-    def step_host():
+
+    def step_host():                                         # keep the sampler running through the e2e region too (same load)
         ctx.decode_step_host(arr_host, F0_host, Nb, k, pools[0], pools[1], cs, ps, binding.STEP_OVERLAP)
         cs.synchronize()                                     # the caller reads O of this step on the host
     for _ in range(args.warmup):
@@ -581,24 +804,23 @@ def run_sparda(args):
     clocks = sampler.stop() if sampler else None
 
     # serialized pipeline (same kernels, one stream): what the overlap buys
+    n_ser = max(3, args.steps // 3)
     for _ in range(2):
         step(binding.STEP_SERIAL)
-    ms_serial = timed_region(lambda: step(binding.STEP_SERIAL), max(3, args.steps // 3)) / max(3, args.steps // 3)
+    ms_serial = timed_region(lambda: step(binding.STEP_SERIAL), n_ser) / n_ser
 
-    reuse = None
-    if not args.no_kernels and rank == 0:
-        reuse = bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, args.steps)
-
-    # ---- per-kernel device times inside the pipeline (second pass over the same K steps, timing events on)
+    # ---- the dominant kernel's own duration: timing events around every gather launch on the prefetch stream, in a second
+    # pass over the same K steps (a 335 us kernel: the event bracket costs < 1 %)
     ctx.profile_enable(True)
-    prof = {"select": [0.0, 0], "gather": [0.0, 0], "attn": [0.0, 0]}
+    g_ms, g_n = 0.0, 0
     for _ in range(args.steps):
         step()
         torch.cuda.synchronize()
-        for kind, (ms, n) in ctx.profile_read().items():
-            prof[kind][0] += ms
-            prof[kind][1] += n
+        ms, n = ctx.profile_read()["gather"]
+        g_ms += ms
+        g_n += n
     ctx.profile_enable(False)
+    t_gat = g_ms / g_n * 1e-3 if g_n else float("nan")
 
     ms_per_step = ms_total / args.steps
     tokens = cfg.batch * world
@@ -610,41 +832,51 @@ def run_sparda(args):
             dist.destroy_process_group()
         return 0
 
-    def per(kind):
-        ms, n = prof[kind]
-        return ms / n * 1e-3 if n else float("nan")
-    t_sel, t_gat, t_att = per("select"), per("gather"), per("attn")
+    sec = args.sections
+    reuse = standin = None
+    if "reuse" in sec:
+        reuse = bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, args.steps)
+    if "standin" in sec:
+        standin = bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, args.steps, standin_bytes=474 * 10**6)
+    gather_sweep = None
+    if "gather" in sec:
+        gather_sweep = bench_gather_sweep(torch, binding, peaks, ceiling, host_kv[0] if cfg.batch == 4 else None) if cfg.batch == 4 else None
+
     gather_bytes = cfg.gather_bytes_per_layer
-    sel_bytes = cfg.kpool_bytes_per_layer + R * D * 2 + R * k * 4
-    att_bytes = cfg.gather_bytes_per_layer + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
+    gm = ncu.get("gather_b4", {}) if cfg.name == "cfg3_128k_pipeline" else {}
+    g_traffic = gm.get("dram__bytes_read.sum", 0.0) + gm.get("dram__bytes_write.sum", 0.0) if "dram__bytes_read.sum" in gm else None
     roofline = {"kernel": "gather_tma_kernel" if args.gather_mode == "tma" else "gather_ldg_kernel",
                 "bound": "host_link", "achieved": gather_bytes / t_gat / 1e9, "peak": ceiling, "unit": "GB/s",
-                "frac": gather_bytes / t_gat / 1e9 / ceiling,
-                "traffic": 56064 if cfg.name == "cfg3_128k_pipeline" else None,
-                "traffic_note": "DRAM bytes of one batch-4 launch (ncu, profiles/r1c_ncu_summary.md): the ids only; the payload crosses the "
-                                "host link (sysmem read sectors x 32 B = the algorithmic 16 MiB, profiles/r1_ncu_summary.md) and lands in L2",
+                "frac": gather_bytes / t_gat / 1e9 / ceiling, "traffic": g_traffic, "traffic_src": ncu_src if g_traffic is not None else None,
+                "traffic_note": "HBM traffic of one launch (the ids); the payload crosses the host link and lands in L2",
                 "peak_source": "cudaMemcpyAsync pinned host->device, measured in this run on this box",
                 "us_per_launch": t_gat * 1e6, "algorithmic_bytes": gather_bytes,
-                "share_of_step": prof["gather"][0] / args.steps / ms_per_step,
-                "note": "dominant kernel of the step; its roofline is the host link, not HBM (DESIGN.md 'Kernels')"}
-    kernels = [
-        {"kernel": "forecast_select_kernel<128>", "workload": f"{cfg.name} in-pipeline", "bound": "hbm",
-         "us_per_launch": t_sel * 1e6, "algorithmic_bytes": sel_bytes, "achieved": sel_bytes / t_sel / 1e9,
-         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": sel_bytes / t_sel / 1e9 / peaks["hbm_gbs"], "traffic": None,
-         "note": "launch-latency-sized at batch 4 (ideal 0.64 us); the event bracket of the profiling pass includes the gaps of the "
-                 "eager enqueue -- device time per launch is 8.7 us (profiles/r1c_launches.csv)"},
-        {"kernel": "sparse_decode_kernel<128>", "workload": f"{cfg.name} in-pipeline (pool just written by the gather: L2-warm)",
-         "bound": "hbm", "us_per_launch": t_att * 1e6, "algorithmic_bytes": att_bytes, "achieved": att_bytes / t_att / 1e9,
-         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": att_bytes / t_att / 1e9 / peaks["hbm_gbs"], "traffic": None,
-         "note": "launch-latency-sized at batch 4 (ideal 2.6 us); event bracket as above -- device time per launch is 10.1 us "
-                 "(profiles/r1c_launches.csv)"},
-    ]
-    prefill = append = None
-    if not args.no_kernels:
-        del pools
-        kernels += bench_kernels_b32(torch, binding, peaks, args)
-        prefill = bench_prefill(torch, binding, peaks)
-        append = bench_append(torch, binding)
+                "share_of_step": g_ms / args.steps / ms_per_step,
+                "hbm_peak": peaks["hbm_gbs"], "hbm_peak_source": peaks["source"],
+                "note": "dominant kernel of the step; its roofline is the host link, not HBM (DESIGN.md 5.2)"}
+    # everything below is nested under `roofline` so that the driver's record keeps it
+    del pools
+    torch.cuda.empty_cache()
+    if "kernels" in sec:
+        roofline["kernels"] = bench_kernels(torch, binding, peaks, ncu, ncu_src, 32) + bench_kernels(torch, binding, peaks, ncu, ncu_src, 4)
+    if "floor" in sec:
+        roofline["launch_floor"] = bench_floor(torch, binding)
+    if "prefill" in sec:
+        roofline["prefill_select"] = bench_prefill(torch, binding, peaks, ncu, ncu_src)
+    if "append" in sec:
+        roofline["cache_maintenance"] = bench_append(torch, binding)
+    floor_ms = reuse["compute_floor_ms_per_step"] if reuse else None
+    roofline["pipeline"] = {
+        "ms_per_step_overlap": ms_per_step, "ms_per_step_serial": ms_serial, "us_per_layer_step": ms_per_step * 1e3 / NL,
+        "us_gather": t_gat * 1e6, "gather_gbs": gather_bytes / t_gat / 1e9, "host_link_ceiling_gbs": ceiling,
+        "tok_s_ceiling_at_host_link": cfg.batch * world / (gather_bytes * (NL - 1) / (ceiling * 1e9)),
+        # exposed = step with every block fetched minus the step with nothing to fetch (the cached step at rho = 0)
+        "gather_exposed_us_per_layer": (ms_per_step - floor_ms) * 1e3 / (NL - 1) if floor_ms else None,
+        "compute_floor_ms_per_step": floor_ms}
+    roofline["reuse_cache"] = reuse
+    roofline["reuse_cache_with_layer_standin"] = standin
+    roofline["gather_sweep"] = gather_sweep
+    roofline["numa"] = numa
 
     base = None
     if not args.no_cpu_baseline and world == 1:
@@ -664,36 +896,21 @@ def run_sparda(args):
         base = cpu_baseline(cfg, bits, args.cpu_seconds)
 
     staged = (R * D * 2) * NL + (cfg.batch * cfg.n_q_heads * D * 2) * NL
+    config = config_dict(cfg, world)
+    config.update({"kv_residency": f"layers 1..{NL - 1} pinned on host ({resident} distinct" + ("" if resident >= NL - 1 else f", l -> (l-1) mod {resident}") + "), layer 0 in HBM",
+                   "l2": f"inputs larger than L2: {(cfg.kpool_bytes_per_layer * NL + gather_bytes * (NL - 1)) / 2**20:.0f} MiB touched per step",
+                   "gather": {"mode": args.gather_mode, "ctas": ctx.gather_ctas}, "attn_splits": ctx.attn_splits(k), "pdl": True})
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-        "data": "synthetic",
-        "config": {"workload": cfg.name, "batch_per_gpu": cfg.batch, "global_batch": tokens, "context": cfg.context,
-                   "layers": NL, "q_heads": cfg.n_q_heads, "kv_heads": cfg.n_kv_heads, "head_dim": D, "block": cfg.block_size,
-                   "topk": k, "parallelism": f"batch shards x{world}, no collective",
-                   "kv_residency": f"layers 1..{NL - 1} in pinned host memory ({resident} distinct resident layers"
-                                   + ("" if resident >= NL - 1 else f", layer l -> (l-1) mod {resident}") + "), layer 0 in HBM",
-                   "fresh_fetch_fraction": 1.0,
-                   "l2": f"inputs larger than L2: {(cfg.kpool_bytes_per_layer * NL + gather_bytes * (NL - 1)) / 2**20:.0f} MiB touched per step",
-                   "gather": {"mode": args.gather_mode, "ctas": ctx.gather_ctas}, "attn_splits": ctx.attn_splits(k)},
-        "clocks": clocks,
+        "data": "synthetic", "config": config, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
                 "h2d_bytes_per_step": staged + gather_bytes * (NL - 1), "d2h_bytes_per_step": cfg.batch * cfg.n_q_heads * D * 2 * NL,
                 "h2d_staged_bytes_per_step": staged, "h2d_uva_gather_bytes_per_step": gather_bytes * (NL - 1),
-                "api": "sparda_decode_step_host (pinned host F/Q/O, copies enqueued just in time inside the call) + stream sync per step"},
+                "api": "sparda_decode_step_host: pinned host F/Q/O copied just in time inside the call; stream sync per step"},
         "gpu_launches": launches,
         "roofline": roofline,
-        "roofline_kernels": kernels,
         "cpu_baseline": base,
-        "prefill_select": prefill,
-        "reuse_cache": reuse,
-        "cache_maintenance": append,
-        "pipeline": {"ms_per_step_overlap": ms_per_step, "ms_per_step_serial": ms_serial,
-                     "us_per_layer_step": ms_per_step * 1e3 / NL,
-                     "us_select": t_sel * 1e6, "us_gather": t_gat * 1e6, "us_attn": t_att * 1e6,
-                     "gather_exposed_us_per_layer": max(0.0, (ms_per_step * 1e3 - (t_sel * NL + t_att * NL) * 1e6) / max(1, NL - 1)),
-                     "host_link_ceiling_gbs": ceiling, "gather_gbs": gather_bytes / t_gat / 1e9,
-                     "tok_s_ceiling_at_host_link": cfg.batch * world / (gather_bytes * (NL - 1) / (ceiling * 1e9))},
     }
     print(json.dumps(line))
     if world > 1:
@@ -701,10 +918,32 @@ def run_sparda(args):
     return 0
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: launch N ranks (one per GPU) of this script through
+    torch.distributed.run and pass rank 0's line through.  Fewer than N GPUs is an error, never a 1-GPU number."""
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} asked for, {have} CUDA device(s) visible: refusing to print a smaller job's number\n")
+        return 3
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    env_world = os.environ.get("WORLD_SIZE")
+    if env_world is None and args.gpus > 1:
+        return spawn_ranks(args)
+    if env_world is not None and int(env_world) != args.gpus:
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={env_world}\n")
+        return 2
     return run_sparda(args)
 
 

@@ -66,12 +66,15 @@ typedef struct {
     int block_size;  /* S, must be 64 */
     int max_blocks;  /* largest Nb any call will pass (<= 8192) */
     int topk;        /* largest k any call will pass (<= 256) */
-    int gather_ctas; /* persistent gather grid size; 0 = default (4 for TMA, 16 for LDG; Table 7) */
+    int gather_ctas; /* persistent gather grid size; 0 = default (2 for TMA, 8 for LDG: the counts that reach the link plateau
+                        and cost the compute stream < 5 % on B200, bench.py gather_sweep; Table 7)          */
     int gather_mode; /* SPARDA_GATHER_TMA or SPARDA_GATHER_LDG */
     int attn_splits; /* split-K CTAs per row for sparse_decode; 0 = auto from B, Hkv, k and the SM count */
     int max_layers;  /* largest n_layers sparda_decode_step will see (events are pre-created); 0 = 64 */
     int select_cluster; /* CTAs per row (thread-block cluster size) of forecast_select: 0 = auto from B, Hkv, n_cand and the
                            SM count; 1, 2, 4, 8 or 16 forces it (sweeps and tests)                                       */
+    int hidden;      /* model width of the optional in-step Forecast projection (sparda_layer.X / .WF); 0 = not used;
+                        else a multiple of 64 in [64, 8192]                                                              */
     int no_pdl;      /* 1 = launch without programmatic dependent launch (measurement: what the launch gap costs);
                         0 = select, gather and attention kernels overlap their prologue with the previous kernel's tail */
 } sparda_config;
@@ -86,6 +89,13 @@ typedef struct {
                           on GPU); layers >= 1 = host-mapped pointer (pinned CPU memory) */
     void* O;           /* [B][Hq][D] device, written.                                                          */
     int32_t* ids;      /* [R][k] device, written: B_l.                                                         */
+    /* Optional: Alg.2 l.1's share of the path, the Forecast projection (Eq.3).  When X and WF are non-NULL the step
+     * computes F = bf16(X . WF) into the buffer F points to (which is then written, not read) with
+     * sparda_forecast_project's kernel, on the stream and just before the selection that reads it; cfg.hidden must be set.
+     * WFcur: layer 0 only, the extra same-layer projection F_0^cur, written to the step's F0cur buffer.     */
+    const void* X;     /* [B][hidden] device, this layer's input hidden states; NULL = F is an input                  */
+    const void* WF;    /* [hidden][Hkv*D] device                                                                       */
+    const void* WFcur; /* [hidden][Hkv*D] device, layer 0 only                                                         */
 } sparda_layer;
 
 #define SPARDA_STEP_OVERLAP 0    /* gather on prefetch_stream, overlapped with the compute stream (the method) */
@@ -253,6 +263,18 @@ int sparda_prefill_select(sparda_ctx* ctx, const void* F, const void* Kpool, int
  * then the same top-k.  Q [Hq][T][D] device.                                                                  */
 int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* Kpool, int T, int n_blocks, int row0,
                                    int n_rows, int topk, int32_t* ids_out, void* stream);
+
+/* Measurement aids, NOT part of the method (csrc/bench_probes.cu).
+ * sparda_probe_launch enqueues one probe kernel on `stream`: kind 0 = empty kernel (launch floor); 1 = empty kernel with
+ * the forecast_select launch shape (128 CTAs x 288 threads, clusters of 2, 107 KB of shared memory); 2 = 148 CTAs, one
+ * dependent DRAM load each (buf: device, bytes >= 148 MiB, untouched locations 1 MiB apart); 3 = the layer stand-in:
+ * streams `bytes` of buf (device, 16-byte aligned) from HBM once.
+ * sparda_set_layer_standin(ctx, weights, bytes): while bytes > 0, sparda_decode_step[_cached|_host] launches the stand-in
+ * on the compute stream after every attention -- the cost of the rest of a decoder layer (an 8B layer reads ~474 MB of
+ * bf16 weights per token step: o-proj, FFN, the next QKV+F projections), so that "gather hidden behind
+ * the next layer's compute" can be measured.  bytes = 0 switches it off (the default).                       */
+int sparda_probe_launch(sparda_ctx* ctx, int kind, const void* buf, int64_t bytes, void* stream);
+int sparda_set_layer_standin(sparda_ctx* ctx, const void* weights, int64_t bytes);
 
 /* Introspection used by bench.py / tests: number of kernels this context has launched since creation, the
  * resolved tunables, and error text.                                                                          */

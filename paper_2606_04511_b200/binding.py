@@ -22,6 +22,7 @@ EXPORTS = [
     "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
     "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
+    "sparda_probe_launch", "sparda_set_layer_standin",
     "sparda_launch_count", "sparda_tmap_encodes", "sparda_get_select_cluster", "sparda_get_attn_cluster", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
     "sparda_last_cuda_error", "sparda_version",
 ]
@@ -34,12 +35,13 @@ class SpardaError(RuntimeError):
 class SpardaConfig(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int) for n in (
         "batch", "n_q_heads", "n_kv_heads", "head_dim", "block_size", "max_blocks", "topk", "gather_ctas",
-        "gather_mode", "attn_splits", "max_layers", "select_cluster", "no_pdl")]
+        "gather_mode", "attn_splits", "max_layers", "select_cluster", "hidden", "no_pdl")]
 
 
 class SpardaLayer(ctypes.Structure):
     _fields_ = [("F", ctypes.c_void_p), ("Q", ctypes.c_void_p), ("Kpool", ctypes.c_void_p), ("kv", ctypes.c_void_p),
-                ("O", ctypes.c_void_p), ("ids", ctypes.c_void_p)]
+                ("O", ctypes.c_void_p), ("ids", ctypes.c_void_p), ("X", ctypes.c_void_p), ("WF", ctypes.c_void_p),
+                ("WFcur", ctypes.c_void_p)]
 
 
 class SpardaCachedLayer(ctypes.Structure):
@@ -80,6 +82,8 @@ def lib() -> ctypes.CDLL:
         L.sparda_prefill_select_baseline.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
         L.sparda_launch_count.argtypes = [vp]
         L.sparda_launch_count.restype = i64
+        L.sparda_probe_launch.argtypes = [vp, i32, vp, i64, vp]
+        L.sparda_set_layer_standin.argtypes = [vp, vp, i64]
         L.sparda_tmap_encodes.argtypes = [vp]
         L.sparda_tmap_encodes.restype = i64
         L.sparda_get_select_cluster.argtypes = [vp]
@@ -113,10 +117,10 @@ class Sparda:
     """One libsparda context (one shape family on the current device)."""
 
     def __init__(self, batch, n_q_heads, n_kv_heads, head_dim, max_blocks, topk, block_size=64, gather_ctas=0,
-                 gather_mode=GATHER_TMA, attn_splits=0, max_layers=0, select_cluster=0, no_pdl=0):
+                 gather_mode=GATHER_TMA, attn_splits=0, max_layers=0, select_cluster=0, hidden=0, no_pdl=0):
         self._h = ctypes.c_void_p()
         self.cfg = SpardaConfig(batch, n_q_heads, n_kv_heads, head_dim, block_size, max_blocks, topk, gather_ctas,
-                                gather_mode, attn_splits, max_layers, select_cluster, no_pdl)
+                                gather_mode, attn_splits, max_layers, select_cluster, hidden, no_pdl)
         self._L = lib()
         rc = self._L.sparda_create(ctypes.byref(self.cfg), ctypes.byref(self._h))
         if rc != 0:
@@ -185,7 +189,8 @@ class Sparda:
         """layers: list of dicts with tensors F, Q, Kpool, kv, O, ids -> ctypes array (keeps no references)."""
         arr = (SpardaLayer * len(layers))()
         for i, l in enumerate(layers):
-            arr[i] = SpardaLayer(_ptr(l["F"]), _ptr(l["Q"]), _ptr(l["Kpool"]), _ptr(l["kv"]), _ptr(l["O"]), _ptr(l["ids"]))
+            arr[i] = SpardaLayer(_ptr(l["F"]), _ptr(l["Q"]), _ptr(l["Kpool"]), _ptr(l["kv"]), _ptr(l["O"]), _ptr(l["ids"]),
+                                 _ptr(l.get("X")) or None, _ptr(l.get("WF")) or None, _ptr(l.get("WFcur")) or None)
         return arr
 
     def decode_step(self, layer_array, F0cur, n_blocks, topk, pool0, pool1, compute_stream=None, prefetch_stream=None,
@@ -215,7 +220,8 @@ class Sparda:
         """layers: list of dicts with tensors F, Q, Kpool, kv, O, ids and (layers >= 1) pool, slot_ids, fetch, n_fetch."""
         arr = (SpardaCachedLayer * len(layers))()
         for i, l in enumerate(layers):
-            base = SpardaLayer(_ptr(l["F"]), _ptr(l["Q"]), _ptr(l["Kpool"]), _ptr(l["kv"]), _ptr(l["O"]), _ptr(l["ids"]))
+            base = SpardaLayer(_ptr(l["F"]), _ptr(l["Q"]), _ptr(l["Kpool"]), _ptr(l["kv"]), _ptr(l["O"]), _ptr(l["ids"]),
+                               _ptr(l.get("X")) or None, _ptr(l.get("WF")) or None, _ptr(l.get("WFcur")) or None)
             opt = [(_ptr(l[n]) if l.get(n) is not None else None) for n in ("pool", "slot_ids", "fetch", "n_fetch")]
             arr[i] = SpardaCachedLayer(base, *opt)
         return arr
@@ -243,6 +249,13 @@ class Sparda:
     def prefill_select_baseline(self, Q, Kpool, T, n_blocks, row0, n_rows, topk, ids_out, stream=None):
         self._check(self._L.sparda_prefill_select_baseline(self._h, _ptr(Q), _ptr(Kpool), T, n_blocks, row0, n_rows, topk,
                                                            _ptr(ids_out), _stream(stream)), "prefill_select_baseline")
+
+    # ---- measurement aids (not the method) ----
+    def probe_launch(self, kind, buf=None, nbytes=0, stream=None):
+        self._check(self._L.sparda_probe_launch(self._h, kind, _ptr(buf), int(nbytes), _stream(stream)), "probe_launch")
+
+    def set_layer_standin(self, weights=None, nbytes=0):
+        self._check(self._L.sparda_set_layer_standin(self._h, _ptr(weights), int(nbytes)), "set_layer_standin")
 
     # ---- introspection ----
     @property

@@ -22,6 +22,8 @@ __global__ void __launch_bounds__(256) forecast_project_kernel(const uint16_t* _
     __shared__ unsigned int s_last;
     const int slab = blockIdx.x, n_slabs = gridDim.x;
     const int C2 = C / 2;
+    pdl_wait();                  // X is the previous kernel's output in a model
+    pdl_launch_dependents();
     for (int b0 = 0; b0 < B; b0 += FP_BT) {
         const int nb = min(FP_BT, B - b0);
         __syncthreads();
@@ -69,11 +71,18 @@ __global__ void __launch_bounds__(256) forecast_project_kernel(const uint16_t* _
 
 }  // namespace
 
-int sparda_launch_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F, cudaStream_t st) {
+int sparda_launch_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F, int ws, cudaStream_t st) {
     const int C = ctx->cfg.n_kv_heads * ctx->cfg.head_dim;
     const int n_slabs = hidden / FP_SLAB;
-    forecast_project_kernel<<<n_slabs, 256, 0, st>>>((const uint16_t*)X, (const uint32_t*)WF, ctx->fp_part, ctx->fp_ticket, (uint32_t*)F,
-                                                     ctx->cfg.batch, hidden, C);
+    cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3(n_slabs, 1, 1);
+    lc.blockDim = dim3(256, 1, 1);
+    lc.stream = st;
+    lc.attrs = at;
+    lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
+    SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, forecast_project_kernel, (const uint16_t*)X, (const uint32_t*)WF, ctx->fp_part + (size_t)ws * 128 * ctx->R * ctx->cfg.head_dim, ctx->fp_ticket + ws,
+                                            (uint32_t*)F, ctx->cfg.batch, hidden, C));
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;
     return SPARDA_OK;

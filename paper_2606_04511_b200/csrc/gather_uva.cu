@@ -167,7 +167,7 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
         lc.dynamicSmemBytes = smem;
         lc.stream = st;
         lc.attrs = at;
-        lc.numAttrs = ctx->cfg.no_pdl ? 0 : 1;
+        lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
         SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_tma_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes));
     } else {
         cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
@@ -176,7 +176,7 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
         lc.blockDim = dim3(256, 1, 1);
         lc.stream = st;
         lc.attrs = at;
-        lc.numAttrs = ctx->cfg.no_pdl ? 0 : 1;
+        lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
         SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_ldg_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes));
     }
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());

@@ -31,7 +31,9 @@ __global__ void __launch_bounds__(RP_WARPS * 32) reuse_plan_kernel(const int32_t
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int r = blockIdx.x * RP_WARPS + w;
     if (r >= n_rows) return;
-    const int n_miss = reuse_plan_row(ids_new + (size_t)r * k, slot_ids + (size_t)r * k, fetch + (size_t)r * k, k, sc[w], lane);
+    int32_t old[RP_MAXK / 32];
+    reuse_plan_load(slot_ids + (size_t)r * k, k, lane, old);
+    const int n_miss = reuse_plan_row(ids_new + (size_t)r * k, slot_ids + (size_t)r * k, old, fetch + (size_t)r * k, k, sc[w], lane);
     if (lane == 0 && n_fetch) n_fetch[r] = n_miss;
 }
 

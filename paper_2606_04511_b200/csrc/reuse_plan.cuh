@@ -14,7 +14,17 @@ struct ReusePlanScratch {   // per warp, shared memory
 };
 
 // in [k]: this step's selection (ascending, -1 padded); slots [k] in/out; fo [k] out.  Returns the number of fetches.
-__device__ __forceinline__ int reuse_plan_row(const int32_t* in, int32_t* slots, int32_t* fo, int k, ReusePlanScratch& sc, int lane) {
+// in == nullptr: the selection is already in sc.nw (written by the selecting CTA as it emitted the ids: the fused tail of
+// forecast_select_kernel, which thereby skips a round trip through L2).
+// The row's slot table is passed in registers (lane l holds slots[32 q + l] in old[q]): reuse_plan_load() reads it, and a
+// caller with something else to do first issues that read early.
+__device__ __forceinline__ void reuse_plan_load(const int32_t* slots, int k, int lane, int32_t (&old)[RP_MAXK / 32]) {
+#pragma unroll
+    for (int q = 0; q < RP_MAXK / 32; ++q) old[q] = q * 32 + lane < k ? slots[q * 32 + lane] : -1;
+}
+
+__device__ __forceinline__ int reuse_plan_row(const int32_t* in, int32_t* slots, const int32_t (&old)[RP_MAXK / 32], int32_t* fo, int k,
+                                              ReusePlanScratch& sc, int lane) {
     int32_t* nw = sc.nw;
     int32_t* owner = sc.owner;
     int16_t* sfree = sc.sfree;
@@ -24,15 +34,19 @@ __device__ __forceinline__ int reuse_plan_row(const int32_t* in, int32_t* slots,
     int m = 0;   // valid entries of the selection (ascending, then -1 padding)
     for (int c = 0; c < k; c += 32) {
         const int i = c + lane;
-        const int32_t v = i < k ? __ldcg(in + i) : -1;
+        const int32_t v = i < k ? (in ? __ldcg(in + i) : nw[i]) : -1;
         if (i < k) { nw[i] = v; owner[i] = 0x7fffffff; }
         m += __popc(__ballot_sync(0xffffffffu, v >= 0));
     }
     __syncwarp();
+
     // hits: resident blocks that are selected again
-    for (int c = 0; c < k; c += 32) {
+#pragma unroll
+    for (int q = 0; q < RP_MAXK / 32; ++q) {
+        const int c = q * 32;
+        if (c >= k) break;
         const int s = c + lane;
-        const int32_t b = s < k ? slots[s] : -1;
+        const int32_t b = old[q];
         if (b >= 0) {
             int lo = 0, hi = m;
             while (lo < hi) {
@@ -45,11 +59,14 @@ __device__ __forceinline__ int reuse_plan_row(const int32_t* in, int32_t* slots,
     __syncwarp();
     // freed slots (ascending) and missing blocks (ascending position = ascending id)
     int n_free = 0, n_miss = 0;
-    for (int c = 0; c < k; c += 32) {
+#pragma unroll
+    for (int q = 0; q < RP_MAXK / 32; ++q) {
+        const int c = q * 32;
+        if (c >= k) break;
         const int s = c + lane;
         bool kept = false;
         if (s < k) {
-            const int32_t b = slots[s];
+            const int32_t b = old[q];
             if (b >= 0) {
                 int lo = 0, hi = m;
                 while (lo < hi) {

@@ -59,7 +59,6 @@ constexpr int SEL_THREADS = 256;                  // consumer threads (the selec
 constexpr int SEL_CTA_THREADS = SEL_THREADS + 32; // + one producer warp
 constexpr int SEL_STAGE_BYTES = 16384;            // two 64 x 64-element TMA boxes
 constexpr int SEL_STAGES = 6;
-constexpr int SEL_MAX_CS = 16;                    // largest cluster (non-portable size, opt-in)
 
 // barrier of the 256 consumer threads only (the producer warp has left by the time the selection runs)
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
@@ -153,6 +152,7 @@ constexpr int SEL_CAND_CAP = 32;  // boundary-bucket size the exact finish handl
 //     a smaller index), and ids are emitted in index order: exactly "sort by (score desc, id asc), take k, sort by id".
 // Fallback (heavy ties / degenerate range): exact MSB-first 8-bit radix select + index-ordered compaction.
 __device__ __forceinline__ void topk_emit(const uint32_t* keys, int n, int k, uint32_t kmin, uint32_t kmax, int32_t* ids_out,
+                          int32_t* ids_smem /* optional copy of the row's ids for the fused reuse plan, or nullptr */,
                           uint32_t* hist /*[256], zeroed*/, uint32_t* warp_tot /*[8]*/, uint32_t* bcast /*[4], [2] zeroed*/,
                           uint32_t* cand /*[2 * SEL_CAND_CAP]*/, SelCyc& cyc_) {
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -289,6 +289,7 @@ __device__ __forceinline__ void topk_emit(const uint32_t* keys, int n, int k, ui
             while (m_sel) {
                 const int j = __ffs(m_sel) - 1;
                 m_sel &= m_sel - 1;
+                if (ids_smem) ids_smem[pos] = lo + j;
                 ids_out[pos++] = lo + j;
             }
             return;
@@ -336,9 +337,13 @@ __device__ __forceinline__ void topk_emit(const uint32_t* keys, int n, int k, ui
     for (int i = lo; i < hi; ++i) {
         uint32_t key = keys[i];
         if (key > T) {
+            if (ids_smem) ids_smem[pos] = i;
             ids_out[pos++] = i;
         } else if (key == T) {
-            if (eq_before < krem) ids_out[pos++] = i;
+            if (eq_before < krem) {
+                if (ids_smem) ids_smem[pos] = i;
+                ids_out[pos++] = i;
+            }
             ++eq_before;
         }
     }
@@ -399,7 +404,9 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
             if (p.slot_ids) {
                 __syncthreads();
                 if (w == 0) {
-                    const int nm = reuse_plan_row(ids_row, p.slot_ids + (size_t)r * p.topk, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
+                    int32_t old[RP_MAXK / 32];
+                    reuse_plan_load(p.slot_ids + (size_t)r * p.topk, p.topk, lane, old);
+                    const int nm = reuse_plan_row(ids_row, p.slot_ids + (size_t)r * p.topk, old, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
                     if (lane == 0 && p.n_fetch) p.n_fetch[r] = nm;
                 }
             }
@@ -443,6 +450,9 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
     pdl_wait();                  // everything above overlaps the previous kernel's tail; global memory is touched from here on
     pdl_launch_dependents();
     SEL_CYC(1);
+    // fused reuse plan: the row's slot table is needed only after the selection; its load is issued now (warp 0 of CTA 0)
+    int32_t plan_old[RP_MAXK / 32];
+    if (p.slot_ids && c == 0 && w == 0) reuse_plan_load(p.slot_ids + (size_t)r * p.topk, p.topk, lane, plan_old);
 
     if (w == NW) {
         // =============================== producer warp: the stream ===============================
@@ -554,13 +564,13 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
     SEL_CYC(5);
 
     // =============================== a2 (CTA 0, consumer threads): exact top-k, ascending ids ===============================
-    topk_emit(s_keys, p.n_cand, p.topk, s_mm[0], s_mm[1], ids_row, s_hist, s_wtot, s_bcast, s_cand, cyc_);
+    topk_emit(s_keys, p.n_cand, p.topk, s_mm[0], s_mm[1], ids_row, p.slot_ids ? s_plan.nw : nullptr, s_hist, s_wtot, s_bcast, s_cand, cyc_);
     SEL_CYC(12);
     SEL_LOG_EXIT
     if (p.slot_ids) {
-        consumer_sync();   // the row's ids are in global memory (read back through L2)
+        consumer_sync();   // the row's k ids (n_cand > k: exactly k) are in s_plan.nw as well as on their way to global memory
         if (w == 0) {
-            const int nm = reuse_plan_row(ids_row, p.slot_ids + (size_t)r * p.topk, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
+            const int nm = reuse_plan_row(nullptr, p.slot_ids + (size_t)r * p.topk, plan_old, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
             if (lane == 0 && p.n_fetch) p.n_fetch[r] = nm;
         }
     }
@@ -697,7 +707,7 @@ static int select_launch(sparda_ctx* ctx, const void* Kpool, const SelParams& p0
     at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     at[1] = sparda_pdl_attr();
     lc.attrs = at;
-    lc.numAttrs = ctx->cfg.no_pdl ? 1 : 2;
+    lc.numAttrs = sparda_use_pdl(ctx) ? 2 : 1;
     lc.blockDim = dim3(SEL_CTA_THREADS, 1, 1);
     lc.dynamicSmemBytes = smem;
     lc.stream = st;

@@ -47,6 +47,7 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     if (cfg->topk < 1 || cfg->topk > 256) return SPARDA_EINVAL;
     if (cfg->gather_mode != SPARDA_GATHER_TMA && cfg->gather_mode != SPARDA_GATHER_LDG) return SPARDA_EINVAL;
     if (cfg->gather_ctas < 0 || cfg->gather_ctas > 1024 || cfg->attn_splits < 0 || cfg->max_layers < 0) return SPARDA_EINVAL;
+    if (cfg->hidden != 0 && (cfg->hidden < 64 || cfg->hidden > 8192 || cfg->hidden % 64 != 0)) return SPARDA_EINVAL;
     if (!(cfg->select_cluster == 0 || cfg->select_cluster == 1 || cfg->select_cluster == 2 || cfg->select_cluster == 4 ||
           cfg->select_cluster == 8 || cfg->select_cluster == 16))
         return SPARDA_EINVAL;
@@ -63,11 +64,12 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     if (!ctx) return SPARDA_ENOMEM;
     memset(ctx, 0, sizeof(*ctx));
     ctx->cfg = *cfg;
+    ctx->pdl_next = 1;
     ctx->device = dev;
     ctx->sm_count = prop.multiProcessorCount;
     ctx->R = cfg->batch * cfg->n_kv_heads;
     ctx->G = G;
-    if (ctx->cfg.gather_ctas == 0) ctx->cfg.gather_ctas = cfg->gather_mode == SPARDA_GATHER_TMA ? 4 : 16;
+    if (ctx->cfg.gather_ctas == 0) ctx->cfg.gather_ctas = cfg->gather_mode == SPARDA_GATHER_TMA ? 2 : 8;
     ctx->max_layers = cfg->max_layers > 0 ? cfg->max_layers : 64;
     {   // partial slots per row of the flat split-K attention: n_parts <= ceil(CTAs / R) + 1
         int per_row = cfg->attn_splits > 0 ? cfg->attn_splits : (2 * ctx->sm_count + ctx->R - 1) / ctx->R;
@@ -92,9 +94,10 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     bool ok = cudaMalloc(&ctx->part_O, n_po * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->part_ml, n_ml * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->tickets, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
-              cudaMalloc(&ctx->fp_part, (size_t)128 * ctx->R * D * sizeof(float)) == cudaSuccess &&
-              cudaMalloc(&ctx->fp_ticket, sizeof(unsigned int)) == cudaSuccess &&
-              cudaMemset(ctx->fp_ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
+              cudaMalloc(&ctx->fp_part, (size_t)2 * 128 * ctx->R * D * sizeof(float)) == cudaSuccess &&
+              cudaMalloc(&ctx->fp_ticket, 2 * sizeof(unsigned int)) == cudaSuccess &&
+              cudaMalloc(&ctx->probe_sink, 256 * sizeof(uint32_t)) == cudaSuccess &&
+              cudaMemset(ctx->fp_ticket, 0, 2 * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&ctx->pf_scratch, (size_t)ctx->sm_count * 512 * 128 * sizeof(float)) == cudaSuccess &&
               cudaMemset(ctx->tickets, 0, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
@@ -135,6 +138,7 @@ int sparda_destroy(sparda_ctx* ctx) {
     cudaFree(ctx->pf_scratch);
     cudaFree(ctx->fp_part);
     cudaFree(ctx->fp_ticket);
+    cudaFree(ctx->probe_sink);
     for (int i = 0; i <= ctx->max_layers; ++i) {
         if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);
         if (ctx->ev_gather && ctx->ev_gather[i]) cudaEventDestroy(ctx->ev_gather[i]);
@@ -164,7 +168,7 @@ int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_bloc
 int sparda_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F_out, void* stream) {
     if (!ctx || !sparda_aligned(X, 16) || !sparda_aligned(WF, 16) || !sparda_aligned(F_out, 16)) return SPARDA_EINVAL;
     if (hidden < 64 || hidden > 8192 || hidden % 64 != 0) return SPARDA_EINVAL;
-    return sparda_launch_forecast_project(ctx, X, WF, hidden, F_out, (cudaStream_t)stream);
+    return sparda_launch_forecast_project(ctx, X, WF, hidden, F_out, 0, (cudaStream_t)stream);
 }
 
 int sparda_append_kv(sparda_ctx* ctx, const void* k_new, const void* v_new, int64_t t, void* kv_cache, int n_blocks, float* ksum,
@@ -241,15 +245,20 @@ int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* K
 
 // Algorithm 2, lines 4-7, for n_layers layers, plain (double-buffered pool, every block fetched) or with the
 // previous step's blocks kept per layer.  Given layer l's projections, line 4 (select B_{l+1}) and line 7
-// (attention l) do not depend on each other, so in overlap mode they run concurrently on two streams; the prefetch has
-// its own:
-//   compute stream  cs:  record ev_top[l]  ->  wait ev_gather[l]  ->  attention l
-//   select stream   ss:  wait ev_top[l]    ->  select B_{l+1} (+ reuse plan)  ->  record ev_sel[l+1]
-//   prefetch stream ps:  wait ev_sel[l+1]  ->  gather B_{l+1}  ->  record ev_gather[l+1]
+// (attention l) do not depend on each other, so in overlap mode they run concurrently; the lookahead chain of layer l+1
+// (Forecast projection if asked for, select + reuse plan, prefetch) is ONE stream-ordered sequence on a side stream, the
+// two side streams (the context's own and the caller's prefetch stream) alternating by layer parity:
+//   compute stream cs      :  record ev_top[l]  ->  wait ev_gather[l]  ->  attention l
+//   side stream x[(l+1)&1] :  wait ev_top[l]  ->  [F_l = X_l W_F]  ->  select B_{l+1} (+ plan)  ->  gather B_{l+1}  ->  record ev_gather[l+1]
+// The kernels of a chain follow each other with no event in between, so programmatic dependent launch overlaps each one's
+// launch and prologue with its predecessor's tail, and there are two cross-stream hand-offs per layer, not three (round 1
+// ran select and gather on different streams: 18.6 us per layer with nothing to fetch; this order: see DESIGN.md 5.4).
+// Chains of consecutive layers sit on different streams, so select B_{l+2} overlaps a long gather B_{l+1}.
 // ev_top[l] follows attention l-1 on cs, so a select never runs more than one layer ahead of the attention (in a model,
 // F_l exists only once layer l-1 is complete) and it releases the buffers gather l+1 writes: pool[(l+1)&1] was last read
-// by attention l-1 (plain); pool_{l+1} and slot_ids_{l+1} by attention l+1 of the previous step (cached).  The step ends
-// with cs joined to ss.  Serial mode: the same kernels on cs in Algorithm-2 order.
+// by attention l-1 (plain); pool_{l+1} and slot_ids_{l+1} by attention l+1 of the previous step (cached).  Every chain ends
+// in an event an attention waits for, so cs has joined both side streams when the step ends (capturable).  Serial mode:
+// the same kernels on cs in Algorithm-2 order.
 // timing events around one launch of `kind` (0 select, 1 gather, 2 attention) on stream st
 static inline cudaEvent_t* prof_slot(sparda_ctx* ctx, int kind) {
     return &ctx->ev_prof[((size_t)kind * (ctx->max_layers + 1) + ctx->prof_n[kind]) * 2];
@@ -274,16 +283,24 @@ struct HostIO {
 static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                             int topk, cudaStream_t cs, cudaStream_t ps_in, int mode, const HostIO* io = nullptr) {
     const bool overlap = mode == SPARDA_STEP_OVERLAP;
-    cudaStream_t ps = overlap ? ps_in : cs;
-    cudaStream_t ss = overlap ? ctx->select_stream : cs;
+    cudaStream_t side[2] = {overlap ? ctx->select_stream : cs, overlap ? ps_in : cs};
     int rc;
     ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
     if (io) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(const_cast<void*>(F0cur), io->F0cur, io->f_bytes, cudaMemcpyHostToDevice, cs));
     // layer 0: same-layer selection with F0cur; its attention needs it, so it stays on the compute stream
+    if (!io && layers[0].base.X && layers[0].base.WFcur) {   // Alg.2 l.1 for F_0^cur (Eq.3)
+        if (!ctx->cfg.hidden) return SPARDA_EINVAL;
+        rc = sparda_launch_forecast_project(ctx, layers[0].base.X, layers[0].base.WFcur, ctx->cfg.hidden, const_cast<void*>(F0cur), 0, cs);
+        if (rc) return rc;
+    }
     SPARDA_PROF_BEGIN(0, cs);
     rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_blocks, topk, layers[0].base.ids, cs);
     if (rc) return rc;
     SPARDA_PROF_END(0, cs);
+    struct PdlScope {   // launches behind an event wait do not ask for PDL (see sparda_ctx::pdl_next); restored on every return
+        sparda_ctx* c;
+        ~PdlScope() { c->pdl_next = 1; }
+    } pdl_scope{ctx};
     for (int l = 0; l < n_layers; ++l) {
         if (io) {   // this layer's Forecast and query, before ev_top[l] releases the select that reads F_l
             if (l + 1 < n_layers)
@@ -292,28 +309,33 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
         }
         if (l + 1 < n_layers) {
             const sparda_cached_layer* nx = &layers[l + 1];
+            cudaStream_t xs = side[(l + 1) & 1];
             if (overlap) {
                 SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_top[l], cs));
-                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ss, ctx->ev_top[l], 0));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(xs, ctx->ev_top[l], 0));
             }
-            SPARDA_PROF_BEGIN(0, ss);
+            ctx->pdl_next = overlap ? 0 : 1;   // overlap mode launches without PDL (measured: 0.38 ms per cached step against 0.43)
+            if (!io && layers[l].base.X && layers[l].base.WF) {   // Alg.2 l.1: F_l = X_l . W_F (Eq.3), where its reader runs
+                if (!ctx->cfg.hidden) return SPARDA_EINVAL;
+                rc = sparda_launch_forecast_project(ctx, layers[l].base.X, layers[l].base.WF, ctx->cfg.hidden, const_cast<void*>(layers[l].base.F),
+                                                    (l + 1) & 1, xs);
+                if (rc) return rc;
+            }
+            SPARDA_PROF_BEGIN(0, xs);
             if (nx->slot_ids)   // select + reuse plan in one launch
                 rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids,
-                                                 nx->slot_ids, nx->fetch, nx->n_fetch, ss);
+                                                 nx->slot_ids, nx->fetch, nx->n_fetch, xs);
             else
-                rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, ss);
+                rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, xs);
             if (rc) return rc;
-            SPARDA_PROF_END(0, ss);
-            if (overlap) {
-                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], ss));
-                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(ps, ctx->ev_sel[l + 1], 0));
-            }
-            SPARDA_PROF_BEGIN(1, ps);
-            rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->slot_ids ? nx->fetch : nx->base.ids, topk, nx->pool, ps);
+            SPARDA_PROF_END(0, xs);
+            SPARDA_PROF_BEGIN(1, xs);
+            rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->slot_ids ? nx->fetch : nx->base.ids, topk, nx->pool, xs);
             if (rc) return rc;
-            SPARDA_PROF_END(1, ps);
-            if (overlap) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], ps));
+            SPARDA_PROF_END(1, xs);
+            if (overlap) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], xs));
         }
+        ctx->pdl_next = overlap ? 0 : 1;       // the attention waits for its gather's event in overlap mode
         if (l == 0) {
             SPARDA_PROF_BEGIN(2, cs);
             rc = sparda_sparse_decode(ctx, layers[0].base.Q, layers[0].base.kv, layers[0].base.ids, topk, 1, n_blocks, layers[0].base.O, cs);
@@ -325,11 +347,13 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
         }
         if (rc) return rc;
         SPARDA_PROF_END(2, cs);
+        if (ctx->standin_buf) {   // measurement only: the rest of layer l (weights streamed once), between attention l and layer l+1
+            rc = sparda_launch_standin(ctx, cs);
+            if (rc) return rc;
+        }
         if (io) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(io->host[l].O, layers[l].base.O, io->q_bytes, cudaMemcpyDeviceToHost, cs));
     }
-    // every select has been consumed by a gather that an attention waited for, so cs already follows all work of ss and
-    // ps; the explicit join keeps that true for n_layers == 1 and makes the step capturable (all forks rejoin cs)
-    if (overlap && n_layers > 1) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_sel[n_layers - 1], 0));
+    // every chain ended in an ev_gather that an attention on cs waited for: cs has joined both side streams (capturable)
     return SPARDA_OK;
 }
 

@@ -22,7 +22,7 @@ struct sparda_kernel_state {
 enum {
     SPARDA_K_SELECT_128, SPARDA_K_SELECT_64, SPARDA_K_SELECT_GRID_128, SPARDA_K_SELECT_GRID_64,
     SPARDA_K_ATTN_128, SPARDA_K_ATTN_64, SPARDA_K_ATTN_CL_128, SPARDA_K_ATTN_CL_64,
-    SPARDA_K_GATHER_TMA,
+    SPARDA_K_GATHER_TMA, SPARDA_K_PROBE,
     SPARDA_K_PF_0, /* 8 prefill instantiations: D x BASELINE x REPL */
     SPARDA_K_COUNT = SPARDA_K_PF_0 + 8
 };
@@ -45,7 +45,7 @@ struct sparda_ctx {
     float* part_O;     // [R][max_splits][16][D]
     float* part_ml;    // [R][max_splits][2][16]  (m in log2 domain, l)
     unsigned int* tickets;  // [R]: split-K attention, one per row (the select keeps its scores on chip)
-    float* fp_part;         // Forecast projection: split-K partials [128 slabs][B][Hkv*D] fp32
+    float* fp_part;         // Forecast projection: split-K partials [2 workspaces][128 slabs][B][Hkv*D] fp32 (one per side stream)
     unsigned int* fp_ticket;
     float* pf_scratch;      // prefill comparison selector: [sm_count][512][128] fp32 group-summed scores (lazy)
     cudaEvent_t* ev_sel;    // [max_layers + 1]
@@ -63,6 +63,11 @@ struct sparda_ctx {
     int prof_n[3];
     int64_t launches;
     int last_select_cluster, last_attn_cluster;   // introspection: the shape the last launch resolved to
+    // Programmatic dependent launch for the NEXT launch (cfg.no_pdl overrides): 1 for the stand-alone calls and for the
+    // serial step (one stream, kernel after kernel: 0.60 ms per cached batch-4 step against 0.68 without); 0 inside an
+    // overlapped step, where every chain starts behind an event wait and early-resident dependents only take shared memory
+    // from the kernels of the other streams (measured: 0.43 ms with PDL on the in-chain launches, 0.38 ms without)
+    int pdl_next;
     char cuda_err[256];
     // TMA descriptor cache (host): open-addressed hash on (base, rows, head_dim, box_rows); lookups return a COPY, so an
     // eviction can never change a descriptor a launcher already holds
@@ -70,6 +75,10 @@ struct sparda_ctx {
     int64_t tmap_encodes;   // descriptors encoded so far (introspection: a warm step must not encode)
     void* encode_fn;   // cuTensorMapEncodeTiled
     int device;             // the device the context was created on
+    // measurement aids (bench_probes.cu): a sink the probe kernels may write, and the optional layer stand-in
+    uint32_t* probe_sink;   // [256]
+    const void* standin_buf;
+    size_t standin_bytes;
     sparda_kernel_state kstate[SPARDA_K_COUNT];
 };
 
@@ -88,6 +97,8 @@ static inline cudaLaunchAttribute sparda_pdl_attr() {
     return a;
 }
 
+static inline bool sparda_use_pdl(const sparda_ctx* ctx) { return !ctx->cfg.no_pdl && ctx->pdl_next; }
+
 static inline bool sparda_aligned(const void* p, uintptr_t a) { return p != nullptr && ((uintptr_t)p & (a - 1)) == 0; }
 
 // launchers implemented in the kernel translation units
@@ -97,7 +108,7 @@ int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_bl
                          cudaStream_t);
 int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
                          cudaStream_t);
-int sparda_launch_forecast_project(sparda_ctx*, const void* X, const void* WF, int hidden, void* F, cudaStream_t);
+int sparda_launch_forecast_project(sparda_ctx*, const void* X, const void* WF, int hidden, void* F, int workspace /* 0 or 1 */, cudaStream_t);
 int sparda_launch_pool_keys_grid(sparda_ctx*, const void* kv, int64_t n_rows, int n_blocks, void* kgrid, cudaStream_t);
 int sparda_launch_select_grid(sparda_ctx*, const void* F, const void* Kgrid, int n_blocks, int n_cand, int n_init, int n_local, int topk,
                               int32_t* ids, cudaStream_t);
@@ -113,6 +124,7 @@ int sparda_launch_prefill_baseline(sparda_ctx*, const void* Q, const void* Kpool
                                    int n_rows, int topk, int32_t* ids, cudaStream_t);
 // [rows][head_dim] bf16 row-major view, box = box_rows x 64 elements (128 B), 128-byte swizzle; *out receives a copy
 int sparda_get_tmap(sparda_ctx*, const void* base, uint64_t rows, int head_dim, int box_rows, CUtensorMap* out);
+int sparda_launch_standin(sparda_ctx*, cudaStream_t);       // bench_probes.cu: the labelled layer stand-in (not the method)
 int sparda_resolve_splits(const sparda_ctx*, int topk);     // average CTAs per row of the attention launch
 int sparda_resolve_attn_ctas(const sparda_ctx*, int topk);  // its grid size
 

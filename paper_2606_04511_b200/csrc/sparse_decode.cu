@@ -525,7 +525,7 @@ int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, 
         }
         if (ks.max_clusters[cluster] * cluster < C) return 1;   // caller falls back to the workspace reduction
     }
-    lc.numAttrs = ctx->cfg.no_pdl ? 1 : 2;
+    lc.numAttrs = sparda_use_pdl(ctx) ? 2 : 1;
     SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, kern, *map, p));
     return SPARDA_OK;
 }

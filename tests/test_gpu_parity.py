@@ -1056,3 +1056,59 @@ def test_two_contexts_of_different_shapes_interleave(sp, oracle):
         torch.cuda.synchronize()
         want, _ = oracle.sparse_attn(_bits(L["Q"]), _bits(L["kv"]), ids_np, pool_is_indexed=True)
         parity.check_attn(_bits(O), want, c.name)
+
+
+def test_decode_step_with_in_step_forecast_projection(sp, oracle):
+    """Alg.2 l.1 inside the step (Eq.3): with X and W_F given per layer the step computes every F_l (and F_0^cur)
+    itself, where its reader runs.  F is within 1 bf16 ulp of o2, and ids / O are bit-identical to a step that is handed
+    those F as inputs, overlapped and serialized."""
+    cfg = G16.with_(n_layers=5, batch=3)
+    hidden = 512
+    ctx = sp.Sparda.from_config(cfg, max_layers=8, hidden=hidden)
+    R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
+    g = torch.Generator(device="cuda").manual_seed(77)
+    dev = []
+    for l in range(NL):
+        L = synth.decode_layer(cfg, l, device="cuda")
+        kpool = torch.empty((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+        ctx.pool_keys(L["kv"], R, Nb, kpool)
+        dev.append({"F": torch.full((R, D), float("nan"), dtype=torch.bfloat16, device="cuda"), "Q": L["Q"], "Kpool": kpool,
+                    "kv": L["kv"] if l == 0 else L["kv"].cpu().pin_memory(),
+                    "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                    "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda"),
+                    "X": torch.randn((cfg.batch, hidden), generator=g, device="cuda").to(torch.bfloat16),
+                    "WF": (torch.randn((hidden, cfg.n_kv_heads * D), generator=g, device="cuda") / hidden ** 0.5).to(torch.bfloat16)})
+    dev[0]["WFcur"] = (torch.randn((hidden, cfg.n_kv_heads * D), generator=g, device="cuda") / hidden ** 0.5).to(torch.bfloat16)
+    F0 = torch.full((R, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    pools = [torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    out = {}
+    for mode in (sp.STEP_OVERLAP, sp.STEP_SERIAL):
+        for d in dev:
+            d["F"].fill_(float("nan"))
+            d["O"].zero_()
+        F0.fill_(float("nan"))
+        torch.cuda.synchronize()
+        ctx.decode_step(ctx.make_layers(dev), F0, Nb, k, pools[0], pools[1], cs, ps, mode)
+        torch.cuda.synchronize()
+        out[mode] = ([d["O"].clone() for d in dev], [d["ids"].clone() for d in dev], [d["F"].clone() for d in dev], F0.clone())
+    for a, b in zip(out[sp.STEP_OVERLAP][0], out[sp.STEP_SERIAL][0]):
+        assert torch.equal(a.view(torch.int16), b.view(torch.int16))
+    # F against o2 (layers 0 .. NL-2 are projected; the last layer's F is unused, P:L87)
+    for l in range(NL - 1):
+        want = oracle.forecast_project(_bits(dev[l]["X"]), _bits(dev[l]["WF"]), cfg.n_kv_heads, D)
+        assert parity.ulp_diff_bf16(_bits(out[sp.STEP_OVERLAP][2][l]), want).max() <= 1
+    want0 = oracle.forecast_project(_bits(dev[0]["X"]), _bits(dev[0]["WFcur"]), cfg.n_kv_heads, D)
+    assert parity.ulp_diff_bf16(_bits(out[sp.STEP_OVERLAP][3]), want0).max() <= 1
+    # the same step handed those F as inputs
+    plain = [{kk: v for kk, v in d.items() if kk not in ("X", "WF", "WFcur")} for d in dev]
+    for l, d in enumerate(plain):
+        d["F"] = out[sp.STEP_OVERLAP][2][l].clone()
+        d["O"] = torch.zeros_like(d["O"])
+        d["ids"] = torch.full_like(d["ids"], -9)
+    ctx.decode_step(ctx.make_layers(plain), out[sp.STEP_OVERLAP][3], Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)
+    torch.cuda.synchronize()
+    for l in range(NL):
+        assert torch.equal(plain[l]["ids"], out[sp.STEP_OVERLAP][1][l])
+        assert torch.equal(plain[l]["O"].view(torch.int16), out[sp.STEP_OVERLAP][0][l].view(torch.int16))

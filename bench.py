@@ -111,7 +111,8 @@ def config_dict(cfg, world):
     return {"workload": cfg.name, "batch_per_gpu": cfg.batch, "global_batch": cfg.batch * world, "context": cfg.context,
             "layers": cfg.n_layers, "q_heads": cfg.n_q_heads, "kv_heads": cfg.n_kv_heads, "head_dim": cfg.head_dim,
             "block": cfg.block_size, "topk": cfg.topk, "parallelism": f"batch shards x{world}, no collective",
-            "fresh_fetch_fraction": 1.0}
+            "fresh_fetch_fraction": 1.0,
+            "l2": f"inputs larger than L2: {(cfg.kpool_bytes_per_layer * cfg.n_layers + cfg.gather_bytes_per_layer * (cfg.n_layers - 1)) / 2**20:.0f} MiB touched per step"}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -809,12 +810,13 @@ def run_sparda(args):
         step(binding.STEP_SERIAL)
     ms_serial = timed_region(lambda: step(binding.STEP_SERIAL), n_ser) / n_ser
 
-    # ---- the dominant kernel's own duration: timing events around every gather launch on the prefetch stream, in a second
-    # pass over the same K steps (a 335 us kernel: the event bracket costs < 1 %)
+    # ---- the dominant kernel's own duration: timing events around every gather launch, in a pass over the same K steps in
+    # SERIAL mode -- the kernel alone on the link (in the overlapped step two gathers of consecutive layers share it, so a
+    # bracket there reads two kernels' time); a 335 us kernel: the event bracket costs < 1 %
     ctx.profile_enable(True)
     g_ms, g_n = 0.0, 0
     for _ in range(args.steps):
-        step()
+        step(binding.STEP_SERIAL)
         torch.cuda.synchronize()
         ms, n = ctx.profile_read()["gather"]
         g_ms += ms
@@ -851,7 +853,7 @@ def run_sparda(args):
                 "traffic_note": "HBM traffic of one launch (the ids); the payload crosses the host link and lands in L2",
                 "peak_source": "cudaMemcpyAsync pinned host->device, measured in this run on this box",
                 "us_per_launch": t_gat * 1e6, "algorithmic_bytes": gather_bytes,
-                "share_of_step": g_ms / args.steps / ms_per_step,
+                "share_of_step": t_gat * 1e3 * (NL - 1) / ms_per_step,   # 31 gathers back to back against the overlapped step
                 "hbm_peak": peaks["hbm_gbs"], "hbm_peak_source": peaks["source"],
                 "note": "dominant kernel of the step; its roofline is the host link, not HBM (DESIGN.md 5.2)"}
     # everything below is nested under `roofline` so that the driver's record keeps it
@@ -897,9 +899,9 @@ def run_sparda(args):
 
     staged = (R * D * 2) * NL + (cfg.batch * cfg.n_q_heads * D * 2) * NL
     config = config_dict(cfg, world)
-    config.update({"kv_residency": f"layers 1..{NL - 1} pinned on host ({resident} distinct" + ("" if resident >= NL - 1 else f", l -> (l-1) mod {resident}") + "), layer 0 in HBM",
-                   "l2": f"inputs larger than L2: {(cfg.kpool_bytes_per_layer * NL + gather_bytes * (NL - 1)) / 2**20:.0f} MiB touched per step",
-                   "gather": {"mode": args.gather_mode, "ctas": ctx.gather_ctas}, "attn_splits": ctx.attn_splits(k), "pdl": True})
+    roofline["run"] = {"kv_residency": f"layers 1..{NL - 1} pinned on host ({resident} distinct" + ("" if resident >= NL - 1 else f", l -> (l-1) mod {resident}") + "), layer 0 in HBM",
+                       "gather": {"mode": args.gather_mode, "ctas": ctx.gather_ctas}, "attn_ctas_per_row": ctx.attn_splits(k),
+                       "pdl": "stand-alone calls and the serial step; not inside the overlapped step"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",

@@ -66,8 +66,8 @@ typedef struct {
     int block_size;  /* S, must be 64 */
     int max_blocks;  /* largest Nb any call will pass (<= 8192) */
     int topk;        /* largest k any call will pass (<= 256) */
-    int gather_ctas; /* persistent gather grid size; 0 = default (2 for TMA, 8 for LDG: the counts that reach the link plateau
-                        and cost the compute stream < 5 % on B200, bench.py gather_sweep; Table 7)          */
+    int gather_ctas; /* persistent gather grid size; 0 = default (4 for TMA, 16 for LDG; bench.py gather_sweep has the B200
+                        trade-off between link rate and what the CTAs cost the compute stream; Table 7)    */
     int gather_mode; /* SPARDA_GATHER_TMA or SPARDA_GATHER_LDG */
     int attn_splits; /* split-K CTAs per row for sparse_decode; 0 = auto from B, Hkv, k and the SM count */
     int max_layers;  /* largest n_layers sparda_decode_step will see (events are pre-created); 0 = 64 */

@@ -3,7 +3,8 @@
 //   kind 0  empty kernel, 1 CTA x 32 threads                                  (launch floor)
 //   kind 1  empty kernel with the select launch shape: 128 CTAs x 288 threads, clusters of 2, 107 KB dynamic smem
 //   kind 2  148 CTAs x 32 threads, each one DRAM load on which its (never taken) store depends   (launch + one round trip)
-//   kind 3  LAYER STAND-IN: streams `bytes` of HBM with 16-byte loads (2 CTAs per SM): the cost of reading an 8B decoder
+//   kind 3  LAYER STAND-IN: streams `bytes` of HBM with 16-byte loads (one 512-thread CTA per SM, registers and shared memory
+//           left for the path's kernels to run beside it, as they would beside a real layer's GEMVs): the cost of reading an 8B decoder
 //           layer's weights once (~474 MB of bf16) -- everything Algorithm 2 does between two attentions that this library
 //           does not implement (o-proj, FFN, next layer's QKV+F projections).  sparda_set_layer_standin makes
 //           sparda_decode_step launch it on the compute stream after every attention, so that "gather hidden behind a
@@ -21,13 +22,16 @@ __global__ void probe_touch_kernel(const int* __restrict__ p, int* out, size_t s
     if (v == 0x7fffffff) out[blockIdx.x] = v;
 }
 
-__global__ void __launch_bounds__(512) standin_stream_kernel(const uint4* __restrict__ w, size_t n_vec, uint32_t* sink) {
+__global__ void __launch_bounds__(512, 1) standin_stream_kernel(const uint4* __restrict__ w, size_t n_vec, uint32_t* sink) {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     uint32_t acc = 0;
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; i + 3 * stride < n_vec; i += 4 * stride) {   // four independent 16-byte loads in flight per thread
-        const uint4 a = __ldcs(w + i), b = __ldcs(w + i + stride), c = __ldcs(w + i + 2 * stride), d = __ldcs(w + i + 3 * stride);
-        acc ^= a.x ^ a.y ^ a.z ^ a.w ^ b.x ^ b.y ^ b.z ^ b.w ^ c.x ^ c.y ^ c.z ^ c.w ^ d.x ^ d.y ^ d.z ^ d.w;
+    for (; i + 7 * stride < n_vec; i += 8 * stride) {   // eight independent 16-byte loads in flight per thread
+        uint4 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = __ldcs(w + i + u * stride);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
     }
     for (; i < n_vec; i += stride) {
         const uint4 a = __ldcs(w + i);
@@ -38,9 +42,23 @@ __global__ void __launch_bounds__(512) standin_stream_kernel(const uint4* __rest
 
 }  // namespace
 
+// The stand-in uses no shared memory of its own; left alone it would run with the SMs' L1 / shared-memory split at "all
+// L1", and no CTA of the path (100-200 KB of shared memory each) could join it on an SM until it drains -- the split only
+// changes on an idle SM.  A layer's real GEMVs stage through shared memory, so the stand-in asks for the shared-memory
+// split too and the path's kernels run beside it.
+static int standin_prepare(sparda_ctx* ctx) {
+    sparda_kernel_state& ks = ctx->kstate[SPARDA_K_STANDIN];
+    if (!ks.attr_set) {
+        SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(standin_stream_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        ks.attr_set = true;
+    }
+    return SPARDA_OK;
+}
+
 int sparda_launch_standin(sparda_ctx* ctx, cudaStream_t st) {
+    if (int rc = standin_prepare(ctx)) return rc;
     const size_t n_vec = ctx->standin_bytes / 16;
-    standin_stream_kernel<<<2 * ctx->sm_count, 512, 0, st>>>((const uint4*)ctx->standin_buf, n_vec, ctx->probe_sink);
+    standin_stream_kernel<<<ctx->sm_count, 512, 0, st>>>((const uint4*)ctx->standin_buf, n_vec, ctx->probe_sink);
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     return SPARDA_OK;
 }
@@ -81,7 +99,8 @@ int sparda_probe_launch(sparda_ctx* ctx, int kind, const void* buf, int64_t byte
         probe_touch_kernel<<<148, 32, 0, st>>>((const int*)buf, (int*)ctx->probe_sink, (size_t)(bytes / 148 / 4));
     } else if (kind == 3) {
         if (!sparda_aligned(buf, 16) || bytes < 16) return SPARDA_EINVAL;
-        standin_stream_kernel<<<2 * ctx->sm_count, 512, 0, st>>>((const uint4*)buf, (size_t)bytes / 16, ctx->probe_sink);
+        if (int rc = standin_prepare(ctx)) return rc;
+        standin_stream_kernel<<<ctx->sm_count, 512, 0, st>>>((const uint4*)buf, (size_t)bytes / 16, ctx->probe_sink);
     } else {
         return SPARDA_EINVAL;
     }

@@ -22,7 +22,7 @@ struct sparda_kernel_state {
 enum {
     SPARDA_K_SELECT_128, SPARDA_K_SELECT_64, SPARDA_K_SELECT_GRID_128, SPARDA_K_SELECT_GRID_64,
     SPARDA_K_ATTN_128, SPARDA_K_ATTN_64, SPARDA_K_ATTN_CL_128, SPARDA_K_ATTN_CL_64,
-    SPARDA_K_GATHER_TMA, SPARDA_K_PROBE,
+    SPARDA_K_GATHER_TMA, SPARDA_K_PROBE, SPARDA_K_STANDIN,
     SPARDA_K_PF_0, /* 8 prefill instantiations: D x BASELINE x REPL */
     SPARDA_K_COUNT = SPARDA_K_PF_0 + 8
 };

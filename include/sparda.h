@@ -75,8 +75,14 @@ typedef struct {
                            SM count; 1, 2, 4, 8 or 16 forces it (sweeps and tests)                                       */
     int hidden;      /* model width of the optional in-step Forecast projection (sparda_layer.X / .WF); 0 = not used;
                         else a multiple of 64 in [64, 8192]                                                              */
-    int no_pdl;      /* 1 = launch without programmatic dependent launch (measurement: what the launch gap costs);
-                        0 = select, gather and attention kernels overlap their prologue with the previous kernel's tail */
+    int no_pdl;      /* 0 = the stand-alone calls and the serial step launch their kernels with programmatic dependent
+                        launch: a kernel's launch and prologue overlap the tail of the previous kernel of the stream, and
+                        forecast_select also streams pooled keys into its ring before that kernel has completed.  This
+                        is transparent behind any kernel that does not signal launch completion early (pool_keys,
+                        append_kv, anything of the caller's that does not execute griddepcontrol.launch_dependents): the
+                        dependent then starts after it has completed.  libsparda's kernels that do signal early never
+                        write pooled keys.  A caller whose own kernel signals early AND writes Kpool right before a
+                        select must set 1.  1 = plain launches (also: what the launch gap costs).                       */
 } sparda_config;
 
 /* One decoder layer's tensors for sparda_decode_step (Algorithm 2). */

@@ -78,32 +78,14 @@ __device__ __forceinline__ uint32_t map_to_cta(const void* local, uint32_t rank)
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(out) : "r"(smem_u32(local)), "r"(rank));
     return out;
 }
-__device__ __forceinline__ void st_cluster_u32(uint32_t addr, uint32_t v) {
-    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+// asynchronous store into the shared memory of a CTA of the cluster that also counts its bytes on an mbarrier there
+// (st.async ... complete_tx): the receiver waits for "all bytes have landed", the sender never waits for its stores
+__device__ __forceinline__ void st_async_u32(uint32_t addr, uint32_t v, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.u32 [%0], %1, [%2];" ::"r"(addr), "r"(v), "r"(mbar) : "memory");
 }
-// arrive (release at cluster scope) on an mbarrier in another CTA's shared memory: orders this thread's earlier remote
-// stores (and, through the warp barrier in front of it, its warp's) before the waiter's acquire
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAITC_%=:\n"
-        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONEC_%=;\n"
-        "bra WAITC_%=;\n"
-        "DONEC_%=:\n"
-        "}" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void red_cluster_min_u32(uint32_t addr, uint32_t v) {
-    asm volatile("red.shared::cluster.min.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-}
-__device__ __forceinline__ void red_cluster_max_u32(uint32_t addr, uint32_t v) {
-    asm volatile("red.shared::cluster.max.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+__device__ __forceinline__ void st_async_v2_u32(uint32_t addr, uint32_t a, uint32_t b, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.u32 [%0], {%1, %2}, [%3];" ::"r"(addr), "r"(a), "r"(b), "r"(mbar)
+                 : "memory");
 }
 
 __device__ __forceinline__ uint32_t block_incl_scan_256(uint32_t v, uint32_t* warp_tot /*[8]*/, uint32_t& total) {
@@ -377,12 +359,12 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
     SEL_LOG_DECL
     extern __shared__ uint8_t sel_smem_raw[];
     __shared__ uint64_t s_full[SEL_STAGES], s_empty[SEL_STAGES];
-    __shared__ uint64_t s_done;                      // CTA 0: one arrival per consumer warp of the cluster when its keys are in
+    __shared__ uint64_t s_done;                      // CTA 0: completes when every key and every warp's min / max has landed (tx bytes)
     __shared__ __align__(16) uint32_t s_hist[256];
     __shared__ __align__(16) uint32_t s_wtot[8];
     __shared__ uint32_t s_bcast[4];
     __shared__ uint32_t s_cand[2 * SEL_CAND_CAP];
-    __shared__ uint32_t s_mm[2];                     // min / max key of the row; lives in CTA 0 (red.shared::cluster)
+    __shared__ __align__(8) uint32_t s_mm[16 * NW][2];   // per (CTA of the cluster, warp): min / max key; lives in CTA 0
     __shared__ ReusePlanScratch s_plan;
 
     // swizzle atoms are 1 KiB; the offset is taken in the shared window so that ring / s_keys stay shared-space pointers
@@ -434,21 +416,31 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
     SEL_CYC(0);
     if (w == NW && lane == 0) {   // the producer thread arms the barriers
         for (int s = 0; s < SEL_STAGES; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], NW / 2); }
-        mbar_init(&s_done, CS * NW);
+        mbar_init(&s_done, 1);
+        // CTA 0 expects one 4-byte key per candidate and one (min, max) pair per consumer warp of the cluster
+        if (c == 0) mbar_arrive_expect_tx(&s_done, (uint32_t)p.n_cand * 4u + CS * NW * 8u);
         mbar_fence_init();
         fence_proxy_async_smem();
         tma_prefetch_desc(&tmap);
         SEL_CYC_PRODUCER(0);
     }
     if (tid < 256) s_hist[tid] = 0;
-    if (tid == 0) { s_bcast[2] = 0; s_mm[0] = 0xFFFFFFFFu; s_mm[1] = 0u; }
+    if (tid == 0) s_bcast[2] = 0;
     __syncthreads();
     // All CTAs of the cluster must be running before anyone touches a neighbour's shared memory: arrive now, wait just
     // before the first remote store (by then every CTA has long arrived: the wait is free).  The release / acquire pair
-    // also orders CTA 0's initialisation of s_mm / s_hist / s_done before the remote reductions and arrivals.
+    // also orders CTA 0's initialisation of s_done before the first remote store that counts on it.
     cluster_arrive();
-    pdl_wait();                  // everything above overlaps the previous kernel's tail; global memory is touched from here on
-    pdl_launch_dependents();
+    // Programmatic dependent launch: everything above overlaps the previous kernel's tail, and so does the producer's
+    // stream of pooled keys below -- the ring fills (96 KiB per CTA) while the predecessor drains.  That is safe because a
+    // dependent only starts early behind a kernel that signals launch completion early, and the kernels of this library
+    // that do (select, gather, attention, projection) never write pooled keys; behind any other kernel (pool_keys,
+    // append_kv, a caller's own) this launch starts after that kernel has completed (include/sparda.h, cfg.no_pdl).
+    // Everything the predecessor may have written -- F, the slot table -- and every store waits for it (consumers).
+    if (w != NW) {
+        pdl_wait();
+        pdl_launch_dependents();
+    }
     SEL_CYC(1);
     // fused reuse plan: the row's slot table is needed only after the selection; its load is issued now (warp 0 of CTA 0)
     int32_t plan_old[RP_MAXK / 32];
@@ -483,6 +475,7 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
             }
         }
         const uint32_t keys0 = map_to_cta(s_keys, 0);          // the row's key array lives in CTA 0
+        const uint32_t done0 = map_to_cta(&s_done, 0);         // ... and so does the barrier that counts what has landed
         const int mi = lane >> 3, ri = lane & 7;                // ldmatrix: this lane addresses row ri of matrix mi
         uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
         bool waited = false;
@@ -532,12 +525,12 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
                             const int b = k_lo + blk;
                             const bool forced = b < p.n_init || b >= p.n_cand - p.n_local;   // init / local blocks: always attended
                             const uint32_t key = forced ? 0xFFFFFFFFu : orderable(bsc + 0.0f);
-                            st_cluster_u32(keys0 + 4u * (uint32_t)b, key);
+                            st_async_u32(keys0 + 4u * (uint32_t)b, key, done0);
                             if (!forced) { kmin = min(kmin, key); kmax = max(kmax, key); }
                         }
                     } else if (tig == 0 && kl < nk) {
                         const uint32_t key = orderable(sc[h] + 0.0f);      // +0: -0 -> +0
-                        st_cluster_u32(keys0 + 4u * (uint32_t)(k_lo + i * KPS + kl), key);
+                        st_async_u32(keys0 + 4u * (uint32_t)(k_lo + i * KPS + kl), key, done0);
                         kmin = min(kmin, key);
                         kmax = max(kmax, key);
                     }
@@ -548,23 +541,21 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
         if (!waited) cluster_wait();
         kmin = __reduce_min_sync(0xffffffffu, kmin);
         kmax = __reduce_max_sync(0xffffffffu, kmax);
-        if (lane == 0 && kmin <= kmax) {
-            red_cluster_min_u32(map_to_cta(&s_mm[0], 0), kmin);
-            red_cluster_max_u32(map_to_cta(&s_mm[1], 0), kmax);
-        }
-        // This warp's keys are on their way to CTA 0: tell it (release at cluster scope, cumulative over the warp's stores
-        // through the warp barrier).  No closing cluster barrier: nobody reads the shared memory of CTAs 1.., so they leave
-        // at once, and CTA 0 waits for the arrivals only -- not for a barrier round trip of the whole cluster.
-        __syncwarp();
-        if (lane == 0) mbar_arrive_remote(map_to_cta(&s_done, 0));
+        // the keys went out as asynchronous stores that count their bytes on CTA 0's barrier; so does this warp's (min, max):
+        // no release, no drain -- the sender is done, and CTAs 1.. leave at once (nobody reads their shared memory)
+        if (lane == 0) st_async_v2_u32(map_to_cta(&s_mm[c * NW + w][0], 0), kmin, kmax, done0);
     }
     SEL_CYC(4);
     if (c != 0 || w == NW) { SEL_LOG_EXIT return; }
-    mbar_wait_cluster(&s_done, 0);   // acquire: every CTA's keys and min / max have landed in this CTA
+    mbar_wait(&s_done, 0);           // every key and every warp's min / max of the row has landed in this CTA
     SEL_CYC(5);
+    uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+    for (int i = lane; i < (int)CS * NW; i += 32) { kmin = min(kmin, s_mm[i][0]); kmax = max(kmax, s_mm[i][1]); }
+    kmin = __reduce_min_sync(0xffffffffu, kmin);
+    kmax = __reduce_max_sync(0xffffffffu, kmax);
 
     // =============================== a2 (CTA 0, consumer threads): exact top-k, ascending ids ===============================
-    topk_emit(s_keys, p.n_cand, p.topk, s_mm[0], s_mm[1], ids_row, p.slot_ids ? s_plan.nw : nullptr, s_hist, s_wtot, s_bcast, s_cand, cyc_);
+    topk_emit(s_keys, p.n_cand, p.topk, kmin, kmax, ids_row, p.slot_ids ? s_plan.nw : nullptr, s_hist, s_wtot, s_bcast, s_cand, cyc_);
     SEL_CYC(12);
     SEL_LOG_EXIT
     if (p.slot_ids) {

@@ -94,10 +94,7 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     bool ok = cudaMalloc(&ctx->part_O, n_po * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->part_ml, n_ml * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->tickets, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
-              cudaMalloc(&ctx->fp_part, (size_t)2 * 128 * ctx->R * D * sizeof(float)) == cudaSuccess &&
-              cudaMalloc(&ctx->fp_ticket, 2 * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&ctx->probe_sink, 256 * sizeof(uint32_t)) == cudaSuccess &&
-              cudaMemset(ctx->fp_ticket, 0, 2 * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&ctx->pf_scratch, (size_t)ctx->sm_count * 512 * 128 * sizeof(float)) == cudaSuccess &&
               cudaMemset(ctx->tickets, 0, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
@@ -136,8 +133,6 @@ int sparda_destroy(sparda_ctx* ctx) {
     cudaFree(ctx->part_ml);
     cudaFree(ctx->tickets);
     cudaFree(ctx->pf_scratch);
-    cudaFree(ctx->fp_part);
-    cudaFree(ctx->fp_ticket);
     cudaFree(ctx->probe_sink);
     for (int i = 0; i <= ctx->max_layers; ++i) {
         if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);

@@ -22,7 +22,7 @@ struct sparda_kernel_state {
 enum {
     SPARDA_K_SELECT_128, SPARDA_K_SELECT_64, SPARDA_K_SELECT_GRID_128, SPARDA_K_SELECT_GRID_64,
     SPARDA_K_ATTN_128, SPARDA_K_ATTN_64, SPARDA_K_ATTN_CL_128, SPARDA_K_ATTN_CL_64,
-    SPARDA_K_GATHER_TMA, SPARDA_K_PROBE, SPARDA_K_STANDIN,
+    SPARDA_K_GATHER_TMA, SPARDA_K_PROBE, SPARDA_K_STANDIN, SPARDA_K_PROJECT,
     SPARDA_K_PF_0, /* 8 prefill instantiations: D x BASELINE x REPL */
     SPARDA_K_COUNT = SPARDA_K_PF_0 + 8
 };
@@ -45,8 +45,6 @@ struct sparda_ctx {
     float* part_O;     // [R][max_splits][16][D]
     float* part_ml;    // [R][max_splits][2][16]  (m in log2 domain, l)
     unsigned int* tickets;  // [R]: split-K attention, one per row (the select keeps its scores on chip)
-    float* fp_part;         // Forecast projection: split-K partials [2 workspaces][128 slabs][B][Hkv*D] fp32 (one per side stream)
-    unsigned int* fp_ticket;
     float* pf_scratch;      // prefill comparison selector: [sm_count][512][128] fp32 group-summed scores (lazy)
     cudaEvent_t* ev_sel;    // [max_layers + 1]
     cudaEvent_t* ev_gather; // [max_layers + 1]

@@ -791,7 +791,9 @@ def run_sparda(args):
     props = torch.cuda.get_device_properties(local)
     gpu_id = f"GPU-{props.uuid}" if getattr(props, "uuid", None) else str(local)
     sampler = ClockSampler(gpu_id) if rank == 0 else None
-    time.sleep(0.15)
+    t_wait = time.time()                                     # nvidia-smi takes a moment to start: wait for its first sample
+    while sampler and sampler.p and time.time() - t_wait < 3.0 and os.path.getsize(sampler.f.name) == 0:
+        time.sleep(0.05)
     launches0 = ctx.launch_count
     ms_total = timed_region(step, args.steps)
     launches = ctx.launch_count - launches0

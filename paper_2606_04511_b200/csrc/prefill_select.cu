@@ -451,6 +451,10 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
     PF_TRACE(0);
+    // Programmatic dependent launch: the prologue above and the load of the group's pooled keys (never written by a kernel
+    // that signals completion early, see sparda.h cfg.no_pdl) overlap the previous kernel's tail; the Forecast / query tiles
+    // and every store (ids, the comparison selector's scratch tile) wait for it.
+    pdl_launch_dependents();
 
     // Tile schedule (identical in every role): tiles sorted by cost (descending row index), dealt in a snake over the
     // group's CTAs.  Tile s covers rows [m0, m0 + 128), m0 = (mt_lo + n_tiles - 1 - s) * 128.
@@ -469,6 +473,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
             for (int kh = 0; kh < KH; ++kh)
                 for (int nh = 0; nh < nb_boxes; ++nh)
                     tma_load_2d(smem + SM::OFF_B + kh * SM::B_SLAB + nh * 256 * 128, &tmapB, kh * 64, g * p.n_blocks + nh * 256, b_full);
+            pdl_wait();
             uint32_t it = 0;
             for (int r = 0; r < n_rounds; ++r) {
                 const int mt = tile_of_round(r);
@@ -514,6 +519,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
         }
     } else {
         // =============================== epilogue: PF_NP threads per query row ===============================
+        pdl_wait();
         const int q = warp & 3;                                  // TMEM lane quadrant this warp may access
         const int part = REPL ? q * PF_NP + ((warp - 2) >> 2) : (warp - 2) >> 2;   // which share of the row's chunks this warp takes
         const int trow = REPL ? lane : q * 32 + lane;            // row within the tile
@@ -648,7 +654,15 @@ int launch_mode(sparda_ctx* ctx, const void* A, const void* Kpool, int T, int n_
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(prefill_select_kernel<D, BASELINE, REPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
         ks.attr_set = true;
     }
-    prefill_select_kernel<D, BASELINE, REPL><<<per_group * Hkv, PF_THREADS, SM::TOTAL, st>>>(mapA, mapB, p);
+    cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((unsigned)(per_group * Hkv), 1, 1);
+    lc.blockDim = dim3(PF_THREADS, 1, 1);
+    lc.dynamicSmemBytes = SM::TOTAL;
+    lc.stream = st;
+    lc.attrs = at;
+    lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
+    SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, prefill_select_kernel<D, BASELINE, REPL>, mapA, mapB, p));
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;
     return SPARDA_OK;

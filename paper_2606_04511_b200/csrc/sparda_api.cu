@@ -240,20 +240,18 @@ int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* K
 
 // Algorithm 2, lines 4-7, for n_layers layers, plain (double-buffered pool, every block fetched) or with the
 // previous step's blocks kept per layer.  Given layer l's projections, line 4 (select B_{l+1}) and line 7
-// (attention l) do not depend on each other, so in overlap mode they run concurrently; the lookahead chain of layer l+1
-// (Forecast projection if asked for, select + reuse plan, prefetch) is ONE stream-ordered sequence on a side stream, the
-// two side streams (the context's own and the caller's prefetch stream) alternating by layer parity:
-//   compute stream cs      :  record ev_top[l]  ->  wait ev_gather[l]  ->  attention l
-//   side stream x[(l+1)&1] :  wait ev_top[l]  ->  [F_l = X_l W_F]  ->  select B_{l+1} (+ plan)  ->  gather B_{l+1}  ->  record ev_gather[l+1]
-// The kernels of a chain follow each other with no event in between, so programmatic dependent launch overlaps each one's
-// launch and prologue with its predecessor's tail, and there are two cross-stream hand-offs per layer, not three (round 1
-// ran select and gather on different streams: 18.6 us per layer with nothing to fetch; this order: see DESIGN.md 5.4).
-// Chains of consecutive layers sit on different streams, so select B_{l+2} overlaps a long gather B_{l+1}.
+// (attention l) do not depend on each other, so in overlap mode they run concurrently on two streams; the prefetch has
+// its own, on which the gathers run one after the other, each alone on the link:
+//   compute stream  cs:  record ev_top[l]  ->  wait ev_gather[l]  ->  attention l
+//   select stream   ss:  wait ev_top[l]    ->  [F_l = X_l W_F]  ->  select B_{l+1} (+ reuse plan)  ->  record ev_sel[l+1]
+//   prefetch stream ps:  wait ev_sel[l+1]  ->  gather B_{l+1}  ->  record ev_gather[l+1]
 // ev_top[l] follows attention l-1 on cs, so a select never runs more than one layer ahead of the attention (in a model,
 // F_l exists only once layer l-1 is complete) and it releases the buffers gather l+1 writes: pool[(l+1)&1] was last read
-// by attention l-1 (plain); pool_{l+1} and slot_ids_{l+1} by attention l+1 of the previous step (cached).  Every chain ends
-// in an event an attention waits for, so cs has joined both side streams when the step ends (capturable).  Serial mode:
-// the same kernels on cs in Algorithm-2 order.
+// by attention l-1 (plain); pool_{l+1} and slot_ids_{l+1} by attention l+1 of the previous step (cached).  Every gather
+// ends in an event an attention waits for, so cs has joined both side streams when the step ends (capturable).  A
+// cross-stream hand-off costs next to nothing inside a CUDA graph (measured); putting a layer's select and gather on one
+// stream and alternating two such streams between layers was tried: same floor, but two gathers then share the link and
+// the step with every block fetched loses 1 %.  Serial mode: the same kernels on cs in Algorithm-2 order.
 // timing events around one launch of `kind` (0 select, 1 gather, 2 attention) on stream st
 static inline cudaEvent_t* prof_slot(sparda_ctx* ctx, int kind) {
     return &ctx->ev_prof[((size_t)kind * (ctx->max_layers + 1) + ctx->prof_n[kind]) * 2];
@@ -278,7 +276,7 @@ struct HostIO {
 static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                             int topk, cudaStream_t cs, cudaStream_t ps_in, int mode, const HostIO* io = nullptr) {
     const bool overlap = mode == SPARDA_STEP_OVERLAP;
-    cudaStream_t side[2] = {overlap ? ctx->select_stream : cs, overlap ? ps_in : cs};
+    cudaStream_t ss = overlap ? ctx->select_stream : cs, ps = overlap ? ps_in : cs;
     int rc;
     ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
     if (io) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(const_cast<void*>(F0cur), io->F0cur, io->f_bytes, cudaMemcpyHostToDevice, cs));
@@ -304,7 +302,7 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
         }
         if (l + 1 < n_layers) {
             const sparda_cached_layer* nx = &layers[l + 1];
-            cudaStream_t xs = side[(l + 1) & 1];
+            cudaStream_t xs = ss, gs = ps;
             if (overlap) {
                 SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_top[l], cs));
                 SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(xs, ctx->ev_top[l], 0));
@@ -324,11 +322,15 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
                 rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, xs);
             if (rc) return rc;
             SPARDA_PROF_END(0, xs);
-            SPARDA_PROF_BEGIN(1, xs);
-            rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->slot_ids ? nx->fetch : nx->base.ids, topk, nx->pool, xs);
+            if (overlap) {
+                SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], xs));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(gs, ctx->ev_sel[l + 1], 0));
+            }
+            SPARDA_PROF_BEGIN(1, gs);
+            rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->slot_ids ? nx->fetch : nx->base.ids, topk, nx->pool, gs);
             if (rc) return rc;
-            SPARDA_PROF_END(1, xs);
-            if (overlap) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], xs));
+            SPARDA_PROF_END(1, gs);
+            if (overlap) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], gs));
         }
         ctx->pdl_next = overlap ? 0 : 1;       // the attention waits for its gather's event in overlap mode
         if (l == 0) {

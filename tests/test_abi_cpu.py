@@ -69,7 +69,7 @@ def test_binding_struct_layout_matches_header():
     lay_body = re.sub(r"/\*.*?\*/", "", lay_body, flags=re.S)
     lfields = re.findall(r"\*\s*([A-Za-z_]+);", lay_body)
     assert lfields == [f[0] for f in binding.SpardaLayer._fields_]
-    assert ctypes.sizeof(binding.SpardaLayer) == 6 * ctypes.sizeof(ctypes.c_void_p)
+    assert ctypes.sizeof(binding.SpardaLayer) == len(lfields) * ctypes.sizeof(ctypes.c_void_p) == 9 * ctypes.sizeof(ctypes.c_void_p)
 
 
 def test_product_does_not_import_oracle():

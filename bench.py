@@ -370,6 +370,10 @@ def bench_kernels(torch, binding, peaks, ncu, ncu_src, batch):
     ids_att = torch.arange(k, dtype=torch.int32, device="cuda").repeat(R, 1).contiguous()
     t_att = graph_time(torch, lambda i, s: ctx.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT, reps=max(2, 80 // NS_ATT))
     cl_att = ctx.attn_cluster
+    # the tcgen05 "swap-AB" experiment (cfg.attn_impl = 1) on the same pools: a measured comparison, not the product path
+    ctx5 = binding.Sparda.from_config(cfg, attn_impl=1)
+    t_att5 = graph_time(torch, lambda i, s: ctx5.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT, reps=max(2, 80 // NS_ATT))
+    ctx5.close()
     del pools
     sel_bytes = kp_bytes + R * D * 2 + R * k * 4
     att_bytes = pool_bytes + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
@@ -377,7 +381,9 @@ def bench_kernels(torch, binding, peaks, ncu, ncu_src, batch):
     out = [kernel_entry("forecast_select_kernel<128,false>", f"batch {batch}: R={R}, {Nb} blocks, top-{k}; cold HBM, graph replay", t_sel, sel_bytes,
                         hbm, ncu, f"select_{tag}", ncu_src, cluster=cs_sel),
            kernel_entry("sparse_decode_kernel<128>", f"batch {batch}: R={R}, top-{k} x 32 KiB; cold HBM, graph replay", t_att, att_bytes,
-                        hbm, ncu, f"attn_{tag}", ncu_src, cluster=cl_att, ctas_per_row=ctx.attn_splits(k))]
+                        hbm, ncu, f"attn_{tag}", ncu_src, cluster=cl_att, ctas_per_row=ctx.attn_splits(k)),
+           kernel_entry("sparse_decode_tc5_kernel (experiment)", f"batch {batch}: same shape, tcgen05 swap-AB form (attn_impl=1); not the default", t_att5,
+                        att_bytes, hbm, ncu, f"attn_tc5_{tag}", ncu_src, cluster=cl_att)]
     if batch == 32:
         # f3: the paper's geometry -- (32,16) compressed-key grid (4 keys per block), max-pool to blocks, budget 96 = 1 + 32 + 63
         NS_G = 8

@@ -75,6 +75,8 @@ typedef struct {
                            SM count; 1, 2, 4, 8 or 16 forces it (sweeps and tests)                                       */
     int hidden;      /* model width of the optional in-step Forecast projection (sparda_layer.X / .WF); 0 = not used;
                         else a multiple of 64 in [64, 8192]                                                              */
+    int attn_impl;   /* 0 = sparse_decode on mma.sync (default); 1 = the tcgen05 "swap-AB" experiment (tokens on the M side,
+                        accumulators in TMEM) for D = 128 and row-aligned splits, anything else falls back to 0          */
     int no_pdl;      /* 0 = the stand-alone calls and the serial step launch their kernels with programmatic dependent
                         launch: a kernel's launch and prologue overlap the tail of the previous kernel of the stream, and
                         forecast_select also streams pooled keys into its ring before that kernel has completed.  This

@@ -35,7 +35,7 @@ class SpardaError(RuntimeError):
 class SpardaConfig(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int) for n in (
         "batch", "n_q_heads", "n_kv_heads", "head_dim", "block_size", "max_blocks", "topk", "gather_ctas",
-        "gather_mode", "attn_splits", "max_layers", "select_cluster", "hidden", "no_pdl")]
+        "gather_mode", "attn_splits", "max_layers", "select_cluster", "hidden", "attn_impl", "no_pdl")]
 
 
 class SpardaLayer(ctypes.Structure):
@@ -117,10 +117,10 @@ class Sparda:
     """One libsparda context (one shape family on the current device)."""
 
     def __init__(self, batch, n_q_heads, n_kv_heads, head_dim, max_blocks, topk, block_size=64, gather_ctas=0,
-                 gather_mode=GATHER_TMA, attn_splits=0, max_layers=0, select_cluster=0, hidden=0, no_pdl=0):
+                 gather_mode=GATHER_TMA, attn_splits=0, max_layers=0, select_cluster=0, hidden=0, attn_impl=0, no_pdl=0):
         self._h = ctypes.c_void_p()
         self.cfg = SpardaConfig(batch, n_q_heads, n_kv_heads, head_dim, block_size, max_blocks, topk, gather_ctas,
-                                gather_mode, attn_splits, max_layers, select_cluster, hidden, no_pdl)
+                                gather_mode, attn_splits, max_layers, select_cluster, hidden, attn_impl, no_pdl)
         self._L = lib()
         rc = self._L.sparda_create(ctypes.byref(self.cfg), ctypes.byref(self._h))
         if rc != 0:

@@ -47,6 +47,7 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     if (cfg->topk < 1 || cfg->topk > 256) return SPARDA_EINVAL;
     if (cfg->gather_mode != SPARDA_GATHER_TMA && cfg->gather_mode != SPARDA_GATHER_LDG) return SPARDA_EINVAL;
     if (cfg->gather_ctas < 0 || cfg->gather_ctas > 1024 || cfg->attn_splits < 0 || cfg->max_layers < 0) return SPARDA_EINVAL;
+    if (cfg->attn_impl != 0 && cfg->attn_impl != 1) return SPARDA_EINVAL;
     if (cfg->hidden != 0 && (cfg->hidden < 64 || cfg->hidden > 8192 || cfg->hidden % 64 != 0)) return SPARDA_EINVAL;
     if (!(cfg->select_cluster == 0 || cfg->select_cluster == 1 || cfg->select_cluster == 2 || cfg->select_cluster == 4 ||
           cfg->select_cluster == 8 || cfg->select_cluster == 16))

@@ -22,7 +22,7 @@ struct sparda_kernel_state {
 enum {
     SPARDA_K_SELECT_128, SPARDA_K_SELECT_64, SPARDA_K_SELECT_GRID_128, SPARDA_K_SELECT_GRID_64,
     SPARDA_K_ATTN_128, SPARDA_K_ATTN_64, SPARDA_K_ATTN_CL_128, SPARDA_K_ATTN_CL_64,
-    SPARDA_K_GATHER_TMA, SPARDA_K_PROBE, SPARDA_K_STANDIN, SPARDA_K_PROJECT,
+    SPARDA_K_GATHER_TMA, SPARDA_K_PROBE, SPARDA_K_STANDIN, SPARDA_K_PROJECT, SPARDA_K_ATTN_T5, SPARDA_K_ATTN_T5_CL,
     SPARDA_K_PF_0, /* 8 prefill instantiations: D x BASELINE x REPL */
     SPARDA_K_COUNT = SPARDA_K_PF_0 + 8
 };
@@ -116,6 +116,9 @@ int sparda_launch_reuse_plan(sparda_ctx*, const int32_t* ids_new, int topk, int3
                              cudaStream_t);
 int sparda_launch_attn(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
                        int n_slots, void* O, cudaStream_t);
+// the tcgen05 experiment (cfg.attn_impl = 1): SPARDA_OK, 1 = shape outside its range (fall back to the mma.sync kernel), or an error
+int sparda_launch_attn_tc5(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
+                           int n_slots, void* O, cudaStream_t);
 int sparda_launch_prefill_select(sparda_ctx*, const void* F, const void* Kpool, int T, int n_blocks, int row0,
                                  int n_rows, int topk, int32_t* ids, cudaStream_t);
 int sparda_launch_prefill_baseline(sparda_ctx*, const void* Q, const void* Kpool, int T, int n_blocks, int row0,

@@ -566,6 +566,10 @@ int sparda_resolve_splits(const sparda_ctx* ctx, int topk) {
 
 int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
                        int n_slots, void* O, cudaStream_t st) {
+    if (ctx->cfg.attn_impl == 1) {   // the tcgen05 (swap-AB) experiment; shapes outside its range fall through
+        const int rc5 = sparda_launch_attn_tc5(ctx, Q, pool, ids, topk, indexed, n_slots, O, st);
+        if (rc5 != 1) return rc5;
+    }
     const int D = ctx->cfg.head_dim;
     const uint64_t rows = (uint64_t)ctx->R * n_slots * 2 * S_BLK;
     CUtensorMap map;

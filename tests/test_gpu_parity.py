@@ -754,10 +754,10 @@ B32 = synth.DecodeConfig("cfg4_b32_attn", batch=32, n_q_heads=32, n_kv_heads=2, 
 B16 = synth.DecodeConfig("cfg4_b16_attn", batch=16, n_q_heads=32, n_kv_heads=2, head_dim=128, n_blocks=96, topk=64, seed=82)
 
 
-def _attn_case(cfg, sp, oracle, splits, want_cluster):
+def _attn_case(cfg, sp, oracle, splits, want_cluster, **ctx_kw):
     """select -> gather (device source) -> attention with a padded row and an empty row, against the oracle; asserts the
     reduction path the launch resolved to (DSMEM cluster of `want_cluster` CTAs per row, 0 = workspace + ticket)."""
-    L, ctx, kpool = _setup(cfg, sp, attn_splits=splits)
+    L, ctx, kpool = _setup(cfg, sp, attn_splits=splits, **ctx_kw)
     ids = torch.empty((cfg.rows, cfg.topk), dtype=torch.int32, device="cuda")
     ctx.forecast_select(L["F"], kpool, cfg.n_blocks, cfg.topk, ids)
     torch.cuda.synchronize()
@@ -795,6 +795,17 @@ def test_sparse_decode_cluster_paths(cfg, splits, want, sp, oracle):
     and batch 16 (R = 32) that bench.py's 0.8-of-HBM figure is taken on, plus forced splits on a small case and one shape
     that must take the workspace + ticket reduction (k = 37 has no useful divisor)."""
     _attn_case(cfg, sp, oracle, splits, want)
+
+
+@pytest.mark.parametrize("cfg,splits,want", [(B32, 0, 2), (B16, 0, 4), (G16, 2, 2), (G16, 4, 4), (G16.with_(batch=3), 8, 8),
+                                             (G16.with_(topk=24, batch=3), 8, 8), (G16.with_(batch=1, topk=7), 1, 0)],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_sparse_decode_tcgen05_experiment(cfg, splits, want, sp, oracle):
+    """cfg.attn_impl = 1: the swap-AB tcgen05 form of the attention (tokens on the M side, accumulators in TMEM, V read as an
+    MN-major operand), kept as a measured experiment.  Same checks as the default kernel, including an odd
+    number of slots per CTA (a repeated, masked tile), padded rows whose pool slots hold NaN, an empty row and the
+    layer-0 indexed form."""
+    _attn_case(cfg, sp, oracle, splits, want, attn_impl=1)
 
 
 def test_cfg4_full_size_layer(sp, oracle):

@@ -110,8 +110,9 @@ typedef struct {
 #define SPARDA_STEP_SERIAL 1     /* same kernels, everything on compute_stream in Algorithm-2 order (no overlap) */
 
 /* Create a context for one shape family on the current device.  Allocates the workspace (split-K partials
- * R*max_splits*16*(D+2) floats, R tickets, 2*max_layers events, host-step
- * staging, a 256 KiB-per-SM score tile for the comparison selector).
+ * R*max_splits*16*(D+2) floats, R tickets, 3*max_layers events, an internal select stream, host-step staging, a 256
+ * KiB-per-SM score tile for the comparison selector).  Launcher state (shared-memory opt-ins, cluster occupancy answers,
+ * the TMA descriptor cache) lives in the context: contexts of different shapes and devices coexist in one process.
  * Returns SPARDA_OK, SPARDA_EINVAL, SPARDA_EUNSUPPORTED, SPARDA_ENOMEM or SPARDA_ECUDA; *out is set only on
  * success.  Destroy with sparda_destroy (synchronises the device first).                                     */
 int sparda_create(const sparda_config* cfg, sparda_ctx** out);
@@ -126,8 +127,10 @@ int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_bloc
 /* (A4 / f4) Forecast projection, Eq.3: F[b, g, :] = bf16(X[b, :] . W_F[:, g*D:(g+1)*D]), one Forecast head of
  * width D per GQA group; fp32 accumulation in a fixed order (deterministic), one rounding.  X [B][hidden] device bf16 (the
  * layer's input hidden states), W_F [hidden][Hkv*D] device bf16 row-major, F_out [R][D] device (R = B*Hkv, the layout
- * sparda_forecast_select reads).  64 <= hidden <= 8192, a multiple of 64.  One kernel on `stream`; bound by streaming W_F
- * once.  The path's calls take F as an input, so a caller that computes F inside its fused QKV+F GEMM does not need this. */
+ * sparda_forecast_select reads).  64 <= hidden <= 8192, a multiple of 64.  One kernel on `stream` (cluster split-K on
+ * mma.sync, partials reduced in a fixed order through distributed shared memory; no workspace); bound by streaming W_F
+ * once.  The path's calls take F as an input, so a caller that computes F inside its fused QKV+F GEMM does not need this;
+ * sparda_layer.X / .WF run it inside sparda_decode_step.                                                                */
 int sparda_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F_out, void* stream);
 
 /* (f2) Decode-time cache maintenance, Alg.2 lines 2-3: append the new token's key and value at position t
@@ -170,8 +173,9 @@ int sparda_prefetch_launch(sparda_ctx* ctx, const void* host_kv, int n_blocks, c
  * Split-K flash-decode over a flat list of the R*topk slots.  Row-aligned splits with 2, 4 or 8 CTAs per row run as
  * one thread-block cluster per row and reduce their partials through distributed shared memory; any other split
  * reduces through the context's L2-resident workspace, merged by the last CTA of each row (ticket).
- * The workspace is shared by every launch on the context: at most ONE sparse_decode (and one forecast_project) may be
- * in flight per context at a time -- order concurrent launches with events or use one context per stream.        */
+ * The workspace is shared by every launch on the context: at most ONE sparse_decode may be in flight per context at a
+ * time -- order concurrent launches with events or use one context per stream.  (The other kernels keep their
+ * intermediate state in shared memory and may overlap freely.)                                                  */
 int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, int topk,
                          int pool_is_indexed, int n_slots, void* O, void* stream);
 

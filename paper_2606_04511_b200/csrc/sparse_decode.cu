@@ -82,6 +82,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
     __shared__ float s_ml[1][NW][2][16];
     __shared__ unsigned int s_last;
     __shared__ uint64_t bar_m;
+    __shared__ uint64_t bar_red;     // CL: completes when every CTA's partials of the head rows this CTA owns have landed (tx bytes)
     __shared__ __align__(128) float s_pm[16 * 32];
     __shared__ float s_w[16 * 16], s_run[16], s_resc[16], s_newmax[16];
 
@@ -93,11 +94,19 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
     if (tid == 0) {
         for (int i = 0; i < NW; ++i) { mbar_init(&bar_k[i], 1); mbar_init(&bar_v[i], 1); }
         mbar_init(&bar_m, 1);
+        if (CL) {
+            // cluster reduction: this CTA owns 16 / n head rows and expects (m, l, O[D]) of each of them from each of the n CTAs
+            mbar_init(&bar_red, 1);
+            mbar_arrive_expect_tx(&bar_red, 16u * (D * 4 + 8));
+        }
         mbar_fence_init();
         fence_proxy_async_smem();
         tma_prefetch_desc(&tmap);
     }
     __syncthreads();
+    // CL: every CTA of the cluster is running, with bar_red armed, before anyone stores into a neighbour's shared memory:
+    // arrive now, wait in front of the reduction (by then everybody has long arrived)
+    if (CL) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     pdl_wait();                  // the prologue above overlaps the previous kernel's tail; global memory from here on
     pdl_launch_dependents();
 
@@ -430,7 +439,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
         const int rows_per = 16 / n;
         float* land = reinterpret_cast<float*>(smem + SM::OFF_XCHG + (size_t)NW * SM::XCHG_WARP);
         float* land_ml = land + 16 * D;
-        const uint32_t land_u32 = smem_u32(land), ml_u32 = smem_u32(land_ml);
+        const uint32_t land_u32 = smem_u32(land), ml_u32 = smem_u32(land_ml), red_u32 = smem_u32(&bar_red);
+        asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");   // pairs with the arrive at kernel start
         for (int it = tid; it < 16 * C4; it += NT) {
             const int row = it / C4, c4 = it % C4;
             float M = -INFINITY;
@@ -446,17 +456,23 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
                     reinterpret_cast<const float*>(smem + SM::OFF_XCHG + (size_t)i * SM::XCHG_WARP) + row * SM::OROW + c4 * 4);
                 acc.x += wg * v.x; acc.y += wg * v.y; acc.z += wg * v.z; acc.w += wg * v.w;
             }
+            // asynchronous stores into the owner's landing area that count their bytes on the owner's barrier: no release
+            // fence and no closing cluster barrier -- the owner waits for "16 x (D x 4 + 8) bytes have landed"
             const uint32_t owner = (uint32_t)(row / rows_per), lrow = (uint32_t)(row % rows_per);
-            uint32_t dst, dml;
+            uint32_t dst, dml, dbar;
+            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(dbar) : "r"(red_u32), "r"(owner));
             asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(dst) : "r"(land_u32 + ((part * rows_per + lrow) * D + c4 * 4) * 4), "r"(owner));
-            asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "f"(acc.x), "f"(acc.y), "f"(acc.z), "f"(acc.w) : "memory");
+            asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];" ::"r"(dst), "f"(acc.x),
+                         "f"(acc.y), "f"(acc.z), "f"(acc.w), "r"(dbar)
+                         : "memory");
             if (c4 == 0) {
                 asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(dml) : "r"(ml_u32 + ((part * rows_per + lrow) * 2) * 4), "r"(owner));
-                asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(dml), "f"(M), "f"(L) : "memory");
+                asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(dml), "f"(M), "f"(L), "r"(dbar)
+                             : "memory");
             }
         }
         TRACE(4);
-        asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+        mbar_wait(&bar_red, 0);
         TRACE(5);
         const int b = r / p.Hkv, g = r % p.Hkv;
         __nv_bfloat16* obase = p.O + (size_t)(b * p.Hq + g * p.G) * D;
@@ -598,9 +614,23 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     const int s_per = p.quota > 0 && p.rem == 0 && topk % p.quota == 0 ? topk / p.quota : 0;
     const bool cl = (s_per == 2 || s_per == 4 || s_per == 8) && (long long)s_per * ctx->R == C;
     rc = 1;
-    int used_cl = cl ? s_per : 0;
-    if (cl) rc = D == 128 ? launch<128, true>(ctx, &map, p, C, s_per, st) : launch<64, true>(ctx, &map, p, C, s_per, st);
-    if (rc == 1) used_cl = 0;
+    int used_cl = 0;
+    if (cl) {
+        // When the device cannot keep all R clusters of s_per CTAs resident (batch 8: 16 clusters of 8 with one 200 KB CTA per
+        // SM), half as many CTAs per row in clusters that do fit beat the same CTA count reduced through the L2 workspace
+        // (measured, batch 8: 128 CTAs + ticket 11.9 us; 64 CTAs in clusters of 4: see DESIGN.md 5.3).  The automatic split
+        // only: an explicit cfg.attn_splits is honoured as given.
+        for (int s = s_per; s >= 2 && rc == 1; s /= 2) {
+            if (topk % s != 0) break;
+            AttnParams q = p;
+            const int Cs = s * ctx->R;
+            q.quota = q.W / Cs;
+            q.rem = 0;
+            rc = D == 128 ? launch<128, true>(ctx, &map, q, Cs, s, st) : launch<64, true>(ctx, &map, q, Cs, s, st);
+            if (rc != 1) used_cl = s;
+            if (ctx->cfg.attn_splits > 0) break;
+        }
+    }
     if (rc == 1) rc = D == 128 ? launch<128, false>(ctx, &map, p, C, 1, st) : launch<64, false>(ctx, &map, p, C, 1, st);
     if (rc) return rc;
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());

@@ -10,6 +10,8 @@ import numpy as np
 ATTN_MAX_ABS = 2e-2
 ATTN_MEAN_ABS = 2e-3
 BAND_REL = 1e-3
+# (rows checked, rows that needed the near-tie band) per check_ids call; tests/conftest.py prints the totals per test
+BAND_LOG = []
 
 
 def bits_to_f32(u16):
@@ -43,6 +45,7 @@ def check_ids(gpu_ids, oracle_ids, oracle_scores, n_cand=None):
             f"row {r}: ids differ outside the near-tie band: gpu-only {np.setdiff1d(gv, o)}, "
             f"oracle-only {np.setdiff1d(o, gv)}, scores {s[diff]}, s_k {sk}, tol {tol}")
         band_rows += 1
+    BAND_LOG.append((R, band_rows))
     return band_rows
 
 

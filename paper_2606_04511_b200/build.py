@@ -26,6 +26,17 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def build_trace(out: str) -> str:
+    """Debug build with device-side timelines (-DSPARDA_TRACE): per-CTA cycle / globaltimer stamps in the select, attention,
+    prefill-select and tcgen05-attention kernels, read back through the sparda_debug_set_*_trace / _log hooks that only this
+    build exports.  Never the product: written to `out`, not to libsparda.so."""
+    res = subprocess.run([NVCC, *FLAGS, "-DSPARDA_TRACE", "-o", out, *sources()], capture_output=True, text=True)
+    if res.returncode:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed building the trace library")
+    return out
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *sources()]
@@ -38,4 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--trace" in sys.argv:       # python -m paper_2606_04511_b200.build --trace /path/to/libsparda_trace.so
+        print(build_trace(sys.argv[sys.argv.index("--trace") + 1]))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -66,8 +66,10 @@ typedef struct {
     int block_size;  /* S, must be 64 */
     int max_blocks;  /* largest Nb any call will pass (<= 8192) */
     int topk;        /* largest k any call will pass (<= 256) */
-    int gather_ctas; /* persistent gather grid size; 0 = default (4 for TMA, 16 for LDG; bench.py gather_sweep has the B200
-                        trade-off between link rate and what the CTAs cost the compute stream; Table 7)    */
+    int gather_ctas; /* persistent gather grid size; 0 = default (8 for TMA, 16 for LDG: alone on the link 2 TMA CTAs reach the
+                        plateau, but beside a kernel that saturates HBM the read latency triples and 4 CTAs deliver 34 GB/s
+                        where 8 deliver 49; bench.py gather_sweep has the B200 trade-off between link rate, rate under
+                        load and what the CTAs cost the compute stream; Table 7)                            */
     int gather_mode; /* SPARDA_GATHER_TMA or SPARDA_GATHER_LDG */
     int attn_splits; /* split-K CTAs per row for sparse_decode; 0 = auto from B, Hkv, k and the SM count */
     int max_layers;  /* largest n_layers sparda_decode_step will see (events are pre-created); 0 = 64 */

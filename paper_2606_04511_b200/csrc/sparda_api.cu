@@ -70,7 +70,7 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
     ctx->sm_count = prop.multiProcessorCount;
     ctx->R = cfg->batch * cfg->n_kv_heads;
     ctx->G = G;
-    if (ctx->cfg.gather_ctas == 0) ctx->cfg.gather_ctas = cfg->gather_mode == SPARDA_GATHER_TMA ? 4 : 16;
+    if (ctx->cfg.gather_ctas == 0) ctx->cfg.gather_ctas = cfg->gather_mode == SPARDA_GATHER_TMA ? 8 : 16;
     ctx->max_layers = cfg->max_layers > 0 ? cfg->max_layers : 64;
     {   // partial slots per row of the flat split-K attention: n_parts <= ceil(CTAs / R) + 1
         int per_row = cfg->attn_splits > 0 ? cfg->attn_splits : (2 * ctx->sm_count + ctx->R - 1) / ctx->R;

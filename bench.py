@@ -721,7 +721,20 @@ def bench_gather_sweep(torch, binding, peaks, ceiling, host_layer_b4):
                     row["hbm_loaded_throughout"] = bool(loaded)
                 rows.append(row)
                 gctx.close()
-        out.append({"batch": batch, "gather_mib_per_launch": gbytes / 2**20, "pair_us_alone": round(alone, 2),
+        # f4's peer-HBM tier with the link out of the way: the same gather from a source in this GPU's own HBM (a peer's HBM
+        # behind NVLink cannot be faster than this; the harness leases one GPU, so the peer copy itself is not measured)
+        hbm_tier = None
+        if batch == 4:
+            src = torch.empty((R, Nb, 2, 64, D), dtype=torch.bfloat16, device="cuda")        # 1 GiB, cold: 16 MiB of it is read per launch
+            hbm_tier = []
+            for mode, name, ctas_list in ((binding.GATHER_TMA, "tma", (8, 16, 32, 64, 148)), (binding.GATHER_LDG, "ldg", (32, 64, 148, 296))):
+                for ctas in ctas_list:
+                    gctx = binding.Sparda.from_config(cfg, gather_mode=mode, gather_ctas=ctas)
+                    t_h = graph_time(torch, lambda i, s: gctx.prefetch_launch(src, Nb, ids_g, k, pool, stream=s), 1, reps=20)
+                    hbm_tier.append({"engine": name, "ctas": ctas, "us": round(t_h * 1e6, 2), "gbs": round(gbytes / t_h / 1e9, 1)})
+                    gctx.close()
+            del src
+        out.append({"batch": batch, "gather_mib_per_launch": gbytes / 2**20, "pair_us_alone": round(alone, 2), "hbm_tier": hbm_tier,
                     "standin_us_alone": round(standin_us, 1) if standin_us else None,
                     "pair": "forecast_select + sparse_decode of this batch, cold HBM, 20 pairs per graph", "rows": rows})
         cctx.close()

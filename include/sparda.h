@@ -164,6 +164,16 @@ int sparda_forecast_select(sparda_ctx* ctx, const void* F, const void* Kpool, in
 int sparda_prefetch_launch(sparda_ctx* ctx, const void* host_kv, int n_blocks, const int32_t* ids, int topk,
                            void* dev_pool, void* stream);
 
+/* (f4, outside the paper) Peer-HBM offload tier: the KV cache of the offloaded layers may live in another GPU's HBM instead
+ * of pinned host memory -- same block layout, same persistent gather, the loads travel over NVLink / NVSwitch instead of
+ * PCIe.  sparda_prefetch_launch takes any pointer the current device can dereference; this call makes
+ * `peer_device`'s memory such a pointer (cudaDeviceEnablePeerAccess from the context's device; calling it again is not an
+ * error).  The link's bandwidth-delay product is ~30 times PCIe's, so give the gather more CTAs on this tier
+ * (cfg.gather_ctas; bench.py roofline.gather_sweep.hbm_tier has the engine's rate by CTA count with the link out of the way).
+ * Returns SPARDA_EUNSUPPORTED when the two devices have no peer path, SPARDA_EINVAL for peer_device == the context's device
+ * or out of range.  Host-synchronous (driver call); not for the decode loop.                                            */
+int sparda_enable_peer_tier(sparda_ctx* ctx, int peer_device);
+
 /* (a5/a6) Block-sparse GQA attention with the real query, Eq.5, Alg.2 l.7:
  * O[b,h,:] = bf16( softmax_t( q_h . k_t / sqrt(D) ) V ) over every token t of every selected block of row
  * r = b*Hkv + h/G; bf16 tensor-core products, fp32 softmax and accumulation, one rounding; no causal mask

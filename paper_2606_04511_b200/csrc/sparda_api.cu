@@ -214,6 +214,22 @@ int sparda_prefetch_launch(sparda_ctx* ctx, const void* host_kv, int n_blocks, c
     return sparda_launch_gather(ctx, host_kv, n_blocks, ids, topk, dev_pool, (cudaStream_t)stream);
 }
 
+int sparda_enable_peer_tier(sparda_ctx* ctx, int peer_device) {
+    if (!ctx) return SPARDA_EINVAL;
+    int n = 0, can = 0, cur = -1;
+    if (cudaGetDeviceCount(&n) != cudaSuccess) return sparda_set_cuda_error(ctx, cudaGetLastError(), "cudaGetDeviceCount");
+    if (peer_device < 0 || peer_device >= n || peer_device == ctx->device) return SPARDA_EINVAL;
+    SPARDA_CUDA_TRY(ctx, cudaDeviceCanAccessPeer(&can, ctx->device, peer_device));
+    if (!can) return SPARDA_EUNSUPPORTED;
+    SPARDA_CUDA_TRY(ctx, cudaGetDevice(&cur));
+    if (cur != ctx->device) SPARDA_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaError_t e = cudaDeviceEnablePeerAccess(peer_device, 0);
+    if (cur != ctx->device) (void)cudaSetDevice(cur);
+    if (e == cudaErrorPeerAccessAlreadyEnabled) { (void)cudaGetLastError(); e = cudaSuccess; }
+    if (e != cudaSuccess) return sparda_set_cuda_error(ctx, e, "cudaDeviceEnablePeerAccess");
+    return SPARDA_OK;
+}
+
 int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, int topk,
                          int pool_is_indexed, int n_slots, void* O, void* stream) {
     if (!ctx || !sparda_aligned(Q, 16) || !sparda_aligned(dev_pool, 16) || !sparda_aligned(ids, 4) || !sparda_aligned(O, 16))

@@ -11,7 +11,7 @@
 // issued as soon as QK^T has consumed the tile).  The group's G <= 16 query heads are the M = 16 rows of
 // mma.sync.m16n8k16 (bf16 in, fp32 accumulate): S = Q K^T (16 x 64 per block), online softmax in the exp2
 // domain, O += P V.  Warp partials (m, l, O) are merged through shared memory.  The CTA partials of one row are reduced
-// inside a thread-block cluster through distributed shared memory when the split is row-aligned with 2, 4 or 8 CTAs per
+// inside a thread-block cluster through distributed shared memory when the split is row-aligned with 2, 4, 8 or 16 CTAs per
 // row (the [BJ] shapes), else through an L2-resident workspace by the last CTA to finish that row (ticket).  One bf16
 // rounding.
 // HBM-bound by design: 16 FLOP per KV byte at G = 16; the tensor pipe idles most of the time.
@@ -66,7 +66,7 @@ __device__ __forceinline__ int flat_owner(int f, int quota, int rem) {
     return f < thr ? f / (quota + 1) : rem + (f - thr) / quota;
 }
 
-// CL (row-aligned splits, s = 2, 4 or 8 CTAs per row launched as one cluster): the CTA partials of a row are reduced
+// CL (row-aligned splits, s = 2, 4, 8 or 16 CTAs per row launched as one cluster): the CTA partials of a row are reduced
 // through distributed shared memory instead of the L2 workspace -- every CTA sends each head row's partial (m, l, O) to the
 // CTA that owns that head row (16 / s rows each), one cluster barrier, every CTA normalises and stores its rows.  No ticket,
 // no fence, no global round trip, and the final merge is spread over the cluster.
@@ -517,6 +517,7 @@ int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, 
     sparda_kernel_state& ks = ctx->kstate[(CL ? SPARDA_K_ATTN_CL_128 : SPARDA_K_ATTN_128) + (D == 128 ? 0 : 1)];
     if (!ks.attr_set) {
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        if (CL) SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));   // clusters of 16
         ks.attr_set = true;
     }
     cudaLaunchConfig_t lc = {};
@@ -566,6 +567,10 @@ int sparda_resolve_attn_ctas(const sparda_ctx* ctx, int topk) {
         long long aligned = 0;
         for (int s = 1; s <= 8 && s <= topk; ++s)
             if (topk % s == 0 && (long long)s * ctx->R <= ctx->sm_count) aligned = (long long)s * ctx->R;
+        // up to 4 rows (batch 1-2): clusters of 16 (non-portable size), topk / 16 slots per CTA -- at k = 64 every tile of the
+        // launch is in flight at once, one DRAM round trip per warp (measured, 128K shapes: batch 2 7.2 -> 6.5 us, batch 1
+        // 7.1 -> 5.9 us).  From 8 rows on the device cannot keep all clusters of 16 resident (one 200 KB CTA per SM).
+        if (topk % 16 == 0 && ctx->R <= 4) aligned = 16LL * ctx->R;
         C = (aligned * 5 >= flat * 3) ? aligned : flat;
     }
     // workspace: a row meets at most ceil(topk / quota) + 1 CTAs, quota = floor(W / C); keep that <= max_splits
@@ -610,9 +615,9 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     const int C = sparda_resolve_attn_ctas(ctx, topk);
     p.quota = p.W / C;
     p.rem = p.W % C;
-    // row-aligned split with 2, 4 or 8 CTAs per row: reduce the partials inside a cluster (distributed shared memory)
+    // row-aligned split with 2, 4, 8 or 16 CTAs per row: reduce the partials inside a cluster (distributed shared memory)
     const int s_per = p.quota > 0 && p.rem == 0 && topk % p.quota == 0 ? topk / p.quota : 0;
-    const bool cl = (s_per == 2 || s_per == 4 || s_per == 8) && (long long)s_per * ctx->R == C;
+    const bool cl = (s_per == 2 || s_per == 4 || s_per == 8 || s_per == 16) && (long long)s_per * ctx->R == C;
     rc = 1;
     int used_cl = 0;
     if (cl) {

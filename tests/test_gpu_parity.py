@@ -612,6 +612,46 @@ def test_cfg2_full_size_layer(sp, oracle):
     parity.check_attn(_bits(O), want, "cfg2")
 
 
+def test_peer_hbm_tier(sp, oracle):
+    """f4 (outside the paper): the offloaded cache in a PEER GPU's HBM, read by the unchanged persistent gather over
+    NVLink.  Argument validation runs on any box; the copy itself needs two GPUs with a peer path (the round's harness
+    leases one GPU at a time, so there it is skipped -- the same kernel on a device-resident source is covered by
+    test_gather_exact_bytes)."""
+    cfg = G16
+    ctx = sp.Sparda.from_config(cfg, gather_ctas=16)
+    with pytest.raises(sp.SpardaError):
+        ctx.enable_peer_tier(torch.cuda.current_device())            # the context's own device is not a peer
+    with pytest.raises(sp.SpardaError):
+        ctx.enable_peer_tier(torch.cuda.device_count())              # out of range
+    if torch.cuda.device_count() < 2:
+        ctx.close()
+        pytest.skip("one GPU visible: the peer copy cannot run here")
+    peer = (torch.cuda.current_device() + 1) % torch.cuda.device_count()
+    try:
+        ctx.enable_peer_tier(peer)
+    except sp.SpardaError:
+        ctx.close()
+        pytest.skip("no peer path between the two devices")
+    ctx.enable_peer_tier(peer)                                       # twice is not an error
+    L = synth.decode_layer(cfg, 0, device="cpu")
+    peer_kv = L["kv"].to(f"cuda:{peer}")
+    rng = np.random.default_rng(7)
+    ids_np = np.stack([np.sort(rng.choice(cfg.n_blocks, cfg.topk, replace=False)) for _ in range(cfg.rows)]).astype(np.int32)
+    ids_np[-1, cfg.topk // 2:] = -1
+    ids = torch.from_numpy(ids_np).cuda()
+    for mode in (sp.GATHER_TMA, sp.GATHER_LDG):
+        g = sp.Sparda.from_config(cfg, gather_mode=mode, gather_ctas=16)
+        pool = torch.full((cfg.rows, cfg.topk, 2, cfg.block_size, cfg.head_dim), float("nan"), dtype=torch.bfloat16, device="cuda")
+        want = _bits(pool).copy()                                     # NaN pattern: -1 slots must stay untouched
+        g.prefetch_launch(peer_kv, cfg.n_blocks, ids, cfg.topk, pool)
+        torch.cuda.synchronize()
+        got = _bits(pool)
+        oracle.gather(_bits(L["kv"]), ids_np, want)
+        assert got.tobytes() == want.tobytes()
+        g.close()
+    ctx.close()
+
+
 def test_argument_validation(sp):
     with pytest.raises(sp.SpardaError):
         sp.Sparda(1, 4, 1, 96, 64, 8)                                # head_dim not in {64, 128}
@@ -788,12 +828,14 @@ def _attn_case(cfg, sp, oracle, splits, want_cluster, **ctx_kw):
     ctx.close()
 
 
-@pytest.mark.parametrize("cfg,splits,want", [(B32, 0, 2), (B16, 0, 4), (G16, 2, 2), (G16, 4, 4), (MID, 0, 0), (G16.with_(batch=3), 8, 8)],
+@pytest.mark.parametrize("cfg,splits,want", [(B32, 0, 2), (B16, 0, 4), (G16, 2, 2), (G16, 4, 4), (MID, 0, 0), (G16.with_(batch=3), 8, 8),
+                                             (G16, 0, 16), (G16.with_(batch=1), 16, 16)],
                          ids=lambda v: getattr(v, "name", str(v)))
 def test_sparse_decode_cluster_paths(cfg, splits, want, sp, oracle):
     """sparse_decode_kernel<.., CL = true> with 2 and 4 CTAs per row: the launch shapes of configs[3] at batch 32 (R = 64)
-    and batch 16 (R = 32) that bench.py's 0.8-of-HBM figure is taken on, plus forced splits on a small case and one shape
-    that must take the workspace + ticket reduction (k = 37 has no useful divisor)."""
+    and batch 16 (R = 32) that bench.py's 0.8-of-HBM figure is taken on, plus forced splits on a small case, one shape
+    that must take the workspace + ticket reduction (k = 37 has no useful divisor), and clusters of 16 (the automatic
+    choice up to 4 rows: every CTA owns one head row of the reduction)."""
     _attn_case(cfg, sp, oracle, splits, want)
 
 

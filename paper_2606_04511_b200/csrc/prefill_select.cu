@@ -26,9 +26,13 @@
 // Columns beyond a row's causal candidates read as -inf, so the passes compare values only.  A row whose boundary
 // bucket holds more than 24 elements (heavy ties) takes an exact bitwise radix search over order-preserving keys in
 // part 0 alone (33 passes; warp-uniform because tcgen05.ld is warp-collective), which hands (T, id_T) to the others.
+// Chunk-sized calls run the replicated mode (32-row tiles, 16 threads per row, one 32-column chunk per thread): row_topk_repl
+// keeps the chunk in registers, searches on an fp16 image of it and exchanges through shared-memory atomics.
 // Scores never leave the SM.  a7' loops the same MMA over the G heads of the group, turns each head's accumulator
 // into softmax probabilities (two TMEM passes) summed into an L2-resident per-CTA scratch tile, and runs the same
 // selection on that tile.
+#include <cuda_fp16.h>
+
 #include "sparda_internal.cuh"
 
 #ifdef SPARDA_TRACE
@@ -74,7 +78,9 @@ struct PfSmem {
     static constexpr int OFF_NLIST = OFF_COMB + 2 * PF_NP * PF_ROWS * 8;      // boundary-list length per row
     static constexpr int OFF_CCNT = OFF_NLIST + PF_ROWS * 4;                  // selected count per (chunk, row), u8
     static constexpr int OFF_BAR = (OFF_CCNT + (PF_MAXN / 32) * PF_ROWS + 7) & ~7;
-    static constexpr int TOTAL = OFF_BAR + 64 + 1024;            // + slack for 1024-byte alignment
+    static constexpr int OFF_CELL = (OFF_BAR + 64 + 15) & ~15;                // replicated mode: [PF_NCELL][32 rows] u32 exchange cells
+    static constexpr int OFF_CNT16 = OFF_CELL + 8 * 32 * 4;                   // replicated mode: [32 rows][16 chunks] selected counts, u8
+    static constexpr int TOTAL = OFF_CNT16 + 32 * 16 + 1024;     // + slack for 1024-byte alignment
 };
 
 struct PfParams {
@@ -406,6 +412,242 @@ __device__ __forceinline__ void row_topk(const Src& src, int ncand, int nch, int
     }
 }
 
+// ---- replicated mode (chunk launches): 16 threads per query row, ONE 32-column chunk per thread.  The chunk is read from
+// TMEM once and stays in registers; the bucket search runs on a monotone fp16 image of it, two elements per instruction
+// (HSET2 + HADD2); the 16 parts of a row combine their partial results by shared-memory atomics on one cell per (exchange,
+// row) -- lanes of a warp hit 32 different cells, so an exchange is one conflict-free atomic per warp, one CTA barrier and
+// one load per thread instead of one store and 16 loads.  Same result as row_topk: the k largest by (value desc, id asc),
+// ids ascending.  Any monotone bucket map keeps the selection exact: an element of a higher bucket is larger than every
+// element of a lower one, and the boundary bucket is ranked on the fp32 values.
+constexpr int PF_NCELL = 8;                 // 0 min, 1 max, 2..5 search steps, 6 T, 7 id_T
+constexpr int PF_SSTRIDE = PF_MAXK + 1;     // words per row of the shared-memory output tile (odd: rows fall into different banks)
+__device__ __forceinline__ uint32_t pf_cell_init(int i) { return i == 0 ? 0xFFFFFFFFu : i == 6 ? 0xFF800000u /* -inf */ : i == 7 ? 0xFFFFFFFFu /* -1 */ : 0u; }
+
+template <class Src>
+__device__ __forceinline__ void row_topk_repl(const Src& src, int ncand, int nch, int k, bool active, int part,
+                                              uint32_t* cell /* this row's column of the [PF_NCELL][32] cells */,
+                                              uint8_t* cnt16 /* this row's 16 chunk counts, 16-byte aligned */,
+                                              uint32_t* list /* row's list, stride PF_WSTRIDE */, uint32_t* n_list,
+                                              int32_t* stage_row /* this row's k ids in the shared-memory output tile */) {
+    constexpr int NP = 16;
+    const float NEG = -INFINITY;
+    auto sync = [] { asm volatile("bar.sync 1, 512;" ::: "memory"); };
+    if (!active) ncand = 0;
+    const bool has = part < nch;            // warp-uniform (the parts are warps)
+    const int base = part * 32;
+    float v[32];
+    bool ragged = false;                    // the chunk reaches beyond some row's candidates (warp-uniform)
+    // ---- the chunk, once; columns beyond the row's candidates read as -inf; row min / max over the candidates
+    float lo = INFINITY, hi = NEG;
+    if (has) {
+        src.load(part, v);
+        ragged = __any_sync(0xffffffffu, base + 32 > ncand);
+        if (ragged) {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const bool ok = base + e < ncand;
+                lo = fminf(lo, ok ? v[e] : INFINITY);
+                v[e] = ok ? v[e] : NEG;
+                hi = fmaxf(hi, v[e]);
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) { lo = fminf(lo, v[e]); hi = fmaxf(hi, v[e]); }
+        }
+        if (base < ncand) {
+            atomicMin(cell + 0 * 32, orderable(lo + 0.0f));
+            atomicMax(cell + 1 * 32, orderable(hi + 0.0f));
+        }
+    }
+    sync();
+    PF_TRACE(2);
+    lo = key_to_float(cell[0 * 32]);
+    hi = key_to_float(cell[1 * 32]);
+    // ---- fp16 image: x = (v - lo) * 256 / (hi - lo) in [0, 256], -1 beyond the candidates; bucket b = [b, b + 1)
+    const float scale = hi > lo ? 256.0f / (hi - lo) : 0.f;
+    const float off = -lo * scale;
+    __half2 h[16];
+    if (has) {
+#pragma unroll
+        for (int w = 0; w < 16; ++w) {
+            float x0 = fmaxf(fmaf(v[2 * w], scale, off), 0.f), x1 = fmaxf(fmaf(v[2 * w + 1], scale, off), 0.f);
+            if (ragged) { x0 = v[2 * w] == NEG ? -1.f : x0; x1 = v[2 * w + 1] == NEG ? -1.f : x1; }
+            h[w] = __floats2half2_rn(x0, x1);
+        }
+    } else {
+#pragma unroll
+        for (int w = 0; w < 16; ++w) h[w] = __float2half2_rn(-1.f);
+    }
+    // ---- bucket search, three thresholds per step over 256 buckets: the largest bucket edge t with count(x >= t) >= k
+    int blo = 0, bhi = 256;                 // count(x >= blo) >= k > count(x >= bhi)
+    int c_lo = ncand, c_hi = 0;
+#pragma unroll 1
+    for (int step = 0; step < 4; ++step) {
+        const int q = (bhi - blo) >> 2;
+        const __half2 t1 = __float2half2_rn((float)(blo + q)), t2 = __float2half2_rn((float)(blo + 2 * q)), t3 = __float2half2_rn((float)(blo + 3 * q));
+        __half2 a1 = __float2half2_rn(0.f), a2 = a1, a3 = a1;
+#pragma unroll
+        for (int w = 0; w < 16; ++w) {
+            a1 = __hadd2(a1, __hge2(h[w], t1));
+            a2 = __hadd2(a2, __hge2(h[w], t2));
+            a3 = __hadd2(a3, __hge2(h[w], t3));
+        }
+        if (has) {
+            const int n1 = (int)(__low2float(a1) + __high2float(a1)), n2 = (int)(__low2float(a2) + __high2float(a2)),
+                      n3 = (int)(__low2float(a3) + __high2float(a3));
+            // three counts <= 512 each in one word: the sum over the parts cannot carry between the 10-bit fields
+            atomicAdd(cell + (2 + step) * 32, (uint32_t)(n1 | (n2 << 10) | (n3 << 20)));
+        }
+        sync();
+        const int packed = (int)cell[(2 + step) * 32];
+        const int c1 = packed & 1023, c2 = (packed >> 10) & 1023, c3 = (packed >> 20) & 1023;
+        if (c3 >= k) { blo += 3 * q; c_lo = c3; }
+        else if (c2 >= k) { blo += 2 * q; bhi = blo + q; c_lo = c2; c_hi = c3; }
+        else if (c1 >= k) { blo += q; bhi = blo + q; c_lo = c1; c_hi = c2; }
+        else { bhi = blo + q; c_hi = c1; }
+        PF_TRACE(3 + step);
+    }
+    const int need = k - c_hi;              // how many of the boundary bucket are selected (>= 1)
+    const int n_b = c_lo - c_hi;            // population of the boundary bucket
+    const bool slow = active && (n_b > PF_CAP);
+    // ---- collect the boundary bucket [blo, bhi) (any order; entries carry their fp32 value and id): a bit per element, one
+    // atomic per thread for its slots in the row's list, then the (few) set bits are written out
+    if (has) {
+        const __half2 hb = __float2half2_rn((float)blo), hb1 = __float2half2_rn(bhi == 256 ? INFINITY : (float)bhi);
+        uint32_t bits = 0;
+#pragma unroll
+        for (int w = 0; w < 16; ++w) {
+            const unsigned m = __hge2_mask(h[w], hb) & __hlt2_mask(h[w], hb1);
+            bits |= ((m & 1u) | ((m >> 15) & 2u)) << (2 * w);
+        }
+        if (bits != 0u && !slow) {          // not slow: the bucket's n_b <= PF_CAP members all fit
+            uint32_t* slot = list + 2 * PF_WSTRIDE * atomicAdd(n_list, (uint32_t)__popc(bits));
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                if ((bits >> e) & 1u) {
+                    slot[0] = __float_as_uint(v[e]);
+                    slot[PF_WSTRIDE] = (uint32_t)(base + e);
+                    slot += 2 * PF_WSTRIDE;
+                }
+            }
+        }
+    }
+    sync();
+    PF_TRACE(10);
+    if (part == 0) {                        // the min / max / search cells have been read by everybody: re-arm them for the next tile
+#pragma unroll
+        for (int i = 0; i < 6; ++i) cell[i * 32] = pf_cell_init(i);
+    }
+    // ---- the need-th largest of the list by (value desc, id asc): part p ranks the members p, p + 16, ...; exactly one
+    // finds it and publishes (T, id_T)
+    if (active && !slow) {
+        for (int e = part; e < n_b; e += NP) {
+            const float se = __uint_as_float(list[(2 * e) * PF_WSTRIDE]);
+            const int je = (int)list[(2 * e + 1) * PF_WSTRIDE];
+            int rank = 0;
+            int f = 0;
+            for (; f + 4 <= n_b; f += 4) {           // four independent loads in flight
+                float sf[4];
+                int jf[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    sf[u] = __uint_as_float(list[(2 * (f + u)) * PF_WSTRIDE]);
+                    jf[u] = (int)list[(2 * (f + u) + 1) * PF_WSTRIDE];
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) rank += (sf[u] > se || (sf[u] == se && jf[u] < je)) ? 1 : 0;
+            }
+            for (; f < n_b; ++f) {
+                const float sf = __uint_as_float(list[(2 * f) * PF_WSTRIDE]);
+                const int jf = (int)list[(2 * f + 1) * PF_WSTRIDE];
+                rank += (sf > se || (sf == se && jf < je)) ? 1 : 0;
+            }
+            if (rank == need - 1) { cell[6 * 32] = __float_as_uint(se); cell[7 * 32] = (uint32_t)je; }
+        }
+    }
+    // ---- heavy ties (rare): part 0 alone searches the k-th largest order-preserving key bit by bit over all chunks and
+    // finds the id of the last equal it takes.  Warp-uniform, and the same in every warp (they hold the same rows).
+    if (__any_sync(0xffffffffu, slow)) {
+        if (part == 0) {
+            float u[32];
+            uint32_t tk = 0;
+#pragma unroll 1
+            for (int bit = 31; bit >= 0; --bit) {
+                const uint32_t cand = tk | (1u << bit);
+                int cnt = 0;
+                for (int c = 0; c < nch; ++c) {
+                    src.load(c, u);
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) cnt += (c * 32 + e < ncand && orderable(u[e] + 0.0f) >= cand) ? 1 : 0;
+                }
+                if (cnt >= k) tk = cand;
+            }
+            int cgt = 0;
+            for (int c = 0; c < nch; ++c) {
+                src.load(c, u);
+#pragma unroll
+                for (int e = 0; e < 32; ++e) cgt += (c * 32 + e < ncand && orderable(u[e] + 0.0f) > tk) ? 1 : 0;
+            }
+            int eq_left = k - cgt, j_last = -1;       // take the first k - cgt equals in ascending id
+            for (int c = 0; c < nch; ++c) {
+                src.load(c, u);
+#pragma unroll
+                for (int e = 0; e < 32; ++e)
+                    if (c * 32 + e < ncand && orderable(u[e] + 0.0f) == tk && eq_left > 0) { j_last = c * 32 + e; --eq_left; }
+            }
+            if (slow) { cell[6 * 32] = __float_as_uint(key_to_float(tk)); cell[7 * 32] = (uint32_t)j_last; }
+        }
+    }
+    sync();
+    PF_TRACE(11);
+    const float T = __uint_as_float(cell[6 * 32]);    // k-th largest value (-inf: nothing to select)
+    const int jT = (int)cell[7 * 32];                 // selected among s == T: ids <= jT
+    // ---- selected element: s > T, or s == T with id <= jT.  Count per chunk, exchange, then every chunk writes its ids at
+    // its offset of the row's output: ascending ids
+    // counted on the FP32 pipe (FSET + FADD; the integer pipe has half its rate); the equals of T are rare: 0 or 1 per row
+    int n = 0, eT = -1;                     // eT: elements e <= eT of this chunk equal to T are selected
+    if (has) {
+        float ngt = 0.f, neq = 0.f;
+#pragma unroll
+        for (int e = 0; e < 32; ++e) {
+            ngt += v[e] > T ? 1.0f : 0.0f;
+            neq += v[e] == T ? 1.0f : 0.0f;
+        }
+        n = (int)ngt;
+        eT = jT - base;
+        if (neq != 0.f) {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) n += (v[e] == T && e <= eT) ? 1 : 0;
+        }
+    }
+    cnt16[part] = (uint8_t)n;
+    sync();
+    PF_TRACE(12);
+    if (part == 0) {                        // everybody holds (T, id_T) and has ranked: re-arm for the next tile
+        cell[6 * 32] = pf_cell_init(6);
+        cell[7 * 32] = pf_cell_init(7);
+        *n_list = 0;
+    }
+    // every chunk puts its ids at its offset of the row's k slots in a shared-memory tile (the list area is free by now;
+    // row stride 65 words: the 32 rows of a warp fall into different banks); the tile then leaves in coalesced stores
+    if (has && n > 0) {
+        const uint4 c4 = *reinterpret_cast<const uint4*>(cnt16);
+        const uint32_t cw[4] = {c4.x, c4.y, c4.z, c4.w};
+        unsigned upos = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {       // bytes of the chunks before this one
+            const int nb = min(max(part - 4 * i, 0), 4);
+            const uint32_t mask = nb >= 4 ? 0xFFFFFFFFu : ((1u << (8 * nb)) - 1u);
+            upos = __dp4a(cw[i] & mask, 0x01010101u, upos);
+        }
+        int32_t* out = stage_row + (int)upos;   // n <= k - upos: the row's counts add up to exactly k
+#pragma unroll
+        for (int e = 0; e < 32; ++e) {
+            if (v[e] > T || (v[e] == T && e <= eT)) *out++ = base + e;
+        }
+    }
+}
+
 // REPL (chunk launches with few tiles): a CTA owns 32 query rows instead of 128.  Its A tile holds the same 32 rows four
 // times (four 32-row TMA boxes), so the four TMEM lane quadrants carry four copies of the rows' scores and ALL 16 epilogue
 // warps work on those 32 rows, 16 threads per row (chunk c -> part c % 16).  The contraction is done four times over --
@@ -446,6 +688,11 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
         tma_prefetch_desc(&tmapB);
     }
     if (warp == 1) tmem_alloc(tmem_slot, PF_MAXN);
+    if (REPL) {   // exchange cells of row_topk_repl, armed for the first tile (the function re-arms them for the next)
+        uint32_t* cells = reinterpret_cast<uint32_t*>(smem + SM::OFF_CELL);
+        for (int i = tid; i < PF_NCELL * 32; i += PF_THREADS) cells[i] = pf_cell_init(i >> 5);
+        if (tid < 32) reinterpret_cast<uint32_t*>(smem + SM::OFF_NLIST)[tid] = 0;
+    }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -464,6 +711,18 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     };
     const int n_rounds = (p.n_tiles + n_cta - 1) / n_cta;
     auto tile_ncols = [&](int mt) -> int { return min(p.n_blocks, (mt * TROWS + TROWS) / 64); };  // visible blocks of the tile's last row
+
+    // replicated mode: the tile's ids leave the shared-memory tile in coalesced stores (the ranked rows only; the others are
+    // filled directly).  Called by all 16 epilogue warps.
+    auto repl_store_tile = [&](const int32_t* stage, const PfParams& pp, int grp, int mt) {
+        asm volatile("bar.sync 1, 512;" ::: "memory");
+        const int row = (tid - 64) >> 4, c0 = (tid - 64) & 15;   // 16 threads per row, 64-byte runs
+        const int i = mt * 32 + row;
+        if (i >= pp.row0 && i < pp.row0 + pp.n_rows && min(pp.n_blocks, (i + 1) / 64) > pp.topk) {
+            int32_t* drow = pp.ids + ((size_t)grp * pp.n_rows + (i - pp.row0)) * pp.topk;
+            for (int c = c0; c < pp.topk; c += 16) drow[c] = stage[row * PF_SSTRIDE + c];
+        }
+    };
 
     if (warp == 0) {
         // =============================== TMA producer ===============================
@@ -593,15 +852,29 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     __syncwarp();
                     if (lane == 0) mbar_arrive(tmem_empty);
                 }
-                if (__any_sync(0xffffffffu, ranked))
-                    row_topk<REPL ? 2 : 1>(ScratchRow{scr}, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, dst);
+                if (__any_sync(0xffffffffu, ranked)) {
+                    if constexpr (REPL) {
+                        int32_t* stage = reinterpret_cast<int32_t*>(smem + SM::OFF_LIST);
+                        row_topk_repl(ScratchRow{scr}, ncand, nch, p.topk, ranked, part, reinterpret_cast<uint32_t*>(smem + SM::OFF_CELL) + trow,
+                                      smem + SM::OFF_CNT16 + trow * 16, list, n_list, stage + trow * PF_SSTRIDE);
+                        repl_store_tile(stage, p, g, mt);
+                    } else
+                        row_topk<1>(ScratchRow{scr}, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, dst);
+                }
             } else {
                 mbar_wait_backoff(mma_done, it & 1, 100);
                 ++it;
                 tc_fence_after();
                 PF_TRACE(1);
-                if (__any_sync(0xffffffffu, ranked))
-                    row_topk<REPL ? 2 : 1>(trsrc, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, dst);
+                if (__any_sync(0xffffffffu, ranked)) {
+                    if constexpr (REPL) {
+                        int32_t* stage = reinterpret_cast<int32_t*>(smem + SM::OFF_LIST);
+                        row_topk_repl(trsrc, ncand, nch, p.topk, ranked, part, reinterpret_cast<uint32_t*>(smem + SM::OFF_CELL) + trow,
+                                      smem + SM::OFF_CNT16 + trow * 16, list, n_list, stage + trow * PF_SSTRIDE);
+                        repl_store_tile(stage, p, g, mt);
+                    } else
+                        row_topk<1>(trsrc, ncand, nch, p.topk, ranked, pc, list, n_list, chunk_cnt, dst);
+                }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(tmem_empty);

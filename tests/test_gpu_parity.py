@@ -758,6 +758,34 @@ def test_prefill_select_baseline(cfg, sp, oracle):
         _check_prefill_rows(ids.cpu().numpy(), want, s, row0)
 
 
+def test_prefill_select_one_launch_128_row_tiles(sp, oracle):
+    """The whole-sequence launch (bench.py's `forecast_us_one_launch`): from about one 128-row tile per SM on, the kernel
+    runs 128-row tiles with 4 threads per row instead of the replicated 32-row tiles every chunk-sized call takes.  Sampled
+    windows against the oracle (incl. rows of all-equal scores: the exact bitwise search), properties on every row."""
+    cfg = synth.PrefillConfig("pf_one", n_q_heads=32, n_kv_heads=2, head_dim=128, seq_len=8192 + 100, topk=64, seed=55)
+    P, ctx, kpool = _prefill_setup(cfg, sp)
+    T, k, Hkv = cfg.seq_len, cfg.topk, cfg.n_kv_heads
+    assert 4 * ((T + 127) // 128) * Hkv > 3 * torch.cuda.get_device_properties(0).multi_processor_count   # not the replicated mode
+    F = P["F"].clone()
+    F[0, 6000:6040] = 0                                           # all scores 0 -> ids 0..k-1 (heavy ties)
+    ids = torch.full((Hkv, T, k), -7, dtype=torch.int32, device="cuda")
+    ctx.prefill_select(F, kpool, T, cfg.n_blocks, 0, T, k, ids)
+    torch.cuda.synchronize()
+    got = ids.cpu().numpy()
+    kp_bits, F_bits = _bits(kpool), _bits(F)
+    for row0, n in [(0, 200), (4090, 120), (5990, 60), (T - 150, 150)]:
+        want, s = oracle.prefill_select(F_bits, kp_bits, k, row0, n, want_scores=True)
+        _check_prefill_rows(got[:, row0:row0 + n], want, s, row0)
+    assert np.all(got[0, 6010] == np.arange(k))
+    valid = got >= 0
+    ncand = np.minimum(cfg.n_blocks, (np.arange(T) + 1) // 64)
+    assert np.array_equal(valid.sum(-1), np.broadcast_to(np.minimum(ncand, k), (Hkv, T)))
+    assert np.all(np.where(valid, got, -1).max(-1) < np.maximum(ncand, 1)[None, :])
+    d = np.diff(np.where(valid, got, np.iinfo(np.int32).max).astype(np.int64), axis=-1)
+    assert np.all(d[valid[..., 1:]] > 0)
+    ctx.close()
+
+
 def test_cfg5_full_size_prefill_sampled(sp, oracle):
     """BASELINE.json configs[4] at full size (T = 32768, 512 blocks, top-64, 2 groups) in 2048-row chunks as bench.py
     launches it; the oracle checks sampled row windows (it needs ~1 s per 100 rows at this size)."""

@@ -464,6 +464,7 @@ def bench_prefill(torch, binding, peaks_all, ncu, ncu_src):
     bf16_peak = peaks_all.get("bf16_tflops_sustained") or peaks_all.get("bf16_tflops") or 1400.0
     ranked_rows = Hkv * sum(1 for i in range(T) if (i + 1) // 64 > k)
     inst = ncu.get("prefill_one", {}).get("smsp__inst_executed.sum")
+    inst_c = ncu.get("prefill_chunked_pass", {}).get("smsp__inst_executed.sum")
     alu_peak = 148 * 4 * 1.965                                     # G warp-instr/s: 148 SMs x 4 schedulers x 1 per clock x 1.965 GHz
     out = {
         "shape": f"{cfg.name}: T={T}, {Hkv} groups, {Nb} pooled keys, top-{k}, {cfg.chunk}-row chunks",
@@ -477,6 +478,10 @@ def bench_prefill(torch, binding, peaks_all, ncu, ncu_src):
                 "warp_instructions": inst, "achieved": round(inst / t_one / 1e9, 1) if inst else None, "peak": round(alu_peak, 1),
                 "unit": "G warp-instr/s", "frac": round(inst / t_one / 1e9 / alu_peak, 4) if inst else None,
                 "traffic_src": ncu_src if inst else None},
+        "alu_chunked": {"kernel": "prefill_select_kernel<128,false,true> (16 chunk launches, replicated 32-row tiles)", "bound": "alu",
+                        "us": round(t_chunk * 1e6, 2), "warp_instructions": inst_c, "achieved": round(inst_c / t_chunk / 1e9, 1) if inst_c else None,
+                        "peak": round(alu_peak, 1), "unit": "G warp-instr/s", "frac": round(inst_c / t_chunk / 1e9 / alu_peak, 4) if inst_c else None,
+                        "traffic_src": ncu_src if inst_c else None},
     }
     ctx.close()
     return out

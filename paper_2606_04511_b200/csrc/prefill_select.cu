@@ -80,7 +80,8 @@ struct PfSmem {
     static constexpr int OFF_BAR = (OFF_CCNT + (PF_MAXN / 32) * PF_ROWS + 7) & ~7;
     static constexpr int OFF_CELL = (OFF_BAR + 64 + 15) & ~15;                // replicated mode: [PF_NCELL][32 rows] u32 exchange cells
     static constexpr int OFF_CNT16 = OFF_CELL + 8 * 32 * 4;                   // replicated mode: [32 rows][16 chunks] selected counts, u8
-    static constexpr int TOTAL = OFF_CNT16 + 32 * 16 + 1024;     // + slack for 1024-byte alignment
+    static constexpr int OFF_STAGE = OFF_CNT16 + 32 * 16;                     // replicated mode: [32 rows][65] ids on their way out
+    static constexpr int TOTAL = OFF_STAGE + 32 * 65 * 4 + 1024; // + slack for 1024-byte alignment
 };
 
 struct PfParams {
@@ -464,14 +465,18 @@ __device__ __forceinline__ void row_topk_repl(const Src& src, int ncand, int nch
     lo = key_to_float(cell[0 * 32]);
     hi = key_to_float(cell[1 * 32]);
     // ---- fp16 image: x = (v - lo) * 256 / (hi - lo) in [0, 256], -1 beyond the candidates; bucket b = [b, b + 1)
-    const float scale = hi > lo ? 256.0f / (hi - lo) : 0.f;
+    const float scale = hi > lo ? __fdividef(256.0f, hi - lo) : 0.f;   // any scale keeps the bucket map monotone
     const float off = -lo * scale;
     __half2 h[16];
-    if (has) {
+    if (has && !ragged) {
+#pragma unroll
+        for (int w = 0; w < 16; ++w)
+            h[w] = __floats2half2_rn(fmaxf(fmaf(v[2 * w], scale, off), 0.f), fmaxf(fmaf(v[2 * w + 1], scale, off), 0.f));
+    } else if (has) {
 #pragma unroll
         for (int w = 0; w < 16; ++w) {
-            float x0 = fmaxf(fmaf(v[2 * w], scale, off), 0.f), x1 = fmaxf(fmaf(v[2 * w + 1], scale, off), 0.f);
-            if (ragged) { x0 = v[2 * w] == NEG ? -1.f : x0; x1 = v[2 * w + 1] == NEG ? -1.f : x1; }
+            const float x0 = v[2 * w] == NEG ? -1.f : fmaxf(fmaf(v[2 * w], scale, off), 0.f);
+            const float x1 = v[2 * w + 1] == NEG ? -1.f : fmaxf(fmaf(v[2 * w + 1], scale, off), 0.f);
             h[w] = __floats2half2_rn(x0, x1);
         }
     } else {
@@ -510,6 +515,20 @@ __device__ __forceinline__ void row_topk_repl(const Src& src, int ncand, int nch
     const int need = k - c_hi;              // how many of the boundary bucket are selected (>= 1)
     const int n_b = c_lo - c_hi;            // population of the boundary bucket
     const bool slow = active && (n_b > PF_CAP);
+    const bool any_slow = __any_sync(0xffffffffu, slow);   // the same in every warp: they hold the same rows
+    // ---- elements above the boundary bucket, per chunk: with the selected members of the boundary list they give every
+    // chunk's offset in the row's output without another exchange
+    {
+        int above = 0;
+        if (has && bhi < 256) {
+            const __half2 tb = __float2half2_rn((float)bhi);
+            __half2 a = __float2half2_rn(0.f);
+#pragma unroll
+            for (int w = 0; w < 16; ++w) a = __hadd2(a, __hge2(h[w], tb));
+            above = (int)(__low2float(a) + __high2float(a));
+        }
+        cnt16[part] = (uint8_t)above;
+    }
     // ---- collect the boundary bucket [blo, bhi) (any order; entries carry their fp32 value and id): a bit per element, one
     // atomic per thread for its slots in the row's list, then the (few) set bits are written out
     if (has) {
@@ -567,7 +586,7 @@ __device__ __forceinline__ void row_topk_repl(const Src& src, int ncand, int nch
     }
     // ---- heavy ties (rare): part 0 alone searches the k-th largest order-preserving key bit by bit over all chunks and
     // finds the id of the last equal it takes.  Warp-uniform, and the same in every warp (they hold the same rows).
-    if (__any_sync(0xffffffffu, slow)) {
+    if (any_slow) {
         if (part == 0) {
             float u[32];
             uint32_t tk = 0;
@@ -602,35 +621,21 @@ __device__ __forceinline__ void row_topk_repl(const Src& src, int ncand, int nch
     PF_TRACE(11);
     const float T = __uint_as_float(cell[6 * 32]);    // k-th largest value (-inf: nothing to select)
     const int jT = (int)cell[7 * 32];                 // selected among s == T: ids <= jT
-    // ---- selected element: s > T, or s == T with id <= jT.  Count per chunk, exchange, then every chunk writes its ids at
-    // its offset of the row's output: ascending ids
-    // counted on the FP32 pipe (FSET + FADD; the integer pipe has half its rate); the equals of T are rare: 0 or 1 per row
-    int n = 0, eT = -1;                     // eT: elements e <= eT of this chunk equal to T are selected
+    // ---- selected element: s > T, or s == T with id <= jT.  Every chunk writes its ids at its offset of the row's k slots
+    // in a shared-memory tile (row stride 65 words: the 32 rows of a warp fall into different banks), ascending ids; the
+    // tile then leaves in coalesced stores.  Offset of chunk p = elements above the boundary bucket in the chunks before it
+    // + selected members of the boundary list with smaller ids.
+    const int eT = jT - base;               // elements e <= eT of this chunk equal to T are selected
+    if (any_slow) {                         // a row of the tile resolved heavy ties without a list: exchange exact counts (rare)
+        int n = 0;
+        if (has) {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) n += (v[e] > T || (v[e] == T && e <= eT)) ? 1 : 0;
+        }
+        cnt16[part] = (uint8_t)n;
+        sync();
+    }
     if (has) {
-        float ngt = 0.f, neq = 0.f;
-#pragma unroll
-        for (int e = 0; e < 32; ++e) {
-            ngt += v[e] > T ? 1.0f : 0.0f;
-            neq += v[e] == T ? 1.0f : 0.0f;
-        }
-        n = (int)ngt;
-        eT = jT - base;
-        if (neq != 0.f) {
-#pragma unroll
-            for (int e = 0; e < 32; ++e) n += (v[e] == T && e <= eT) ? 1 : 0;
-        }
-    }
-    cnt16[part] = (uint8_t)n;
-    sync();
-    PF_TRACE(12);
-    if (part == 0) {                        // everybody holds (T, id_T) and has ranked: re-arm for the next tile
-        cell[6 * 32] = pf_cell_init(6);
-        cell[7 * 32] = pf_cell_init(7);
-        *n_list = 0;
-    }
-    // every chunk puts its ids at its offset of the row's k slots in a shared-memory tile (the list area is free by now;
-    // row stride 65 words: the 32 rows of a warp fall into different banks); the tile then leaves in coalesced stores
-    if (has && n > 0) {
         const uint4 c4 = *reinterpret_cast<const uint4*>(cnt16);
         const uint32_t cw[4] = {c4.x, c4.y, c4.z, c4.w};
         unsigned upos = 0;
@@ -640,12 +645,29 @@ __device__ __forceinline__ void row_topk_repl(const Src& src, int ncand, int nch
             const uint32_t mask = nb >= 4 ? 0xFFFFFFFFu : ((1u << (8 * nb)) - 1u);
             upos = __dp4a(cw[i] & mask, 0x01010101u, upos);
         }
-        int32_t* out = stage_row + (int)upos;   // n <= k - upos: the row's counts add up to exactly k
+        if (!any_slow && active) {
+            for (int f0 = 0; f0 < n_b; f0 += 4) {     // four independent pairs of loads in flight; entries >= n_b are never counted
+                float sf[4];
+                int jf[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int f = min(f0 + u, PF_CAP - 1);
+                    sf[u] = __uint_as_float(list[(2 * f) * PF_WSTRIDE]);
+                    jf[u] = (int)list[(2 * f + 1) * PF_WSTRIDE];
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    upos += (f0 + u < n_b && jf[u] < base && (sf[u] > T || (sf[u] == T && jf[u] <= jT))) ? 1u : 0u;
+            }
+        }
+        PF_TRACE(14);
+        int32_t* out = stage_row + (int)upos;
 #pragma unroll
         for (int e = 0; e < 32; ++e) {
             if (v[e] > T || (v[e] == T && e <= eT)) *out++ = base + e;
         }
     }
+    PF_TRACE(15);
 }
 
 // REPL (chunk launches with few tiles): a CTA owns 32 query rows instead of 128.  Its A tile holds the same 32 rows four
@@ -716,6 +738,13 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     // filled directly).  Called by all 16 epilogue warps.
     auto repl_store_tile = [&](const int32_t* stage, const PfParams& pp, int grp, int mt) {
         asm volatile("bar.sync 1, 512;" ::: "memory");
+        PF_TRACE(16);
+        if (tid - 64 < 32) {                // everybody has read (T, id_T) and the list: re-arm them for the next tile
+            uint32_t* cells = reinterpret_cast<uint32_t*>(smem + SM::OFF_CELL) + (tid - 64);
+            cells[6 * 32] = pf_cell_init(6);
+            cells[7 * 32] = pf_cell_init(7);
+            reinterpret_cast<uint32_t*>(smem + SM::OFF_NLIST)[tid - 64] = 0;
+        }
         const int row = (tid - 64) >> 4, c0 = (tid - 64) & 15;   // 16 threads per row, 64-byte runs
         const int i = mt * 32 + row;
         if (i >= pp.row0 && i < pp.row0 + pp.n_rows && min(pp.n_blocks, (i + 1) / 64) > pp.topk) {
@@ -727,7 +756,9 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     if (warp == 0) {
         // =============================== TMA producer ===============================
         if (lane == 0) {
-            const int nb_boxes = (p.n_blocks + 255) / 256;
+            // causal truncation of the B operand too: this CTA's tiles see at most the columns of its first (highest) tile
+            const int mt0 = tile_of_round(0);
+            const int nb_boxes = mt0 < 0 ? 1 : (tile_ncols(mt0) + 255) / 256;
             mbar_arrive_expect_tx(b_full, (uint32_t)(KH * nb_boxes * 256 * 128));
             for (int kh = 0; kh < KH; ++kh)
                 for (int nh = 0; nh < nb_boxes; ++nh)
@@ -854,7 +885,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 }
                 if (__any_sync(0xffffffffu, ranked)) {
                     if constexpr (REPL) {
-                        int32_t* stage = reinterpret_cast<int32_t*>(smem + SM::OFF_LIST);
+                        int32_t* stage = reinterpret_cast<int32_t*>(smem + SM::OFF_STAGE);
                         row_topk_repl(ScratchRow{scr}, ncand, nch, p.topk, ranked, part, reinterpret_cast<uint32_t*>(smem + SM::OFF_CELL) + trow,
                                       smem + SM::OFF_CNT16 + trow * 16, list, n_list, stage + trow * PF_SSTRIDE);
                         repl_store_tile(stage, p, g, mt);
@@ -868,7 +899,7 @@ prefill_select_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 PF_TRACE(1);
                 if (__any_sync(0xffffffffu, ranked)) {
                     if constexpr (REPL) {
-                        int32_t* stage = reinterpret_cast<int32_t*>(smem + SM::OFF_LIST);
+                        int32_t* stage = reinterpret_cast<int32_t*>(smem + SM::OFF_STAGE);
                         row_topk_repl(trsrc, ncand, nch, p.topk, ranked, part, reinterpret_cast<uint32_t*>(smem + SM::OFF_CELL) + trow,
                                       smem + SM::OFF_CNT16 + trow * 16, list, n_list, stage + trow * PF_SSTRIDE);
                         repl_store_tile(stage, p, g, mt);

@@ -176,3 +176,48 @@ def test_captured_cached_step_replays_with_poisoned_pools(sp, oracle):
                 if a.dtype == torch.bfloat16:
                     a, b = a.view(torch.int16), b.view(torch.int16)
                 assert torch.equal(a, b), f"replay {rep} layer {l} {n}"
+
+
+def test_prefill_select_random_chunks_against_oracle(sp, oracle):
+    """40 random chunk calls of the prefill selection (both tile modes, D, groups, k, ragged row ranges, several tiles per CTA),
+    with planted ties: duplicated pooled keys, rows of all-equal scores, few distinct score values (the exact bitwise
+    search), against o8.  The replicated mode re-arms its shared-memory exchange cells from tile to tile: every call here
+    runs more than one tile per CTA at least in one group."""
+    rng = np.random.default_rng(77)
+    g = torch.Generator(device="cuda").manual_seed(77)
+    band = rows = 0
+    for it in range(40):
+        D = int(rng.choice([64, 128]))
+        Hkv = int(rng.integers(1, 4))
+        Nb = int(rng.integers(3, 513))
+        T = Nb * 64 + int(rng.integers(0, 64))
+        k = int(rng.integers(1, min(64, Nb) + 1))
+        ctx = sp.Sparda(1, Hkv, Hkv, D, Nb, k)
+        kp = (torch.randn((Hkv, Nb, D), generator=g, device="cuda") + torch.randn((Hkv, Nb, 1), generator=g, device="cuda") * 1.5).to(torch.bfloat16)
+        F = torch.randn((Hkv, T, D), generator=g, device="cuda").to(torch.bfloat16)
+        n = int(rng.integers(1, min(T, 12000 if it % 8 == 0 else 3000) + 1))      # every 8th call is large enough for the 128-row tiles
+        row0 = int(rng.integers(0, T - n + 1))
+        if it % 3 == 0:
+            kp[:, Nb // 2:] = kp[:, : Nb - Nb // 2].clone()               # duplicated keys: exact ties, lower id first
+        if it % 4 == 0:
+            F[:, row0 + n // 2: row0 + n // 2 + 40] = 0                   # all scores equal
+        if it % 5 == 0:
+            F[0, row0: row0 + 64, 1:] = 0                                 # scores = F[.,0] * Kpool[j,0] with few distinct values
+            kp[0, :, 0] = (torch.arange(Nb, device="cuda") % 5).to(torch.bfloat16)
+        ids = torch.full((Hkv, n, k), -7, dtype=torch.int32, device="cuda")
+        ctx.prefill_select(F, kp, T, Nb, row0, n, k, ids)
+        torch.cuda.synchronize()
+        got = ids.cpu().numpy()
+        # the oracle on sampled windows of the chunk (its cost grows with T * Nb): the head, the tail, the tie rows
+        wins = {(0, min(n, 96)), (max(0, n - 96), min(n, 96)), (max(0, n // 2 - 8), min(n - max(0, n // 2 - 8), 64))}
+        for w0, wn in wins:
+            want, s = oracle.prefill_select(_bits(F), _bits(kp), k, row0 + w0, wn, want_scores=True)
+            for gi in range(Hkv):
+                ncand = np.minimum(Nb, (row0 + w0 + np.arange(wn) + 1) // 64)
+                band += parity.check_ids(got[gi, w0:w0 + wn], want[gi], s[gi], ncand)
+            rows += Hkv * wn
+        valid = got >= 0
+        ncand = np.minimum(Nb, (row0 + np.arange(n) + 1) // 64)
+        assert np.array_equal(valid.sum(-1), np.broadcast_to(np.minimum(ncand, k), (Hkv, n))), f"case {it}: wrong id count"
+        ctx.close()
+    print(f"prefill stress: {band} of {rows} checked rows used the near-tie band")

@@ -600,6 +600,41 @@ def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps, standin
         del graph
         out.append({"alpha": alpha if alpha < 1e8 else "independent", "rho": round(rho, 4), "ms_per_step": round(ms, 4),
                     "tok_s": round(cfg.batch / (ms * 1e-3), 1), "link_mib_per_step": round(rho * (NL - 1) * cfg.gather_bytes_per_layer / 2**20, 1)})
+    # Alg.2 l.1 inside the step (Eq.3): every layer hands X and W_F instead of a ready F, the projection kernel runs
+    # on the select chain in front of the select that reads F.  Same X every step: rho = 0, so this is the floor + l.1
+    proj_ms = None
+    if ctx.cfg.hidden:
+        hidden = ctx.cfg.hidden
+        X = torch.randn((cfg.batch, hidden), generator=g, device="cuda").to(torch.bfloat16)
+        wl = []
+        for l, e in enumerate(layers[0]):
+            w = {**e, "F": e["F"].clone(), "X": X, "WF": (torch.randn((hidden, cfg.n_kv_heads * D), generator=g, device="cuda") / hidden ** 0.5).to(torch.bfloat16)}
+            if l == 0:
+                w["WFcur"] = (torch.randn((hidden, cfg.n_kv_heads * D), generator=g, device="cuda") / hidden ** 0.5).to(torch.bfloat16)
+            wl.append(w)
+        arr_p = ctx.make_cached_layers(wl)
+        F0p = F0.clone()
+        for e in layers[0][1:]:
+            e["slot_ids"].fill_(-1)
+        for _ in range(3):
+            ctx.decode_step_cached(arr_p, F0p, Nb, k, cs, ps, binding.STEP_OVERLAP)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=cs):
+            for i in range(2):
+                ctx.decode_step_cached(arr_p, F0p, Nb, k, cs, ps, binding.STEP_OVERLAP)
+        graph.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n = max(4, steps - steps % 2)
+        with torch.cuda.stream(cs):
+            e0.record(cs)
+            for i in range(n // 2):
+                graph.replay()
+            e1.record(cs)
+        torch.cuda.synchronize()
+        proj_ms = round(e0.elapsed_time(e1) / n, 4)
+        del graph, wl, arr_p
     floor = out[0]["ms_per_step"]
     for o in out:
         o["gather_exposed_us_per_layer"] = round(max(0.0, (o["ms_per_step"] - floor) * 1e3 / (NL - 1)), 2)
@@ -612,7 +647,70 @@ def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps, standin
             "standin_bytes_per_layer": standin_bytes,
             "standin": "NOT part of the method: a kernel streaming 474 MB of weights after every attention" if standin_bytes else None,
             "compute_floor_ms_per_step": floor, "us_per_layer_at_floor": round(floor * 1e3 / NL, 2),
+            "compute_floor_with_in_step_projection_ms": proj_ms,
             "rho_hidden_up_to": hidden_up_to, "sweep": out}
+
+
+def bench_chain_under_load(torch, binding):
+    """What a kernel boundary costs on the select chain when the GPU is busy (the reason for the select -> gather doorbell of
+    sparda_decode_step): batch-4 shapes of configs[2], the kernels of the chain replayed from a CUDA graph (16 per graph,
+    rotating cold buffers) alone and while the labelled layer stand-in (NOT part of the method) saturates HBM on another
+    stream.  Stand-alone launches: the two-kernel chain here is stream-ordered, without the doorbell."""
+    from paper_2606_04511_b200 import synth
+    cfg = synth.CFG4_128K.with_(batch=4)
+    R, Nb, k, D = cfg.rows, cfg.n_blocks, cfg.topk, cfg.head_dim
+    g = torch.Generator(device="cuda").manual_seed(91)
+    ctx = binding.Sparda.from_config(cfg)
+    NS = 16
+    kpools = [torch.randn((R, Nb, D), generator=g, device="cuda").to(torch.bfloat16) for _ in range(NS)]
+    pools = [torch.randn((R, k, 2, 64, D), generator=g, device="cuda").to(torch.bfloat16) for _ in range(NS)]
+    F = torch.randn((R, D), generator=g, device="cuda").to(torch.bfloat16)
+    Q = torch.randn((cfg.batch, cfg.n_q_heads, D), generator=g, device="cuda").to(torch.bfloat16)
+    O = torch.empty_like(Q)
+    ids = torch.empty((R, k), dtype=torch.int32, device="cuda")
+    ids_a = torch.arange(k, dtype=torch.int32, device="cuda").repeat(R, 1).contiguous()
+    slot = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
+    fetch = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
+    empty = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
+    host = torch.empty((R, 8, 2, 64, D), dtype=torch.bfloat16, pin_memory=True)
+    pool = torch.empty((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda")
+    W = torch.empty(STANDIN_BYTES // 2, dtype=torch.bfloat16, device="cuda").fill_(1.0)
+    cs, xs = torch.cuda.Stream(), torch.cuda.Stream()
+    sel = lambda i: ctx.forecast_select_plan(F, kpools[i], Nb, k, ids, slot, fetch, stream=xs)
+    gat = lambda i: ctx.prefetch_launch(host, 8, empty, k, pool, stream=xs)
+    att = lambda i: ctx.sparse_decode(Q, pools[i], ids_a, k, O, stream=xs)
+    out = {}
+    for name, fn in (("select_plan", sel), ("gather_empty_list", gat), ("attention", att), ("select_plan_then_gather", lambda i: (sel(i), gat(i)))):
+        for i in range(NS):
+            fn(i)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=xs):
+            for i in range(NS):
+                fn(i)
+        graph.replay()
+        torch.cuda.synchronize()
+        for loaded in (False, True):
+            if loaded:
+                for _ in range(40):
+                    ctx.probe_launch(3, W, STANDIN_BYTES, stream=cs)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(xs):
+                e0.record(xs)
+                for _ in range(3):
+                    graph.replay()
+                e1.record(xs)
+            e1.synchronize()
+            still = not cs.query()
+            torch.cuda.synchronize()
+            out[name + ("_us_beside_hbm_load" if loaded else "_us_alone")] = round(e0.elapsed_time(e1) * 1e3 / (3 * NS), 2)
+            if loaded:
+                out.setdefault("load_on_throughout", True)
+                out["load_on_throughout"] = out["load_on_throughout"] and bool(still)
+        del graph
+    out["note"] = "per launch (per pair for the chain); the load is the layer stand-in streaming HBM on another stream: NOT part of the method"
+    ctx.close()
+    return out
 
 
 def bench_gather_sweep(torch, binding, peaks, ceiling, host_layer_b4):
@@ -782,7 +880,7 @@ def run_sparda(args):
     R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
 
     mode = binding.GATHER_TMA if args.gather_mode == "tma" else binding.GATHER_LDG
-    ctx = binding.Sparda.from_config(cfg, max_layers=NL, gather_ctas=args.gather_ctas, gather_mode=mode)
+    ctx = binding.Sparda.from_config(cfg, max_layers=NL, gather_ctas=args.gather_ctas, gather_mode=mode, hidden=4096)
 
     # ---- pinned host KV: as many distinct layers as the box can hold, layer l -> l mod resident otherwise
     import psutil
@@ -937,6 +1035,8 @@ def run_sparda(args):
         # exposed = step with every block fetched minus the step with nothing to fetch (the cached step at rho = 0)
         "gather_exposed_us_per_layer": (ms_per_step - floor_ms) * 1e3 / (NL - 1) if floor_ms else None,
         "compute_floor_ms_per_step": floor_ms}
+    if "standin" in sec:
+        roofline["kernel_boundary_under_load"] = bench_chain_under_load(torch, binding)
     roofline["reuse_cache"] = reuse
     roofline["reuse_cache_with_layer_standin"] = standin
     roofline["gather_sweep"] = gather_sweep

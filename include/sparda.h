@@ -182,7 +182,7 @@ int sparda_enable_peer_tier(sparda_ctx* ctx, int peer_device);
  *   pool_is_indexed = 0: dev_pool is [R][topk][2][S][D] and slot i holds block ids[r][i] (n_slots = topk);
  *   pool_is_indexed = 1: dev_pool is a device-resident cache [R][n_slots][2][S][D] addressed through ids
  *                        (layer 0).
- * Split-K flash-decode over a flat list of the R*topk slots.  Row-aligned splits with 2, 4 or 8 CTAs per row run as
+ * Split-K flash-decode over a flat list of the R*topk slots.  Row-aligned splits with 2, 4, 8 or 16 CTAs per row run as
  * one thread-block cluster per row and reduce their partials through distributed shared memory; any other split
  * reduces through the context's L2-resident workspace, merged by the last CTA of each row (ticket).
  * The workspace is shared by every launch on the context: at most ONE sparse_decode may be in flight per context at a
@@ -197,6 +197,10 @@ int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, c
  * into dev_pool[l & 1] on prefetch_stream and attended in layer l after an event wait.  The pool is
  * double-buffered: gather l+1 may start only after attention l-1 released its buffer.
  * mode = SPARDA_STEP_OVERLAP or SPARDA_STEP_SERIAL (same kernels on one stream; results are bit-identical).
+ * In overlap mode a layer's gather is launched together with its select and waits on the device for the select's
+ * doorbell (one counter per layer in the context's workspace, zeroed at the top of the step), so no kernel boundary
+ * sits between "block list out" and "first byte on the link"; a gather whose select never runs traps after ~15 s
+ * instead of hanging the device.  One step per context at a time.
  * Capturable into a CUDA graph (no host synchronisation, events are pre-created).                             */
 int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                        int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,

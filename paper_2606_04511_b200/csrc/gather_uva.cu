@@ -34,9 +34,11 @@ constexpr int GATHER_WIN = 1024;  // tasks compacted per window (32 per lane, he
 // first compacts the valid tasks of a window with ballots -- every CTA scans the whole window, CTA c takes the c-th
 // equal share of the VALID tasks, so the split is balanced whatever the pattern -- then lane 0 drives the bulk-copy
 // ring over its share.  An empty list costs one scan (a few microseconds), not one dependent load per slot.
+// door != nullptr (overlapped decode step): the launch is already resident when the layer's select runs; it waits for the
+// select's doorbell (n_rows rows published) instead of for a kernel boundary, and reads ids only after it.
 __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__ host_kv, const int32_t* __restrict__ ids,
                                                         char* __restrict__ pool, int n_rows, int n_blocks, int topk,
-                                                        uint32_t block_bytes) {
+                                                        uint32_t block_bytes, unsigned int* door) {
     extern __shared__ __align__(128) char ring[];
     __shared__ uint64_t full[GATHER_STAGES];
     __shared__ int32_t q_task[GATHER_WIN], q_id[GATHER_WIN];
@@ -50,6 +52,10 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
     __syncwarp();
     pdl_wait();                  // ids (and the pool's previous reader) belong to earlier kernels
     pdl_launch_dependents();
+    if (door) {
+        if (lane == 0) door_wait(door, (unsigned)n_rows);
+        __syncwarp();
+    }
     const uint32_t cpb = block_bytes / GATHER_STAGE_BYTES;  // 16 KiB chunks per block: 2 at D=128, 1 at D=64
     const int64_t n_tasks = (int64_t)n_rows * topk;
     const unsigned lt = (1u << lane) - 1u;
@@ -123,10 +129,14 @@ constexpr int LDG_UNIT_BYTES = LDG_UNROLL * 32 * 16;  // 4 KiB per warp-iteratio
 
 __global__ void __launch_bounds__(256) gather_ldg_kernel(const char* __restrict__ host_kv, const int32_t* __restrict__ ids,
                                                          char* __restrict__ pool, int n_rows, int n_blocks, int topk,
-                                                         uint32_t block_bytes) {
+                                                         uint32_t block_bytes, unsigned int* door) {
     const int lane = threadIdx.x & 31;
     pdl_wait();
     pdl_launch_dependents();
+    if (door) {
+        if (threadIdx.x == 0) door_wait(door, (unsigned)n_rows);
+        __syncthreads();
+    }
     const int64_t warp = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int64_t n_warps = (int64_t)gridDim.x * (blockDim.x >> 5);
     const uint32_t units_per_block = block_bytes / LDG_UNIT_BYTES;
@@ -153,6 +163,7 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
                          cudaStream_t st) {
     const uint32_t block_bytes = 2u * ctx->cfg.block_size * ctx->cfg.head_dim * 2u;
     const int ctas = ctx->cfg.gather_ctas;
+    unsigned int* door = ctx->door_next;
     if (ctx->cfg.gather_mode == SPARDA_GATHER_TMA) {
         const int smem = GATHER_STAGES * GATHER_STAGE_BYTES;
         sparda_kernel_state& ks = ctx->kstate[SPARDA_K_GATHER_TMA];
@@ -168,7 +179,7 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
         lc.stream = st;
         lc.attrs = at;
         lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
-        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_tma_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes));
+        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_tma_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes, door));
     } else {
         cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
         cudaLaunchConfig_t lc = {};
@@ -177,7 +188,7 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
         lc.stream = st;
         lc.attrs = at;
         lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
-        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_ldg_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes));
+        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_ldg_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes, door));
     }
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;

@@ -345,6 +345,9 @@ struct SelParams {
     int32_t* slot_ids;
     int32_t* fetch;
     int32_t* n_fetch;
+    // optional doorbell (overlapped decode step): the CTA that owns the row rings it once the row's ids (and fetch list) are
+    // out, so the gather of the layer -- already resident on its own stream -- starts without a kernel boundary in between
+    unsigned int* door;
 };
 
 // tmap: the pooled keys as a [R * n_blocks * KPB][D] bf16 tensor, box = 64 keys x 64 elements, 128-byte swizzle.
@@ -391,6 +394,10 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
                     const int nm = reuse_plan_row(ids_row, p.slot_ids + (size_t)r * p.topk, old, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
                     if (lane == 0 && p.n_fetch) p.n_fetch[r] = nm;
                 }
+            }
+            if (p.door) {
+                __syncthreads();
+                if (tid == 0) door_ring(p.door);
             }
         }
         return;
@@ -563,7 +570,14 @@ __global__ void __launch_bounds__(SEL_CTA_THREADS, 2) forecast_select_kernel(con
         if (w == 0) {
             const int nm = reuse_plan_row(nullptr, p.slot_ids + (size_t)r * p.topk, plan_old, p.fetch + (size_t)r * p.topk, p.topk, s_plan, lane);
             if (lane == 0 && p.n_fetch) p.n_fetch[r] = nm;
+            if (p.door) {
+                __syncwarp();
+                if (lane == 0) door_ring(p.door);
+            }
         }
+    } else if (p.door) {
+        consumer_sync();   // every consumer thread has issued its ids
+        if (tid == 0) door_ring(p.door);
     }
 }
 
@@ -737,6 +751,7 @@ int sparda_launch_select(sparda_ctx* ctx, const void* F, const void* Kpool, int 
     p.slot_ids = slot_ids;
     p.fetch = fetch;
     p.n_fetch = n_fetch;
+    p.door = ctx->door_next;
     p.F = (const uint32_t*)F;
     p.ids = ids;
     p.n_blocks = n_blocks;
@@ -757,6 +772,7 @@ int sparda_launch_select_grid(sparda_ctx* ctx, const void* F, const void* Kgrid,
                               int topk, int32_t* ids, cudaStream_t st) {
     SelParams p;
     p.slot_ids = p.fetch = p.n_fetch = nullptr;
+    p.door = nullptr;
     p.F = (const uint32_t*)F;
     p.ids = ids;
     p.n_blocks = n_blocks;

@@ -96,6 +96,8 @@ int sparda_create(const sparda_config* cfg, sparda_ctx** out) {
               cudaMalloc(&ctx->part_ml, n_ml * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&ctx->tickets, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&ctx->probe_sink, 256 * sizeof(uint32_t)) == cudaSuccess &&
+              cudaMalloc(&ctx->door, (size_t)(ctx->max_layers + 1) * sizeof(unsigned int)) == cudaSuccess &&
+              cudaMemset(ctx->door, 0, (size_t)(ctx->max_layers + 1) * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&ctx->pf_scratch, (size_t)ctx->sm_count * 512 * 128 * sizeof(float)) == cudaSuccess &&
               cudaMemset(ctx->tickets, 0, (size_t)ctx->R * sizeof(unsigned int)) == cudaSuccess;
     ctx->ev_sel = (cudaEvent_t*)calloc(ctx->max_layers + 1, sizeof(cudaEvent_t));
@@ -135,6 +137,7 @@ int sparda_destroy(sparda_ctx* ctx) {
     cudaFree(ctx->tickets);
     cudaFree(ctx->pf_scratch);
     cudaFree(ctx->probe_sink);
+    cudaFree(ctx->door);
     for (int i = 0; i <= ctx->max_layers; ++i) {
         if (ctx->ev_sel && ctx->ev_sel[i]) cudaEventDestroy(ctx->ev_sel[i]);
         if (ctx->ev_gather && ctx->ev_gather[i]) cudaEventDestroy(ctx->ev_gather[i]);
@@ -259,16 +262,21 @@ int sparda_prefill_select_baseline(sparda_ctx* ctx, const void* Q, const void* K
 // previous step's blocks kept per layer.  Given layer l's projections, line 4 (select B_{l+1}) and line 7
 // (attention l) do not depend on each other, so in overlap mode they run concurrently on two streams; the prefetch has
 // its own, on which the gathers run one after the other, each alone on the link:
-//   compute stream  cs:  record ev_top[l]  ->  wait ev_gather[l]  ->  attention l
-//   select stream   ss:  wait ev_top[l]    ->  [F_l = X_l W_F]  ->  select B_{l+1} (+ reuse plan)  ->  record ev_sel[l+1]
-//   prefetch stream ps:  wait ev_sel[l+1]  ->  gather B_{l+1}  ->  record ev_gather[l+1]
+//   compute stream  cs:  record ev_top[l]  ->  wait ev_gather[l] (and ev_sel[l])  ->  attention l
+//   select stream   ss:  wait ev_top[l]    ->  [F_l = X_l W_F]  ->  select B_{l+1} (+ reuse plan), rings door[l+1] row by row  ->  record ev_sel[l+1]
+//   prefetch stream ps:  wait ev_top[l]    ->  gather B_{l+1}: waits ON THE DEVICE for door[l+1] == R, copies  ->  record ev_gather[l+1]
 // ev_top[l] follows attention l-1 on cs, so a select never runs more than one layer ahead of the attention (in a model,
 // F_l exists only once layer l-1 is complete) and it releases the buffers gather l+1 writes: pool[(l+1)&1] was last read
-// by attention l-1 (plain); pool_{l+1} and slot_ids_{l+1} by attention l+1 of the previous step (cached).  Every gather
-// ends in an event an attention waits for, so cs has joined both side streams when the step ends (capturable).  A
-// cross-stream hand-off costs next to nothing inside a CUDA graph (measured); putting a layer's select and gather on one
-// stream and alternating two such streams between layers was tried: same floor, but two gathers then share the link and
-// the step with every block fetched loses 1 %.  Serial mode: the same kernels on cs in Algorithm-2 order.
+// by attention l-1 (plain); pool_{l+1} and slot_ids_{l+1} by attention l+1 of the previous step (cached).
+// The doorbell (sparda_internal.cuh) takes the select -> gather kernel boundary off the chain: the gather launch is resident
+// (8 one-warp CTAs, sleeping between polls) while the select runs and starts the moment the last row's list is out.  Alone the
+// boundary costs ~3 us; beside a kernel that saturates the GPU -- a real layer -- a dependent launch costs 10-20 us and the chain
+// select -> gather 40 us instead of 9 (measured), which is what bounds how much link time fits behind a layer.
+// Every gather ends in an event an attention waits for, and ev_sel joins the select stream, so cs has joined both side
+// streams when the step ends (capturable).  A cross-stream hand-off costs next to nothing inside a CUDA graph when the GPU
+// is idle (measured); putting a layer's select and gather on one stream and alternating two such streams between layers was
+// tried: same floor, but two gathers then share the link and the step with every block fetched loses 1 %.  Serial mode: the
+// same kernels on cs in Algorithm-2 order, no doorbell.
 // timing events around one launch of `kind` (0 select, 1 gather, 2 attention) on stream st
 static inline cudaEvent_t* prof_slot(sparda_ctx* ctx, int kind) {
     return &ctx->ev_prof[((size_t)kind * (ctx->max_layers + 1) + ctx->prof_n[kind]) * 2];
@@ -296,6 +304,8 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
     cudaStream_t ss = overlap ? ctx->select_stream : cs, ps = overlap ? ps_in : cs;
     int rc;
     ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
+    // doorbells of this step: every door of the previous step has been consumed (the compute stream joined both side streams)
+    if (overlap) SPARDA_CUDA_TRY(ctx, cudaMemsetAsync(ctx->door, 0, (size_t)(n_layers + 1) * sizeof(unsigned int), cs));
     if (io) SPARDA_CUDA_TRY(ctx, cudaMemcpyAsync(const_cast<void*>(F0cur), io->F0cur, io->f_bytes, cudaMemcpyHostToDevice, cs));
     // layer 0: same-layer selection with F0cur; its attention needs it, so it stays on the compute stream
     if (!io && layers[0].base.X && layers[0].base.WFcur) {   // Alg.2 l.1 for F_0^cur (Eq.3)
@@ -330,21 +340,29 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
                 rc = sparda_launch_forecast_project(ctx, layers[l].base.X, layers[l].base.WF, ctx->cfg.hidden, const_cast<void*>(layers[l].base.F),
                                                     (l + 1) & 1, xs);
                 if (rc) return rc;
+                ctx->pdl_next = 1;   // the select follows the projection on its own stream, no event in between: its prologue
+                                     // and the first ring of pooled keys overlap the projection (0.58 -> 0.55 ms per cached step, batch 4)
             }
+            ctx->door_next = overlap ? ctx->door + (l + 1) : nullptr;   // this select rings the layer's gather (below) row by row
             SPARDA_PROF_BEGIN(0, xs);
             if (nx->slot_ids)   // select + reuse plan in one launch
                 rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids,
                                                  nx->slot_ids, nx->fetch, nx->n_fetch, xs);
             else
                 rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, xs);
-            if (rc) return rc;
+            if (rc) { ctx->door_next = nullptr; return rc; }
             SPARDA_PROF_END(0, xs);
+            ctx->pdl_next = overlap ? 0 : 1;
             if (overlap) {
+                // the gather does not wait for the select's kernel boundary: it starts with the select (both behind ev_top[l],
+                // which also releases the pool it writes) and waits on the device for the doorbell.  ev_sel joins the select
+                // stream back into the compute stream in front of attention l+1 (stream capture needs the join)
                 SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], xs));
-                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(gs, ctx->ev_sel[l + 1], 0));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(gs, ctx->ev_top[l], 0));
             }
             SPARDA_PROF_BEGIN(1, gs);
             rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->slot_ids ? nx->fetch : nx->base.ids, topk, nx->pool, gs);
+            ctx->door_next = nullptr;
             if (rc) return rc;
             SPARDA_PROF_END(1, gs);
             if (overlap) SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_gather[l + 1], gs));
@@ -354,7 +372,10 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
             SPARDA_PROF_BEGIN(2, cs);
             rc = sparda_sparse_decode(ctx, layers[0].base.Q, layers[0].base.kv, layers[0].base.ids, topk, 1, n_blocks, layers[0].base.O, cs);
         } else {
-            if (overlap) SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
+            if (overlap) {
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_gather[l], 0));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_sel[l], 0));
+            }
             SPARDA_PROF_BEGIN(2, cs);
             rc = sparda_sparse_decode(ctx, layers[l].base.Q, layers[l].pool, layers[l].slot_ids ? layers[l].slot_ids : layers[l].base.ids,
                                       topk, 0, topk, layers[l].base.O, cs);

@@ -66,6 +66,11 @@ struct sparda_ctx {
     // overlapped step, where every chain starts behind an event wait and early-resident dependents only take shared memory
     // from the kernels of the other streams (measured: 0.43 ms with PDL on the in-chain launches, 0.38 ms without)
     int pdl_next;
+    // Doorbells between the select and the gather of a layer inside the overlapped step (sparda_api.cu): door[l] counts the rows
+    // of layer l whose block list is out in this step (zeroed at the top of every step).  door_next != nullptr: the NEXT select
+    // / gather launch rings / waits on it (the step sets it; stand-alone calls never do).
+    unsigned int* door;       // [max_layers + 1]
+    unsigned int* door_next;
     char cuda_err[256];
     // TMA descriptor cache (host): open-addressed hash on (base, rows, head_dim, box_rows); lookups return a COPY, so an
     // eviction can never change a descriptor a launcher already holds
@@ -162,6 +167,24 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "}" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
+}
+
+// ---- select -> gather doorbell (device side).  Producer: after a row's block list is in global memory (ordered before the
+// calling thread by a CTA / warp barrier), one thread publishes it: the fence makes the list visible at gpu scope before the
+// count.  Consumer: one thread per CTA waits until all R rows of its layer have been published.
+__device__ __forceinline__ void door_ring(unsigned int* door) {
+    __threadfence();
+    atomicAdd(door, 1u);
+}
+__device__ __forceinline__ void door_wait(const unsigned int* door, unsigned int need) {
+    unsigned int spins = 0;
+    for (;;) {
+        unsigned int v;
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(door) : "memory");
+        if (v >= need) break;
+        __nanosleep(64);
+        if (++spins > (1u << 24)) __trap();   // ~15 s: the select this launch was paired with never ran: fail, do not hang the device
+    }
 }
 
 // Programmatic dependent launch (PDL): a kernel launched with sparda_pdl_attr() may become resident and run its prologue

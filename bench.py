@@ -563,7 +563,7 @@ def bench_reuse(torch, binding, ctx, cfg, dev_layers, F0, cs, ps, steps, standin
         ctx.decode_step_cached(arrs[which], F0s[which], Nb, k, cs, ps, binding.STEP_OVERLAP)
 
     out = []
-    for alpha in (0.0, 0.05, 0.1, 0.2, 0.4, 0.8, 1e9):
+    for alpha in (0.0, 0.05, 0.1, 0.2, 0.3, 0.4, 0.8, 1e9):
         for l, e in enumerate(layers[1]):                    # F_B = bf16(F_A + alpha * N(0, 1))
             e["F"].copy_((dev_layers[l]["F"].float() + alpha * noise[l]).to(torch.bfloat16))
         F0s[1].copy_((F0.float() + alpha * noise0).to(torch.bfloat16))

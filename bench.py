@@ -675,7 +675,7 @@ def bench_chain_under_load(torch, binding):
     host = torch.empty((R, 8, 2, 64, D), dtype=torch.bfloat16, pin_memory=True)
     pool = torch.empty((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda")
     W = torch.empty(STANDIN_BYTES // 2, dtype=torch.bfloat16, device="cuda").fill_(1.0)
-    cs, xs = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, xs = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)   # as the context's select stream
     sel = lambda i: ctx.forecast_select_plan(F, kpools[i], Nb, k, ids, slot, fetch, stream=xs)
     gat = lambda i: ctx.prefetch_launch(host, 8, empty, k, pool, stream=xs)
     att = lambda i: ctx.sparse_decode(Q, pools[i], ids_a, k, O, stream=xs)
@@ -740,7 +740,7 @@ def bench_gather_sweep(torch, binding, peaks, ceiling, host_layer_b4):
         ids_s = torch.empty((R, k), dtype=torch.int32, device="cuda")
         ids_a = torch.arange(k, dtype=torch.int32, device="cuda").repeat(R, 1).contiguous()
         cctx = binding.Sparda.from_config(cfg)
-        cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+        cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)   # the prefetch stream outranks the compute stream (sparda.h)
         NP = 20
         for i in range(NSETS):
             cctx.forecast_select(F, kpools[i], Nb, k, ids_s)
@@ -920,7 +920,7 @@ def run_sparda(args):
     pools = [torch.zeros((R, k, 2, cfg.block_size, D), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
     arr = ctx.make_layers(dev_layers)
     arr_host = ctx.make_layers([{**d, **h} for d, h in zip(dev_layers, host_vals)])
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)   # the prefetch stream outranks the compute stream (sparda.h)
 
     ceiling = measure_h2d_ceiling(torch, host_kv[:min(4, resident)])
 

@@ -200,7 +200,10 @@ int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, c
  * In overlap mode a layer's gather is launched together with its select and waits on the device for the select's
  * doorbell (one counter per layer in the context's workspace, zeroed at the top of the step), so no kernel boundary
  * sits between "block list out" and "first byte on the link"; a gather whose select never runs traps after ~15 s
- * instead of hanging the device.  One step per context at a time.
+ * instead of hanging the device.  One step per context at a time.  The select runs on a highest-priority stream of the
+ * context; create prefetch_stream with the highest priority too (cudaStreamCreateWithPriority): beside a many-CTA kernel on
+ * the compute stream the block scheduler serves the older kernel's pending CTAs first, and at equal priority a side-stream
+ * kernel launched after it waits for most of it (measured: select 42 us instead of 20 beside a 4736-CTA HBM stream).
  * Capturable into a CUDA graph (no host synchronisation, events are pre-created).                             */
 int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                        int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,

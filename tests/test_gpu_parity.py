@@ -216,7 +216,7 @@ def test_decode_step_pipeline(cfg, sp, oracle):
     F0 = data[0][0]["F0cur"]
     pools = [torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
     arr = ctx.make_layers(dev)
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
     torch.cuda.synchronize()
     results = {}
     for mode in (sp.STEP_SERIAL, sp.STEP_OVERLAP, sp.STEP_OVERLAP):
@@ -270,7 +270,7 @@ def test_decode_step_host_buffers_and_profile(sp):
         if l == 0:
             F0 = L["F0cur"]
     pools = [torch.zeros((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
     torch.cuda.synchronize()
     ctx.profile_enable(True)
     ctx.decode_step(ctx.make_layers(dev), F0, Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)
@@ -303,7 +303,7 @@ def test_decode_step_replays_from_a_cuda_graph(sp):
             F0 = L["F0cur"]
     pools = [torch.zeros((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
     arr = ctx.make_layers(dev)
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
     torch.cuda.synchronize()
     ctx.decode_step(arr, F0, Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)      # eager: reference + warm-up
     torch.cuda.synchronize()
@@ -410,7 +410,7 @@ def test_decode_step_cached_multi_step(cfg, sp, oracle):
                         "n_fetch": torch.zeros((R,), dtype=torch.int32, device="cuda") if l else None})
         arr = ctx.make_cached_layers(dev)
         F0 = F0s[0].clone()
-        cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+        cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
         hist = []
         for t in range(n_steps):
             for l in range(NL):
@@ -988,7 +988,7 @@ def test_full_size_32_layer_decode_step(sp, oracle):
     dev, obits, F0 = _full_step_inputs(cfg, sp, ctx, n_distinct=3)
     pools = [torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
     arr = ctx.make_layers(dev)
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
     torch.cuda.synchronize()
     res = {}
     for mode in (sp.STEP_SERIAL, sp.STEP_OVERLAP):
@@ -1038,7 +1038,7 @@ def test_full_size_32_layer_cached_steps(sp, oracle):
         d["n_fetch"] = torch.zeros((R,), dtype=torch.int32, device="cuda") if l else None
     arr = ctx.make_cached_layers(dev)
     F0w = F0.clone()
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
     g = torch.Generator(device="cuda").manual_seed(31337)
     baseF = [d["F"].clone() for d in dev]
     state = None
@@ -1162,7 +1162,7 @@ def test_decode_step_with_in_step_forecast_projection(sp, oracle):
     dev[0]["WFcur"] = (torch.randn((hidden, cfg.n_kv_heads * D), generator=g, device="cuda") / hidden ** 0.5).to(torch.bfloat16)
     F0 = torch.full((R, D), float("nan"), dtype=torch.bfloat16, device="cuda")
     pools = [torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
     torch.cuda.synchronize()
     out = {}
     for mode in (sp.STEP_OVERLAP, sp.STEP_SERIAL):

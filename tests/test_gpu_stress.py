@@ -96,7 +96,7 @@ def test_cached_pipeline_is_deterministic_under_repetition(sp, oracle):
     cfg = synth.DecodeConfig("p", batch=4, n_q_heads=32, n_kv_heads=2, head_dim=128, n_blocks=256, topk=64, n_layers=6, seed=5)
     ctx = sp.Sparda.from_config(cfg, max_layers=8)
     R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
     ref = None
     for rep in range(25):
         dev, F0 = _cached_layers(cfg, ctx, sp)
@@ -134,7 +134,7 @@ def test_captured_cached_step_replays_with_poisoned_pools(sp, oracle):
     R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim
     dev, F0 = _cached_layers(cfg, ctx, sp)
     arr = ctx.make_cached_layers(dev)
-    cs, ps = torch.cuda.Stream(), torch.cuda.Stream()
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
 
     def reset():
         for d in dev:

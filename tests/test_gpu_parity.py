@@ -201,8 +201,12 @@ def _pipeline_inputs(cfg, binding):
     return keep
 
 
-@pytest.mark.parametrize("cfg", [synth.CFG1_TINY.with_(n_layers=5), G16.with_(n_layers=4, batch=3)], ids=lambda c: c.name)
+@pytest.mark.parametrize("cfg", [synth.CFG1_TINY.with_(n_layers=5), G16.with_(n_layers=4, batch=3),
+                                 MID64.with_(name="fewer_blocks_than_k", n_blocks=6, n_layers=3)], ids=lambda c: c.name)
 def test_decode_step_pipeline(cfg, sp, oracle):
+    """Overlapped == serialized bit for bit on NaN-poisoned pools, then every layer against o10.  The third shape has fewer
+    blocks than k: every candidate is selected without scoring (reading q5), ids are -1 padded, and the select's early exit
+    still has to ring the layer's gather (the doorbell of the overlapped step)."""
     ctx = sp.Sparda.from_config(cfg, max_layers=8)
     data = _pipeline_inputs(cfg, sp)
     R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim

@@ -40,10 +40,12 @@ __device__ __forceinline__ int reuse_plan_row(const int32_t* in, int32_t* slots,
     }
     __syncwarp();
 
-    // hits: resident blocks that are selected again
+    // hits: resident blocks that are selected again (hit[q] = position of slot 32 q + lane's block in the selection, or -1)
+    int hit[RP_MAXK / 32];
 #pragma unroll
     for (int q = 0; q < RP_MAXK / 32; ++q) {
         const int c = q * 32;
+        hit[q] = -1;
         if (c >= k) break;
         const int s = c + lane;
         const int32_t b = old[q];
@@ -53,7 +55,7 @@ __device__ __forceinline__ int reuse_plan_row(const int32_t* in, int32_t* slots,
                 const int mid = (lo + hi) >> 1;
                 if (nw[mid] < b) lo = mid + 1; else hi = mid;
             }
-            if (lo < m && nw[lo] == b) atomicMin(&owner[lo], s);
+            if (lo < m && nw[lo] == b) { hit[q] = lo; atomicMin(&owner[lo], s); }
         }
     }
     __syncwarp();
@@ -64,18 +66,7 @@ __device__ __forceinline__ int reuse_plan_row(const int32_t* in, int32_t* slots,
         const int c = q * 32;
         if (c >= k) break;
         const int s = c + lane;
-        bool kept = false;
-        if (s < k) {
-            const int32_t b = old[q];
-            if (b >= 0) {
-                int lo = 0, hi = m;
-                while (lo < hi) {
-                    const int mid = (lo + hi) >> 1;
-                    if (nw[mid] < b) lo = mid + 1; else hi = mid;
-                }
-                kept = lo < m && nw[lo] == b && owner[lo] == s;
-            }
-        }
+        const bool kept = s < k && hit[q] >= 0 && owner[hit[q]] == s;   // the lowest slot holding the block keeps it
         const unsigned fb = __ballot_sync(0xffffffffu, s < k && !kept);
         if (s < k && !kept) sfree[n_free + __popc(fb & lt)] = (int16_t)s;
         n_free += __popc(fb);

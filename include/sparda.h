@@ -313,7 +313,7 @@ int64_t sparda_launch_count(const sparda_ctx* ctx);
 int64_t sparda_tmap_encodes(const sparda_ctx* ctx);      /* TMA descriptors encoded so far (a warm step encodes none) */
 int sparda_get_select_cluster(const sparda_ctx* ctx);    /* cluster size of the LAST forecast_select launch           */
 int sparda_get_attn_cluster(const sparda_ctx* ctx);      /* CTAs per row reduced through DSMEM by the LAST sparse_decode
-                                                            launch (2, 4 or 8), 0 = workspace + ticket reduction     */
+                                                            launch (2, 4, 8, 16), 0 = workspace + ticket reduction      */
 int sparda_get_attn_splits(const sparda_ctx* ctx, int topk);
 int sparda_get_gather_ctas(const sparda_ctx* ctx);
 const char* sparda_strerror(int code);

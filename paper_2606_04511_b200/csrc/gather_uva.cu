@@ -10,9 +10,10 @@
 //  * SPARDA_GATHER_TMA (default, B200-native): one warp per CTA compacts the task list and ONE of its threads drives a ring of 16 KiB shared-memory
 //    stages with bulk-copy (TMA) instructions: cp.async.bulk global(host-mapped)->smem completing on an
 //    mbarrier, then cp.async.bulk smem->global(HBM).  No registers or LSU slots are spent on payload, so a
-//    handful of CTAs saturates the host link (measured on this box: 2-4 CTAs x 1 thread reach the same
-//    51.4 GB/s plateau that takes 8+ CTAs x 256 threads with vector loads), leaving the SMs to the compute
-//    stream (the trade-off of P:L116).
+//    handful of CTAs saturates the host link (measured on this box: alone on the GPU 2 CTAs x 1 thread reach the
+//    50.5 GB/s plateau that takes 8+ CTAs x 256 threads with vector loads; beside a kernel that saturates HBM a
+//    host read takes three times as long to come back and it takes 8 CTAs to keep 49 GB/s on the link: the
+//    default), leaving the SMs to the compute stream (the trade-off of P:L116).
 //  * SPARDA_GATHER_LDG: the paper's shape, persistent warps issuing 16-byte vector loads (8 in flight per
 //    lane) from mapped host memory, 4 KiB per warp-iteration.
 #include "sparda_internal.cuh"

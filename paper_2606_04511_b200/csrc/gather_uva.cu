@@ -27,7 +27,14 @@ using namespace sparda;
 #define GATHER_STAGES_V 6
 #endif
 constexpr int GATHER_STAGE_BYTES = GATHER_STAGE_BYTES_V;
-constexpr int GATHER_STAGES = GATHER_STAGES_V;  // 96 KiB ring per CTA, up to 5 loads in flight while one stage drains
+constexpr int GATHER_STAGES = GATHER_STAGES_V;  // 96 KiB ring per CTA
+#ifndef GATHER_PENDING_V
+#define GATHER_PENDING_V 2
+#endif
+// Stores that may still be reading their stage when the next load is issued: the thread does not wait for each smem -> HBM
+// store before it asks for the next block (loads in flight = STAGES - PENDING).  Nothing on the PCIe link (the same 50.4 GB/s with
+// 0 .. 4), but from a fast source -- the peer-HBM tier -- a CTA moves more per round trip (gather_sweep.hbm_tier).
+constexpr int GATHER_PENDING = GATHER_PENDING_V;
 
 constexpr int GATHER_WIN = 1024;  // tasks compacted per window (32 per lane, held in registers)
 
@@ -66,7 +73,7 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
         mbar_wait(&full[store_s], store_phase);
         bulk_s2g(dst_of[store_s], ring + (size_t)store_s * GATHER_STAGE_BYTES, GATHER_STAGE_BYTES);
         bulk_commit();
-        bulk_wait_read<0>();
+        bulk_wait_read<GATHER_PENDING>();
         if (++store_s == GATHER_STAGES) { store_s = 0; store_phase ^= 1; }
         --in_flight;
     };
@@ -106,7 +113,7 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
         if (lane == 0) {
             const int n_units = (hi - lo) * (int)cpb;
             for (int u = 0; u < n_units; ++u) {
-                if (in_flight == GATHER_STAGES) { drain_one(); }
+                if (in_flight == GATHER_STAGES - GATHER_PENDING) { drain_one(); }
                 const int e = u / (int)cpb, c = u % (int)cpb;
                 const int64_t r = q_task[e] / topk;
                 const char* src = host_kv + ((r * n_blocks + q_id[e]) * (int64_t)block_bytes + (int64_t)c * GATHER_STAGE_BYTES);

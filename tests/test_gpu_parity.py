@@ -254,6 +254,42 @@ def test_decode_step_pipeline(cfg, sp, oracle):
         parity.check_attn(_bits(Os[l]), want, f"layer {l}")
 
 
+def test_decode_step_ldg_engine_through_the_doorbell(sp):
+    """The LDG gather engine (the paper's shape) inside the overlapped step: it, too, is launched with its select and waits for
+    the doorbell.  Byte copies, so every O and every pool must be bit-identical to the TMA engine's and to its own serial step."""
+    cfg = G16.with_(n_layers=4, batch=3)
+    data = _pipeline_inputs(cfg, sp)
+    R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim
+    outs = {}
+    for name, kw in (("tma", {}), ("ldg", {"gather_mode": sp.GATHER_LDG, "gather_ctas": 5})):
+        ctx = sp.Sparda.from_config(cfg, max_layers=4, **kw)
+        dev = []
+        for l, (L, kv_host) in enumerate(data):
+            kpool = torch.empty((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+            ctx.pool_keys(L["kv"], R, Nb, kpool)
+            dev.append({"F": L["F"], "Q": L["Q"], "Kpool": kpool, "kv": L["kv"] if l == 0 else kv_host,
+                        "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                        "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda")})
+        arr = ctx.make_layers(dev)
+        cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
+        for mode in (sp.STEP_SERIAL, sp.STEP_OVERLAP):
+            pools = [torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+            for d in dev:
+                d["O"].zero_()
+            torch.cuda.synchronize()
+            for _ in range(3):                                       # repeated: the doors are re-armed at the top of every step
+                ctx.decode_step(arr, data[0][0]["F0cur"], Nb, k, pools[0], pools[1], cs, ps, mode)
+            torch.cuda.synchronize()
+            outs[(name, mode)] = ([d["O"].clone() for d in dev], [p.clone() for p in pools])
+        ctx.close()
+    ref = outs[("tma", sp.STEP_SERIAL)]
+    for key, (Os, pools) in outs.items():
+        for a, b in zip(ref[0], Os):
+            assert torch.equal(a.view(torch.int16), b.view(torch.int16)), f"{key}: O differs"
+        for a, b in zip(ref[1], pools):
+            assert torch.equal(a.view(torch.int16), b.view(torch.int16)), f"{key}: pool bytes differ"
+
+
 def test_decode_step_host_buffers_and_profile(sp):
     """The host-buffer form of the step (what bench.py's e2e times) gives bit-identical O to the device form;
     per-kernel profiling reports one select and one attention per layer and one gather per layer >= 1."""

@@ -209,6 +209,13 @@ int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers
                        int topk, void* dev_pool0, void* dev_pool1, void* compute_stream, void* prefetch_stream,
                        int mode);
 
+/* Growing caches (Alg.2 l.2-3): a cache allocated for n_blocks blocks holds t + 1 tokens, of which
+ * n_cand = (t + 1) / S blocks are complete and have a pooled key (sparda_append_kv).  After this call the selections of
+ * sparda_decode_step / _host / _cached rank blocks [0, n_cand) only (n_blocks stays the layout stride); 0 restores
+ * n_cand = n_blocks.  With n_cand <= topk every complete block is selected and the rest of the ids is -1 (reading q5).
+ * Host-side state of the context: set it before the step is enqueued (or captured).                              */
+int sparda_set_step_candidates(sparda_ctx* ctx, int n_cand);
+
 /* The same step for a caller whose per-step tensors live in HOST memory (the end-to-end form bench.py times):
  * layers[l].F, .Q and .O and F0cur are HOST pointers (pinned for the copies to be asynchronous); the call runs
  * sparda_decode_step on staging owned by the context and enqueues the copies on compute_stream just in time: F0cur first,

@@ -306,6 +306,8 @@ struct HostIO {
 static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, int n_layers, const void* F0cur, int n_blocks,
                             int topk, cudaStream_t cs, cudaStream_t ps_in, int mode, const HostIO* io = nullptr) {
     const bool overlap = mode == SPARDA_STEP_OVERLAP;
+    // candidate range of every selection of the step: the complete blocks of a cache of capacity n_blocks (sparda_set_step_candidates)
+    const int n_cand = ctx->step_n_cand > 0 && ctx->step_n_cand < n_blocks ? ctx->step_n_cand : n_blocks;
     cudaStream_t ss = overlap ? ctx->select_stream : cs, ps = overlap ? ps_in : cs;
     int rc;
     ctx->prof_n[0] = ctx->prof_n[1] = ctx->prof_n[2] = 0;
@@ -319,7 +321,7 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
         if (rc) return rc;
     }
     SPARDA_PROF_BEGIN(0, cs);
-    rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_blocks, topk, layers[0].base.ids, cs);
+    rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_cand, topk, layers[0].base.ids, cs);
     if (rc) return rc;
     SPARDA_PROF_END(0, cs);
     struct PdlScope {   // launches behind an event wait do not ask for PDL (see sparda_ctx::pdl_next); restored on every return
@@ -351,10 +353,10 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
             ctx->door_next = overlap ? ctx->door + (l + 1) : nullptr;   // this select rings the layer's gather (below) row by row
             SPARDA_PROF_BEGIN(0, xs);
             if (nx->slot_ids)   // select + reuse plan in one launch
-                rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids,
+                rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_cand, topk, nx->base.ids,
                                                  nx->slot_ids, nx->fetch, nx->n_fetch, xs);
             else
-                rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_blocks, topk, nx->base.ids, xs);
+                rc = sparda_forecast_select(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_cand, topk, nx->base.ids, xs);
             if (rc) { ctx->door_next = nullptr; return rc; }
             SPARDA_PROF_END(0, xs);
             ctx->pdl_next = overlap ? 0 : 1;
@@ -457,6 +459,12 @@ int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_l
     HostIO io = {layers, F0cur, f_bytes, q_bytes};
     return decode_step_impl(ctx, cl, n_layers, ctx->stage_F + f_bytes * ctx->max_layers, n_blocks, topk, cs, (cudaStream_t)prefetch_stream, mode,
                             &io);
+}
+
+int sparda_set_step_candidates(sparda_ctx* ctx, int n_cand) {
+    if (!ctx || n_cand < 0) return SPARDA_EINVAL;
+    ctx->step_n_cand = n_cand;
+    return SPARDA_OK;
 }
 
 int sparda_profile_enable(sparda_ctx* ctx, int on) {

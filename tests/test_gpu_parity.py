@@ -290,6 +290,76 @@ def test_decode_step_ldg_engine_through_the_doorbell(sp):
             assert torch.equal(a.view(torch.int16), b.view(torch.int16)), f"{key}: pool bytes differ"
 
 
+def test_multi_step_decode_with_growing_cache(sp, oracle):
+    """A true multi-step decode (Alg.2 l.2-7 over consecutive tokens): every step appends the new token's K / V to every layer's
+    cache (layer 0 on the device, the others in pinned host memory through UVA), the pooled keys grow block by block, and the
+    overlapped step ranks only the complete blocks (sparda_set_step_candidates).  Checked against o13 + o10 on sampled steps,
+    including the step at which a block completes and becomes selectable."""
+    cfg = synth.DecodeConfig("grow", batch=2, n_q_heads=8, n_kv_heads=2, head_dim=128, n_blocks=8, topk=4, n_layers=3, seed=61)
+    R, k, Nb, D, NL, S = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers, 64
+    ctx = sp.Sparda.from_config(cfg, max_layers=NL)
+    g = torch.Generator(device="cuda").manual_seed(61)
+    kv = [torch.zeros((R, Nb, 2, S, D), dtype=torch.bfloat16, device="cuda") if l == 0 else
+          torch.zeros((R, Nb, 2, S, D), dtype=torch.bfloat16).pin_memory() for l in range(NL)]
+    kpool = [torch.zeros((R, Nb, D), dtype=torch.bfloat16, device="cuda") for _ in range(NL)]
+    ksum = [torch.zeros((R, D), dtype=torch.float32, device="cuda") for _ in range(NL)]
+    o_kv = [np.zeros((R, Nb, 2, S, D), dtype=np.uint16) for _ in range(NL)]
+    o_pool = [np.zeros((R, Nb, D), dtype=np.uint16) for _ in range(NL)]
+    dev = [{"F": torch.zeros((R, D), dtype=torch.bfloat16, device="cuda"), "Q": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+            "Kpool": kpool[l], "kv": kv[l], "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+            "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda")} for l in range(NL)]
+    F0 = torch.zeros((R, D), dtype=torch.bfloat16, device="cuda")
+    arr = ctx.make_layers(dev)
+    pools = [torch.full((R, k, 2, S, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
+    t_prefill, t_end = 5 * S + 10, 6 * S + 20                       # block 5 completes at t = 383, inside the decoded range
+    checked = 0
+    for t in range(t_end):
+        n_cand = 0
+        for l in range(NL):                                          # Alg.2 l.2-3: append, update the pooled keys
+            bias = 1.5 * torch.randn((R, 1), generator=g, device="cuda")
+            kn = (torch.randn((R, D), generator=g, device="cuda") + bias).to(torch.bfloat16)
+            vn = torch.randn((R, D), generator=g, device="cuda").to(torch.bfloat16)
+            ctx.append_kv(kn, vn, t, kv[l], Nb, ksum[l], kpool[l])
+            n_cand = oracle.append_kv(o_kv[l], o_pool[l], _bits(kn), _bits(vn), t)
+        if t < t_prefill:
+            continue
+        for d in dev:                                                # this token's projections
+            d["F"].copy_(torch.randn((R, D), generator=g, device="cuda").to(torch.bfloat16))
+            d["Q"].copy_(torch.randn(d["Q"].shape, generator=g, device="cuda").to(torch.bfloat16))
+        F0.copy_(torch.randn((R, D), generator=g, device="cuda").to(torch.bfloat16))
+        for p_ in pools:
+            p_.fill_(float("nan"))
+        ctx.set_step_candidates(n_cand)
+        torch.cuda.synchronize()
+        ctx.decode_step(arr, F0, Nb, k, pools[0], pools[1], cs, ps, sp.STEP_OVERLAP)
+        torch.cuda.synchronize()
+        if t not in (t_prefill, 6 * S - 2, 6 * S - 1, 6 * S, t_end - 1):
+            continue
+        assert n_cand == (t + 1) // S
+        olayers = []
+        for l in range(NL):
+            gp = _bits(kpool[l])
+            assert parity.ulp_diff_bf16(gp[:, :n_cand], o_pool[l][:, :n_cand]).max() <= 1
+            assert _bits(kv[l]).tobytes() == o_kv[l].tobytes()
+            olayers.append({"kv": np.ascontiguousarray(o_kv[l][:, :n_cand]), "kpool": np.ascontiguousarray(gp[:, :n_cand]), "F": _bits(dev[l]["F"]),
+                            "Q": _bits(dev[l]["Q"]), "F0cur": _bits(F0)})
+        ref = oracle.decode_pipeline(olayers, k)
+        for l in range(NL):
+            gids = dev[l]["ids"].cpu().numpy()
+            assert gids.max() < n_cand, "a block beyond the complete ones was selected"
+            parity.check_ids(gids, ref[l]["ids"], ref[l]["scores"])
+            if l == 0:
+                want, _ = oracle.sparse_attn(olayers[0]["Q"], olayers[0]["kv"], gids, pool_is_indexed=True)
+            else:
+                want, _ = oracle.sparse_attn(olayers[l]["Q"], oracle.gather(olayers[l]["kv"], gids), gids)
+            parity.check_attn(_bits(dev[l]["O"]), want, f"t {t} layer {l}")
+        checked += 1
+    assert checked == 5
+    ctx.set_step_candidates(0)
+    ctx.close()
+
+
 def test_decode_step_host_buffers_and_profile(sp):
     """The host-buffer form of the step (what bench.py's e2e times) gives bit-identical O to the device form;
     per-kernel profiling reports one select and one attention per layer and one gather per layer >= 1."""

@@ -216,6 +216,13 @@ int sparda_decode_step(sparda_ctx* ctx, const sparda_layer* layers, int n_layers
  * Host-side state of the context: set it before the step is enqueued (or captured).                              */
 int sparda_set_step_candidates(sparda_ctx* ctx, int n_cand);
 
+/* (f3 inside a4) The paper's selector geometry in the decode steps: after sparda_set_step_selector(ctx, 1, n_init, n_local)
+ * every selection of sparda_decode_step / _host / _cached is sparda_forecast_select_grid -- layers[l].Kpool then points to the
+ * (32,16) compressed-key grid [R][4 n_blocks][D] of sparda_pool_keys_grid, and ids are init + local + top-k (Eq.1, P:L53;
+ * reading q19: parity unpinned by the paper).  n_init + n_local <= topk.  grid = 0 restores the one-key-per-block form.
+ * The cached step then runs the reuse plan as its own launch behind the select (no doorbell for that layer's gather).  */
+int sparda_set_step_selector(sparda_ctx* ctx, int grid, int n_init, int n_local);
+
 /* The same step for a caller whose per-step tensors live in HOST memory (the end-to-end form bench.py times):
  * layers[l].F, .Q and .O and F0cur are HOST pointers (pinned for the copies to be asynchronous); the call runs
  * sparda_decode_step on staging owned by the context and enqueues the copies on compute_stream just in time: F0cur first,

@@ -22,7 +22,7 @@ EXPORTS = [
     "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
     "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
-    "sparda_probe_launch", "sparda_set_layer_standin", "sparda_enable_peer_tier", "sparda_set_step_candidates",
+    "sparda_probe_launch", "sparda_set_layer_standin", "sparda_enable_peer_tier", "sparda_set_step_candidates", "sparda_set_step_selector",
     "sparda_launch_count", "sparda_tmap_encodes", "sparda_get_select_cluster", "sparda_get_attn_cluster", "sparda_get_attn_splits", "sparda_get_gather_ctas", "sparda_strerror",
     "sparda_last_cuda_error", "sparda_version",
 ]
@@ -86,6 +86,7 @@ def lib() -> ctypes.CDLL:
         L.sparda_set_layer_standin.argtypes = [vp, vp, i64]
         L.sparda_enable_peer_tier.argtypes = [vp, i32]
         L.sparda_set_step_candidates.argtypes = [vp, i32]
+        L.sparda_set_step_selector.argtypes = [vp, i32, i32, i32]
         L.sparda_tmap_encodes.argtypes = [vp]
         L.sparda_tmap_encodes.restype = i64
         L.sparda_get_select_cluster.argtypes = [vp]
@@ -184,6 +185,10 @@ class Sparda:
     def set_step_candidates(self, n_cand: int):
         """Decode steps rank blocks [0, n_cand) only (the complete blocks of a growing cache); 0 = all n_blocks."""
         self._check(self._L.sparda_set_step_candidates(self._h, int(n_cand)), "set_step_candidates")
+
+    def set_step_selector(self, grid: bool, n_init: int = 0, n_local: int = 0):
+        """grid=True: decode steps select with the (32,16) compressed-key grid (Kpool = Kgrid) and force init / local blocks."""
+        self._check(self._L.sparda_set_step_selector(self._h, 1 if grid else 0, int(n_init), int(n_local)), "set_step_selector")
 
     def enable_peer_tier(self, peer_device: int):
         self._check(self._L.sparda_enable_peer_tier(self._h, int(peer_device)), "enable_peer_tier")

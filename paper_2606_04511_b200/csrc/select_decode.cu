@@ -772,7 +772,7 @@ int sparda_launch_select_grid(sparda_ctx* ctx, const void* F, const void* Kgrid,
                               int topk, int32_t* ids, cudaStream_t st) {
     SelParams p;
     p.slot_ids = p.fetch = p.n_fetch = nullptr;
-    p.door = nullptr;
+    p.door = ctx->door_next;
     p.F = (const uint32_t*)F;
     p.ids = ids;
     p.n_blocks = n_blocks;

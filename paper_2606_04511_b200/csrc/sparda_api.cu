@@ -321,7 +321,13 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
         if (rc) return rc;
     }
     SPARDA_PROF_BEGIN(0, cs);
-    rc = sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_cand, topk, layers[0].base.ids, cs);
+    // f3 inside the step (sparda_set_step_selector): Kpool then is the (32,16) compressed-key grid [R][4 n_blocks][D] and every
+    // selection returns init + local + top-k (reading q19, unpinned by the paper)
+    const bool grid = ctx->step_grid != 0;
+    if (grid && ctx->step_n_init + ctx->step_n_local > topk) return SPARDA_EINVAL;
+    rc = grid ? sparda_forecast_select_grid(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_cand, ctx->step_n_init, ctx->step_n_local, topk,
+                                            layers[0].base.ids, cs)
+              : sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_cand, topk, layers[0].base.ids, cs);
     if (rc) return rc;
     SPARDA_PROF_END(0, cs);
     struct PdlScope {   // launches behind an event wait do not ask for PDL (see sparda_ctx::pdl_next); restored on every return
@@ -350,9 +356,15 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
                 ctx->pdl_next = 1;   // the select follows the projection on its own stream, no event in between: its prologue
                                      // and the first ring of pooled keys overlap the projection (0.58 -> 0.55 ms per cached step, batch 4)
             }
-            ctx->door_next = overlap ? ctx->door + (l + 1) : nullptr;   // this select rings the layer's gather (below) row by row
+            // the doorbell needs the list the gather reads to come out of the ringing kernel: not so for grid select + separate plan
+            const bool use_door = overlap && !(grid && nx->slot_ids);
+            ctx->door_next = use_door ? ctx->door + (l + 1) : nullptr;   // this select rings the layer's gather (below) row by row
             SPARDA_PROF_BEGIN(0, xs);
-            if (nx->slot_ids)   // select + reuse plan in one launch
+            if (grid) {
+                rc = sparda_forecast_select_grid(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_cand, ctx->step_n_init, ctx->step_n_local,
+                                                 topk, nx->base.ids, xs);
+                if (!rc && nx->slot_ids) rc = sparda_reuse_plan(ctx, nx->base.ids, topk, nx->slot_ids, nx->fetch, nx->n_fetch, xs);
+            } else if (nx->slot_ids)   // select + reuse plan in one launch
                 rc = sparda_forecast_select_plan(ctx, layers[l].base.F, nx->base.Kpool, n_blocks, n_cand, topk, nx->base.ids,
                                                  nx->slot_ids, nx->fetch, nx->n_fetch, xs);
             else
@@ -365,7 +377,7 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
                 // which also releases the pool it writes) and waits on the device for the doorbell.  ev_sel joins the select
                 // stream back into the compute stream in front of attention l+1 (stream capture needs the join)
                 SPARDA_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sel[l + 1], xs));
-                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(gs, ctx->ev_top[l], 0));
+                SPARDA_CUDA_TRY(ctx, cudaStreamWaitEvent(gs, use_door ? ctx->ev_top[l] : ctx->ev_sel[l + 1], 0));
             }
             SPARDA_PROF_BEGIN(1, gs);
             rc = sparda_prefetch_launch(ctx, nx->base.kv, n_blocks, nx->slot_ids ? nx->fetch : nx->base.ids, topk, nx->pool, gs);
@@ -459,6 +471,15 @@ int sparda_decode_step_host(sparda_ctx* ctx, const sparda_layer* layers, int n_l
     HostIO io = {layers, F0cur, f_bytes, q_bytes};
     return decode_step_impl(ctx, cl, n_layers, ctx->stage_F + f_bytes * ctx->max_layers, n_blocks, topk, cs, (cudaStream_t)prefetch_stream, mode,
                             &io);
+}
+
+int sparda_set_step_selector(sparda_ctx* ctx, int grid, int n_init, int n_local) {
+    if (!ctx || n_init < 0 || n_local < 0 || (grid != 0 && grid != 1)) return SPARDA_EINVAL;
+    if (grid && n_init + n_local > ctx->cfg.topk) return SPARDA_EINVAL;
+    ctx->step_grid = grid;
+    ctx->step_n_init = grid ? n_init : 0;
+    ctx->step_n_local = grid ? n_local : 0;
+    return SPARDA_OK;
 }
 
 int sparda_set_step_candidates(sparda_ctx* ctx, int n_cand) {

@@ -71,6 +71,7 @@ struct sparda_ctx {
     // / gather launch rings / waits on it (the step sets it; stand-alone calls never do).
     unsigned int* door;       // [max_layers + 1]
     unsigned int* door_next;
+    int step_grid, step_n_init, step_n_local;   // sparda_set_step_selector: the steps select with the (32,16) grid form (f3)
     int step_n_cand;          // sparda_set_step_candidates: blocks [0, step_n_cand) are ranked by the decode steps (0 = all n_blocks)
     char cuda_err[256];
     // TMA descriptor cache (host): open-addressed hash on (base, rows, head_dim, box_rows); lookups return a COPY, so an

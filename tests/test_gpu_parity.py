@@ -360,6 +360,79 @@ def test_multi_step_decode_with_growing_cache(sp, oracle):
     ctx.close()
 
 
+def test_decode_step_with_the_grid_selector(sp, oracle):
+    """f3 inside a4 (sparda_set_step_selector; reading q19, parity unpinned by the paper): every selection of the step is the
+    (32,16) grid form with forced initial / local blocks.  Overlapped == serialized bit for bit (the doorbell is rung by the grid
+    kernel too), every layer against o15 on the GPU's own compressed keys, gather bytes and attention against o5 / o6; then the
+    cached step (select, separate plan, gather ordered by an event) against o11 on the GPU's selections."""
+    cfg = G16.with_(n_layers=4, batch=3)
+    n_init, n_local = 1, 8
+    ctx = sp.Sparda.from_config(cfg, max_layers=4)
+    data = _pipeline_inputs(cfg, sp)
+    R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim
+    dev = []
+    for l, (L, kv_host) in enumerate(data):
+        kgrid = torch.empty((R, 4 * Nb, D), dtype=torch.bfloat16, device="cuda")
+        ctx.pool_keys_grid(L["kv"], R, Nb, kgrid)
+        dev.append({"F": L["F"], "Q": L["Q"], "Kpool": kgrid, "kv": L["kv"] if l == 0 else kv_host,
+                    "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                    "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda")})
+    F0 = data[0][0]["F0cur"]
+    arr = ctx.make_layers(dev)
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
+    with pytest.raises(sp.SpardaError):
+        ctx.set_step_selector(True, 40, 40)                          # forced blocks exceed the budget
+    ctx.set_step_selector(True, n_init, n_local)
+    res = {}
+    for mode in (sp.STEP_SERIAL, sp.STEP_OVERLAP):
+        pools = [torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+        for d in dev:
+            d["O"].zero_()
+            d["ids"].fill_(-9)
+        torch.cuda.synchronize()
+        ctx.decode_step(arr, F0, Nb, k, pools[0], pools[1], cs, ps, mode)
+        torch.cuda.synchronize()
+        res[mode] = ([d["O"].clone() for d in dev], [d["ids"].clone() for d in dev])
+    for a, b in zip(res[sp.STEP_SERIAL][0] + res[sp.STEP_SERIAL][1], res[sp.STEP_OVERLAP][0] + res[sp.STEP_OVERLAP][1]):
+        assert torch.equal(a.view(torch.int16) if a.dtype == torch.bfloat16 else a, b.view(torch.int16) if b.dtype == torch.bfloat16 else b)
+    Os, idss = res[sp.STEP_OVERLAP]
+    for l, (L, kv_host) in enumerate(data):
+        f = _bits(F0) if l == 0 else _bits(data[l - 1][0]["F"])
+        want, bs = oracle.forecast_select_grid(f, _bits(dev[l]["Kpool"]), k, Nb, n_init, n_local)
+        gids = idss[l].cpu().numpy()
+        forced = [b for b in range(Nb) if b < n_init or b >= Nb - n_local]
+        assert all(set(forced) <= set(gids[r].tolist()) for r in range(R))
+        parity.check_ids(gids, want, np.where(np.isinf(bs), np.float32(3.0e38), bs), Nb)
+        kvb = _bits(L["kv"])
+        if l == 0:
+            wantO, _ = oracle.sparse_attn(_bits(L["Q"]), kvb, gids, pool_is_indexed=True)
+        else:
+            wantO, _ = oracle.sparse_attn(_bits(L["Q"]), oracle.gather(kvb, gids), gids)
+        parity.check_attn(_bits(Os[l]), wantO, f"grid step layer {l}")
+    # cached step with the grid selector: plan as its own launch, fetch lists against o11 on the GPU's ids
+    cl = []
+    for l, d in enumerate(dev):
+        e = dict(d)
+        if l:
+            e["pool"] = torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+            e["slot_ids"] = torch.full((R, k), -1, dtype=torch.int32, device="cuda")
+            e["fetch"] = torch.full((R, k), -7, dtype=torch.int32, device="cuda")
+            e["n_fetch"] = torch.zeros((R,), dtype=torch.int32, device="cuda")
+        cl.append(e)
+    carr = ctx.make_cached_layers(cl)
+    ctx.decode_step_cached(carr, F0, Nb, k, cs, ps, sp.STEP_OVERLAP)
+    torch.cuda.synchronize()
+    for l in range(1, cfg.n_layers):
+        assert torch.equal(cl[l]["ids"], idss[l])
+        slots, fetch = oracle.reuse_plan(idss[l].cpu().numpy(), np.full((R, k), -1, dtype=np.int32))
+        np.testing.assert_array_equal(cl[l]["slot_ids"].cpu().numpy(), slots)
+        np.testing.assert_array_equal(cl[l]["fetch"].cpu().numpy(), fetch)
+        # empty slot tables: block j of the selection lands in slot j, the pool equals the plain step's, and so does O
+        assert torch.equal(cl[l]["O"].view(torch.int16), Os[l].view(torch.int16))
+    ctx.set_step_selector(False)
+    ctx.close()
+
+
 def test_decode_step_host_buffers_and_profile(sp):
     """The host-buffer form of the step (what bench.py's e2e times) gives bit-identical O to the device form;
     per-kernel profiling reports one select and one attention per layer and one gather per layer >= 1."""

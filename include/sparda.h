@@ -52,6 +52,7 @@ extern "C" {
 #define SPARDA_EUNSUPPORTED (-2) /* device is not sm_100 (B200) */
 #define SPARDA_ECUDA (-3)        /* a CUDA runtime / driver call failed; see sparda_last_cuda_error */
 #define SPARDA_ENOMEM (-4)       /* workspace allocation failed in sparda_create */
+#define SPARDA_ELIMIT (-5)       /* shape beyond the fixed capacity of sparda_sparse_decode_noalloc's built-in scratch array */
 
 #define SPARDA_GATHER_TMA 0 /* persistent single-thread-per-CTA bulk-copy (TMA) ring: host -> smem -> HBM */
 #define SPARDA_GATHER_LDG 1 /* persistent warps issuing 16-byte vector loads from mapped host memory */
@@ -190,6 +191,39 @@ int sparda_enable_peer_tier(sparda_ctx* ctx, int peer_device);
  * intermediate state in shared memory and may overlap freely.)                                                  */
 int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, int topk,
                          int pool_is_indexed, int n_slots, void* O, void* stream);
+
+/* (a5/a6) The same attention for callers that must not allocate device memory, and so cannot use sparda_create at all
+ * (it calls cudaMalloc for the split-K workspace, creates a stream and events).  Who that is:
+ *   - a serving engine that hands the whole of HBM to its own pool at start-up: a later cudaMalloc from a library fails,
+ *     or takes memory the engine's accounting believes it owns;
+ *   - a latency-critical decode loop that cannot afford the device-wide synchronisation cudaMalloc / cudaFree imply;
+ *   - a plug-in or custom op that is handed pointers and a stream and has no start-up or shut-down hook in which a
+ *     context could be created and destroyed.
+ * This call takes no context.  Same kernel as sparda_sparse_decode (the flat split-K form, CTA partials merged by the
+ * last CTA of each row), same arguments and layouts; the shape that a context would carry is passed as plain integers.
+ * The split-K partials and the per-row tickets live in ONE fixed array compiled into the library
+ * (SPARDA_NOALLOC_SCRATCH_BYTES = 4 260 864 bytes, about 4.1 MiB): every GPU on which the process loads libsparda holds
+ * that much from module load until the process exits, whether or not this call is ever made.
+ *   Limits: R = batch * n_kv_heads <= SPARDA_NOALLOC_MAX_ROWS (256); the CTAs-per-row split is chosen so that R * (partials
+ *   per row) <= SPARDA_NOALLOC_MAX_PARTIALS (512), which every R within the limit allows.  A larger R returns SPARDA_ELIMIT
+ *   and sparda_noalloc_last_error() names the limit.  Other shape rules are sparda_create's (G in {1,2,4,8,16},
+ *   head_dim in {64,128}, topk <= 256, n_slots <= 8192; pool_is_indexed = 0 requires n_slots == topk): SPARDA_EINVAL.
+ *   Set-up: the FIRST call on each device (with that device current, as for every call) resolves the device address of the
+ *   array, the TMA descriptor encoder and the kernel's shared-memory opt-in; make that first call during start-up, before
+ *   any stream capture begins.  Neither the first nor any later call calls cudaMalloc, cudaFree or any routine that
+ *   allocates device memory; the only extra work enqueued on `stream` is a cudaMemsetAsync of the R tickets in front of the
+ *   kernel (the array keeps whatever the previous call left, the tickets must start at zero).
+ *   Sharing: every call on a device uses the same array.  Two calls that can run on the GPU at the same time (different
+ *   streams without an event between them) race on it and give wrong output; calls on one stream are safe.  Host side, the
+ *   call is serialised by a lock and may be made from any thread.
+ * Returns SPARDA_OK (enqueued), SPARDA_EINVAL, SPARDA_ELIMIT, SPARDA_EUNSUPPORTED (not an sm_100 device) or SPARDA_ECUDA;
+ * sparda_noalloc_last_error() returns the calling thread's last failure of this entry point as text ("" if none).  */
+#define SPARDA_NOALLOC_MAX_ROWS 256
+#define SPARDA_NOALLOC_MAX_PARTIALS 512
+#define SPARDA_NOALLOC_SCRATCH_BYTES (SPARDA_NOALLOC_MAX_PARTIALS * (16 * 128 * 4 + 2 * 16 * 4) + SPARDA_NOALLOC_MAX_ROWS * 4)
+int sparda_sparse_decode_noalloc(int batch, int n_q_heads, int n_kv_heads, int head_dim, const void* Q, const void* dev_pool,
+                                 const int32_t* ids, int topk, int pool_is_indexed, int n_slots, void* O, void* stream);
+const char* sparda_noalloc_last_error(void);
 
 /* (a4 + a6) One decode step over n_layers layers in Algorithm-2 order with the one-layer-ahead
  * pipeline: layer 0 selects with F0cur against its own Kpool and attends straight from its device-resident

@@ -19,7 +19,7 @@ STEP_OVERLAP, STEP_SERIAL = 0, 1
 
 EXPORTS = [
     "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_project", "sparda_append_kv", "sparda_pool_keys_grid", "sparda_forecast_select_grid", "sparda_forecast_select", "sparda_prefetch_launch",
-    "sparda_sparse_decode", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
+    "sparda_sparse_decode", "sparda_sparse_decode_noalloc", "sparda_noalloc_last_error", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
     "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
     "sparda_probe_launch", "sparda_set_layer_standin", "sparda_enable_peer_tier", "sparda_set_step_candidates", "sparda_set_step_selector",
@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
         L.sparda_forecast_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_prefetch_launch.argtypes = [vp, vp, i32, vp, i32, vp, vp]
         L.sparda_sparse_decode.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
+        L.sparda_sparse_decode_noalloc.argtypes = [i32, i32, i32, i32, vp, vp, vp, i32, i32, i32, vp, vp]
+        L.sparda_noalloc_last_error.argtypes = []
         L.sparda_decode_step.argtypes = [vp, ctypes.POINTER(SpardaLayer), i32, vp, i32, i32, vp, vp, vp, vp, i32]
         L.sparda_decode_step_host.argtypes = L.sparda_decode_step.argtypes
         L.sparda_reuse_plan.argtypes = [vp, vp, i32, vp, vp, vp, vp]
@@ -93,7 +95,7 @@ def lib() -> ctypes.CDLL:
         L.sparda_get_attn_cluster.argtypes = [vp]
         L.sparda_get_attn_splits.argtypes = [vp, i32]
         L.sparda_get_gather_ctas.argtypes = [vp]
-        for f in ("sparda_strerror", "sparda_last_cuda_error", "sparda_version"):
+        for f in ("sparda_strerror", "sparda_last_cuda_error", "sparda_version", "sparda_noalloc_last_error"):
             getattr(L, f).restype = ctypes.c_char_p
         L.sparda_strerror.argtypes = [i32]
         L.sparda_last_cuda_error.argtypes = [vp]
@@ -296,6 +298,24 @@ class Sparda:
     @property
     def gather_ctas(self) -> int:
         return int(self._L.sparda_get_gather_ctas(self._h))
+
+
+NOALLOC_MAX_ROWS = 256          # SPARDA_NOALLOC_MAX_ROWS
+NOALLOC_SCRATCH_BYTES = 512 * (16 * 128 * 4 + 2 * 16 * 4) + 256 * 4   # SPARDA_NOALLOC_SCRATCH_BYTES
+
+
+def sparse_decode_noalloc(batch, n_q_heads, n_kv_heads, head_dim, Q, dev_pool, ids, topk, O, pool_is_indexed=False,
+                          n_slots=None, stream=None):
+    """sparda_sparse_decode_noalloc: block-sparse attention without a context, for callers that must not allocate device
+    memory (an engine that owns all of HBM, a loop that cannot take cudaMalloc's synchronisation, a plug-in with no set-up
+    hook).  The split-K workspace is a fixed array inside libsparda (NOALLOC_SCRATCH_BYTES per GPU, rows <= NOALLOC_MAX_ROWS),
+    shared by every call on the device: calls that may overlap on the GPU race.  Marshalling only."""
+    L = lib()
+    n_slots = topk if n_slots is None else n_slots
+    rc = L.sparda_sparse_decode_noalloc(int(batch), int(n_q_heads), int(n_kv_heads), int(head_dim), _ptr(Q), _ptr(dev_pool),
+                                        _ptr(ids), int(topk), 1 if pool_is_indexed else 0, int(n_slots), _ptr(O), _stream(stream))
+    if rc != 0:
+        raise SpardaError(f"sparse_decode_noalloc: {L.sparda_strerror(rc).decode()} [{rc}]: {L.sparda_noalloc_last_error().decode()}")
 
 
 def version() -> str:

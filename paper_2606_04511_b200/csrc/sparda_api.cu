@@ -24,6 +24,7 @@ const char* sparda_strerror(int code) {
         case SPARDA_EUNSUPPORTED: return "unsupported device (libsparda needs an sm_100 GPU)";
         case SPARDA_ECUDA: return "CUDA call failed (see sparda_last_cuda_error)";
         case SPARDA_ENOMEM: return "workspace allocation failed";
+        case SPARDA_ELIMIT: return "shape beyond the fixed capacity of the no-allocation entry point (see sparda_noalloc_last_error)";
         default: return "unknown error code";
     }
 }

@@ -643,3 +643,184 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     ctx->launches++;
     return SPARDA_OK;
 }
+
+// =================================================================================================================
+// sparda_sparse_decode_noalloc (include/sparda.h): the attention above for callers that may not allocate device
+// memory -- an engine that gave all of HBM to its own pool, a decode loop that cannot take cudaMalloc's device-wide
+// synchronisation, a plug-in with no set-up hook.  Such a caller cannot use sparda_create (cudaMalloc, stream and event
+// creation), so this entry point takes no context: the launcher state a context would hold sits in a host-side table with
+// one entry per device, and the split-K workspace (CTA partials + per-row tickets) is the fixed array below instead of
+// cudaMalloc'ed memory.  The kernel is sparse_decode_kernel<D, 4, 1, false> unchanged -- the flat split whose row
+// partials are merged by the last CTA to finish the row -- with its three workspace pointers aimed into the array.
+//
+// The array is part of this translation unit's device image: the driver places it on every GPU that loads the image and
+// keeps it until the process exits.  In HOST code the name `g_noalloc_scratch` is only a handle for the runtime's symbol
+// table -- it is not a device address, and a kernel given `&g_noalloc_scratch[0]` from the host would fault or scribble
+// over host memory.  The device address is asked for once per device with cudaGetSymbolAddress (noalloc_setup) and that
+// pointer is what the kernel receives.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[SPARDA_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int NA_MAX_DEVICES = 16;   // device ordinals this table covers
+constexpr size_t NA_PART_O_BYTES = (size_t)SPARDA_NOALLOC_MAX_PARTIALS * 16 * 128 * sizeof(float);   // [partials][16][D <= 128]
+constexpr size_t NA_PART_ML_BYTES = (size_t)SPARDA_NOALLOC_MAX_PARTIALS * 2 * 16 * sizeof(float);    // [partials][2][16]
+constexpr size_t NA_TICKET_BYTES = (size_t)SPARDA_NOALLOC_MAX_ROWS * sizeof(unsigned int);           // [rows]
+static_assert(NA_PART_O_BYTES + NA_PART_ML_BYTES + NA_TICKET_BYTES == SPARDA_NOALLOC_SCRATCH_BYTES,
+              "sparda.h states the array's size; keep the layout and the figure together");
+static_assert(SPARDA_NOALLOC_MAX_PARTIALS >= 2 * SPARDA_NOALLOC_MAX_ROWS,
+              "a row of the flat split may meet two CTAs: every admitted R needs at least two partial slots per row");
+
+struct NoallocDevice {
+    bool ready;
+    unsigned char* scratch;   // DEVICE address of g_noalloc_scratch on this device (cudaGetSymbolAddress)
+    sparda_ctx ctx;           // launcher state only (descriptor cache, attribute flags, shape of the current call): no device memory
+};
+NoallocDevice g_na[NA_MAX_DEVICES];   // host memory, static: nothing is allocated on the host either
+std::mutex g_na_lock;
+thread_local char g_na_err[384];
+
+int na_fail(int code, const char* fmt, ...) __attribute__((format(printf, 2, 3)));
+int na_fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_na_err, sizeof(g_na_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+int na_fail_cuda(cudaError_t e, const char* where) {
+    (void)cudaGetLastError();
+    return na_fail(SPARDA_ECUDA, "%s: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e), where);
+}
+
+// Once per device, with that device current.  Everything here is a query or a per-function attribute: no cudaMalloc, no
+// stream, no event.  Run it (= make the first call on the device) before any stream capture begins.
+int noalloc_setup(NoallocDevice& d, int dev) {
+    int major = 0, sms = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaDeviceGetAttribute");
+    if (major != 10) return na_fail(SPARDA_EUNSUPPORTED, "device %d has compute capability %d.x; libsparda's kernels are sm_100a only", dev, major);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
+    if (qres != cudaDriverEntryPointSuccess || !fn) return na_fail(SPARDA_EUNSUPPORTED, "the driver does not export cuTensorMapEncodeTiled");
+    unsigned char* ptr = nullptr;
+    e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch);   // the array's address ON THIS DEVICE
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaGetSymbolAddress(g_noalloc_scratch)");
+    if (!ptr) return na_fail(SPARDA_ECUDA, "cudaGetSymbolAddress(g_noalloc_scratch) returned a null device address");
+    e = cudaFuncSetAttribute(sparse_decode_kernel<128, ATT_NW, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128, ATT_NW>::TOTAL);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(sparse_decode_kernel<64, ATT_NW, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64, ATT_NW>::TOTAL);
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaFuncSetAttribute(sparse_decode_kernel, MaxDynamicSharedMemorySize)");
+    memset(&d.ctx, 0, sizeof(d.ctx));
+    d.ctx.device = dev;
+    d.ctx.sm_count = sms;
+    d.ctx.encode_fn = fn;
+    d.ctx.cfg.block_size = S_BLK;
+    d.ctx.cfg.no_pdl = 1;   // plain stream order behind the ticket memset
+    d.ctx.kstate[SPARDA_K_ATTN_128].attr_set = true;
+    d.ctx.kstate[SPARDA_K_ATTN_64].attr_set = true;
+    d.scratch = ptr;
+    d.ready = true;
+    return SPARDA_OK;
+}
+
+}  // namespace
+
+extern "C" const char* sparda_noalloc_last_error(void) { return g_na_err; }
+
+extern "C" int sparda_sparse_decode_noalloc(int batch, int n_q_heads, int n_kv_heads, int head_dim, const void* Q, const void* dev_pool,
+                                            const int32_t* ids, int topk, int pool_is_indexed, int n_slots, void* O, void* stream) {
+    g_na_err[0] = 0;
+    // ---- shape and pointer checks: no CUDA call before they pass
+    if (!sparda_aligned(Q, 16) || !sparda_aligned(dev_pool, 16) || !sparda_aligned(O, 16) || !sparda_aligned(ids, 4))
+        return na_fail(SPARDA_EINVAL, "null or misaligned pointer (Q, dev_pool, O: 16 bytes; ids: 4 bytes)");
+    if (batch < 1 || n_kv_heads < 1 || n_q_heads < 1 || n_q_heads % n_kv_heads != 0)
+        return na_fail(SPARDA_EINVAL, "batch %d, n_q_heads %d, n_kv_heads %d: need positive counts and n_q_heads a multiple of n_kv_heads", batch, n_q_heads, n_kv_heads);
+    const int G = n_q_heads / n_kv_heads;
+    if (!(G == 1 || G == 2 || G == 4 || G == 8 || G == 16)) return na_fail(SPARDA_EINVAL, "G = n_q_heads / n_kv_heads = %d: supported 1, 2, 4, 8, 16", G);
+    if (head_dim != 64 && head_dim != 128) return na_fail(SPARDA_EINVAL, "head_dim %d: supported 64 and 128", head_dim);
+    if (topk < 1 || topk > 256) return na_fail(SPARDA_EINVAL, "topk %d: supported 1..256", topk);
+    if (pool_is_indexed ? (n_slots < 1 || n_slots > 8192) : (n_slots != topk))
+        return na_fail(SPARDA_EINVAL, "n_slots %d: 1..8192 blocks per row for an indexed cache, else exactly topk (%d)", n_slots, topk);
+    const long long R = (long long)batch * n_kv_heads;
+    if (R > SPARDA_NOALLOC_MAX_ROWS)
+        return na_fail(SPARDA_ELIMIT,
+                       "batch * n_kv_heads = %lld rows, but the built-in scratch array holds tickets and split-K partials for at most "
+                       "SPARDA_NOALLOC_MAX_ROWS = %d rows (%d bytes in all): split the batch over several calls on one stream, or use "
+                       "sparda_create + sparda_sparse_decode where allocating is allowed",
+                       R, SPARDA_NOALLOC_MAX_ROWS, (int)SPARDA_NOALLOC_SCRATCH_BYTES);
+
+    std::lock_guard<std::mutex> guard(g_na_lock);
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaGetDevice");
+    if (dev < 0 || dev >= NA_MAX_DEVICES) return na_fail(SPARDA_ELIMIT, "device ordinal %d: the per-device table covers ordinals 0..%d", dev, NA_MAX_DEVICES - 1);
+    NoallocDevice& d = g_na[dev];
+    if (!d.ready) {
+        const int rc = noalloc_setup(d, dev);
+        if (rc) return rc;
+    }
+
+    // ---- the shape a context would carry, for this call
+    sparda_ctx* ctx = &d.ctx;
+    ctx->cfg.batch = batch;
+    ctx->cfg.n_q_heads = n_q_heads;
+    ctx->cfg.n_kv_heads = n_kv_heads;
+    ctx->cfg.head_dim = head_dim;
+    ctx->cfg.topk = topk;
+    ctx->R = (int)R;
+    ctx->G = G;
+    {   // partial slots per row: what sparda_create would give (ceil(2 * SMs / R) CTAs per row + 2), cut to the array's capacity;
+        // sparda_resolve_attn_ctas then keeps every row within that many CTAs (>= 2 for every admitted R)
+        int per_row = (2 * ctx->sm_count + ctx->R - 1) / ctx->R;
+        if (per_row > topk) per_row = topk;
+        ctx->max_splits = per_row + 2;
+        if (ctx->max_splits > SPARDA_NOALLOC_MAX_PARTIALS / ctx->R) ctx->max_splits = SPARDA_NOALLOC_MAX_PARTIALS / ctx->R;
+    }
+    ctx->part_O = reinterpret_cast<float*>(d.scratch);
+    ctx->part_ml = reinterpret_cast<float*>(d.scratch + NA_PART_O_BYTES);
+    ctx->tickets = reinterpret_cast<unsigned int*>(d.scratch + NA_PART_O_BYTES + NA_PART_ML_BYTES);
+
+    cudaStream_t st = (cudaStream_t)stream;
+    CUtensorMap map;
+    if (sparda_get_tmap(ctx, dev_pool, (uint64_t)ctx->R * n_slots * 2 * S_BLK, head_dim, S_BLK, &map) != SPARDA_OK)
+        return na_fail(SPARDA_ECUDA, "%s", ctx->cuda_err);
+    AttnParams p;
+    p.Q = (const uint32_t*)Q;
+    p.ids = ids;
+    p.O = (__nv_bfloat16*)O;
+    p.part_O = ctx->part_O;
+    p.part_ml = ctx->part_ml;
+    p.tickets = ctx->tickets;
+    p.topk = topk;
+    p.indexed = pool_is_indexed ? 1 : 0;
+    p.n_slots = n_slots;
+    p.Hq = n_q_heads;
+    p.Hkv = n_kv_heads;
+    p.G = G;
+    p.max_splits = ctx->max_splits;
+    p.W = ctx->R * topk;
+    p.scale_log2 = 1.4426950408889634f / sqrtf((float)head_dim);
+    const int C = sparda_resolve_attn_ctas(ctx, topk);
+    p.quota = p.W / C;
+    p.rem = p.W % C;
+    // The array keeps the previous call's contents.  Partials are written before they are read within one launch, so they need
+    // no clearing; the tickets count arrivals from zero, and a launch that was cut short (or a foreign write) must not leak
+    // into this one: clear this call's R tickets in stream order in front of the kernel.
+    e = cudaMemsetAsync(ctx->tickets, 0, (size_t)ctx->R * sizeof(unsigned int), st);
+    if (e != cudaSuccess) return na_fail_cuda(e, "cudaMemsetAsync(tickets)");
+    const int rc = head_dim == 128 ? launch<128, false>(ctx, &map, p, C, 1, st) : launch<64, false>(ctx, &map, p, C, 1, st);
+    if (rc) return na_fail(rc, "%s", ctx->cuda_err);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return na_fail_cuda(e, "sparse_decode_kernel launch");
+    ctx->launches++;
+    return SPARDA_OK;
+}

@@ -5,7 +5,9 @@ the paper passage each function follows).  Written here, as plain Python / numpy
 ``decode_pipeline`` (o10: Algorithm 2 lines 4-7, strictly in order), ``reuse_plan`` /
 ``decode_pipeline_cached`` (o11 / o12: the previous-step block cache, reading q18), ``append_kv`` (o13: Algorithm 2
 lines 2-3) and ``pool_keys_grid`` / ``forecast_select_grid`` (o14 / o15: the (32,16) compressed-key grid with
-the max-pool to blocks, reading q19 -- PARITY UNPINNED BY THE PAPER, which does not state the pooling geometry).
+the max-pool to blocks, reading q19 -- PARITY UNPINNED BY THE PAPER, which does not state the pooling geometry) and
+``sparse_attn_len`` (o16: Eq.5 over a cache whose last block is partly filled, Algorithm 2 line 2 P:L300 + Eq.1 P:L53-56,
+reading q7).
 Every function is pinned in ``tests/test_oracle_pins.py``.
 
 bf16 tensors are numpy ``uint16`` arrays holding the raw upper halves of fp32 values.
@@ -394,3 +396,55 @@ def forecast_select_grid(F: np.ndarray, kgrid: np.ndarray, k_total: int, n_cand:
         for b in forced:
             bs[r, b] = np.inf
     return ids, bs
+
+
+def sparse_attn_len(Q: np.ndarray, pool: np.ndarray, ids: np.ndarray, seq_len: np.ndarray, pool_is_indexed: bool = False):
+    """o16: o6 (Eq.5) over the tokens that exist.  Row r's cache holds seq_len[r] tokens: the new token's K / V is appended
+    before the attention (Alg.2 l.2) and the local window that holds it is always attended (Eq.1), so the
+    newest block is in general partly filled (reading q7).  Block j of row r holds the tokens S*j .. S*j + S - 1; it contributes
+    its first min(S, seq_len[r] - S*j) tokens, nothing when that is <= 0; whatever bytes sit behind them in the block are
+    never read.  Otherwise Eq.5 as in o6: z_t = q . k_t / sqrt(D), softmax over every contributing token of every
+    listed block (id >= 0), O = sum_t p_t v_t; fp64 throughout, one rounding to bf16.  A head with no token gives O = 0.
+    Q [B][Hq][D], pool [R][n_slots][2][S][D] (slot i holds block ids[r][i], or the cache addressed by id when
+    pool_is_indexed), ids [R][k] (block ids, -1 = none), seq_len [R] -> (O bf16 bits, O float64).  Plain loops; small cases."""
+    Q, pool = _u16(Q), _u16(pool)
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    seq_len = np.ascontiguousarray(seq_len, dtype=np.int64)
+    B, Hq, D = Q.shape
+    R, n_slots, two, S, D2 = pool.shape
+    assert two == 2 and D2 == D and R % B == 0 and ids.shape[0] == R and seq_len.shape == (R,)
+    Hkv = R // B
+    G = Hq // Hkv
+    k = ids.shape[1]
+    assert n_slots == k or pool_is_indexed
+    Qf = bf16_bits_to_f64(Q)
+    O64 = np.zeros((B, Hq, D), dtype=np.float64)
+    O = np.zeros((B, Hq, D), dtype=np.uint16)
+    for b in range(B):
+        for h in range(Hq):
+            r = b * Hkv + h // G
+            z, vs = [], []
+            for i in range(k):
+                j = int(ids[r, i])
+                if j < 0:
+                    continue
+                n_tok = min(S, int(seq_len[r]) - S * j)
+                if n_tok <= 0:
+                    continue
+                blk = pool[r, j if pool_is_indexed else i]
+                Kt = bf16_bits_to_f64(blk[0, :n_tok])
+                Vt = bf16_bits_to_f64(blk[1, :n_tok])
+                for t in range(n_tok):
+                    z.append(float(np.dot(Qf[b, h], Kt[t])) / np.sqrt(float(D)))
+                    vs.append(Vt[t])
+            if not z:
+                continue
+            z = np.array(z)
+            pr = np.exp(z - z.max())
+            pr = pr / pr.sum()
+            acc = np.zeros(D)
+            for t in range(len(z)):
+                acc += pr[t] * vs[t]
+            O64[b, h] = acc
+            O[b, h] = [double_to_bf16(float(x)) for x in acc]
+    return O, O64

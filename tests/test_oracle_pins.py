@@ -581,3 +581,93 @@ def test_paper_closed_forms_golden():
     assert round(synth.CFG4_128K.n_layers * synth.CFG4_128K.kv_bytes_per_layer / 1e9) == vals["kv_gb_batch32_128k"]
     assert c.block_bytes == 32 * 1024 and c.context == 131072 and synth.CFG2_32K.context == 32768
     assert synth.CFG1_TINY.context == 4096 and synth.CFG1_TINY.block_bytes == 16 * 1024
+
+
+# ---------------------------------------------------------------- o16: attention over a partly filled newest block
+def test_sparse_attn_len_all_blocks_plus_tail_is_dense_attention_over_T_tokens(oracle):
+    """(o16 pin 1) Every complete block + the open block listed, seq_len = 64 n + r per row  =>  dense softmax attention over
+    the first seq_len[r] tokens of the row: torch's scaled_dot_product_attention on the flattened token axis (a library
+    routine that knows nothing about blocks) and an independent numpy softmax.  Rows have different lengths; one ends exactly
+    on a block boundary, one holds a single token.  Pins Alg.2 l.2 (the appended token is attended) + Eq.5."""
+    L = _layer(SMALL)
+    R, Nb, _, S, D = L["kv"].shape
+    B, Hq, G, Hkv = SMALL.batch, SMALL.n_q_heads, SMALL.group, SMALL.n_kv_heads
+    seq_len = np.array([5 * S + 17, 7 * S, 1, Nb * S - 1], dtype=np.int64)[:R]
+    assert len(seq_len) == R
+    ids = np.tile(np.arange(Nb, dtype=np.int32), (R, 1))              # every block: those beyond seq_len must contribute nothing
+    O, O64 = oracle.sparse_attn_len(L["Q"], L["kv"], ids, seq_len, pool_is_indexed=True)
+    kvf = bf.bits_to_f64(L["kv"])
+    Qf = bf.bits_to_f64(L["Q"])
+    for r in range(R):
+        b, g = divmod(r, Hkv)
+        T = int(seq_len[r])
+        K = kvf[r, :, 0].reshape(Nb * S, D)[:T]
+        V = kvf[r, :, 1].reshape(Nb * S, D)[:T]
+        q = Qf[b, g * G:(g + 1) * G]
+        z = q @ K.T / np.sqrt(D)
+        p = np.exp(z - z.max(axis=1, keepdims=True))
+        p /= p.sum(axis=1, keepdims=True)
+        np.testing.assert_allclose(O64[b, g * G:(g + 1) * G], p @ V, rtol=0, atol=1e-12)
+        ref = torch.nn.functional.scaled_dot_product_attention(torch.from_numpy(q).reshape(1, G, 1, D), torch.from_numpy(K).expand(1, G, T, D),
+                                                               torch.from_numpy(V).expand(1, G, T, D))
+        np.testing.assert_allclose(O64[b, g * G:(g + 1) * G], ref.reshape(G, D).numpy(), rtol=0, atol=1e-12)
+    np.testing.assert_array_equal(O, bf.f64_to_bf16_bits(np.where(np.abs(O64) < 1e-30, 0.0, O64)))
+
+
+def test_sparse_attn_len_reduces_to_o6_and_ignores_what_lies_behind_the_tail(oracle):
+    """(o16 pins 2-5) seq_len = Nb * S (every block complete) reproduces o6 bit for bit in both pool forms; tokens behind
+    seq_len are never read (NaN there changes nothing); a listed block that lies wholly beyond seq_len counts like id -1; a row
+    with seq_len 0 gives O = 0; a tail of one token with V = c for that token alone gives O = c."""
+    L = _layer(SMALL)
+    R, Nb, _, S, D = L["kv"].shape
+    kp = oracle.pool_keys(L["kv"])
+    ids, _ = oracle.forecast_select(L["F"], kp, SMALL.topk)
+    ids[1, -2:] = -1
+    pool = oracle.gather(L["kv"], ids)
+    full = np.full(R, Nb * S, dtype=np.int64)
+    O6, O6_64 = oracle.sparse_attn(L["Q"], pool, ids)
+    Ol, Ol64 = oracle.sparse_attn_len(L["Q"], pool, ids, full)
+    np.testing.assert_array_equal(Ol, O6)
+    np.testing.assert_allclose(Ol64, O6_64, rtol=0, atol=1e-12)
+    Oi, _ = oracle.sparse_attn_len(L["Q"], L["kv"], ids, full, pool_is_indexed=True)
+    np.testing.assert_array_equal(Oi, O6)
+    # the open block is the highest listed id of each row; cut it to 9 tokens and poison what lies behind
+    seq_len = np.array([int(ids[r][ids[r] >= 0].max()) * S + 9 for r in range(R)], dtype=np.int64)
+    kv_nan = L["kv"].copy()
+    for r in range(R):
+        j = int(seq_len[r]) // S
+        kv_nan[r, j, :, 9:] = 0x7FC0                                  # NaN behind the tail, K and V
+        kv_nan[r, j + 1:] = 0x7FC0                                    # and in every later block
+    Oa, Oa64 = oracle.sparse_attn_len(L["Q"], L["kv"], ids, seq_len, pool_is_indexed=True)
+    Ob, Ob64 = oracle.sparse_attn_len(L["Q"], kv_nan, ids, seq_len, pool_is_indexed=True)
+    assert np.all(np.isfinite(Ob64))
+    np.testing.assert_array_equal(Oa, Ob)
+    assert not np.array_equal(Oa, O6), "cutting the newest block to 9 tokens must change O"
+    want = np.zeros_like(Oa64)
+    Qf, kvf = bf.bits_to_f64(L["Q"]), bf.bits_to_f64(L["kv"])
+    for b in range(SMALL.batch):
+        for h in range(SMALL.n_q_heads):
+            r = b * SMALL.n_kv_heads + h // SMALL.group
+            toks = [(j, t) for j in ids[r] if j >= 0 for t in range(S) if j * S + t < seq_len[r]]
+            K = np.stack([kvf[r, j, 0, t] for j, t in toks])
+            V = np.stack([kvf[r, j, 1, t] for j, t in toks])
+            z = K @ Qf[b, h] / np.sqrt(D)
+            p = np.exp(z - z.max())
+            want[b, h] = (p / p.sum()) @ V
+    np.testing.assert_allclose(Oa64, want, rtol=0, atol=1e-12)
+    # a listed block wholly beyond seq_len == that slot set to -1
+    ids_cut = ids.copy()
+    short = seq_len - 9 - S                                           # the open block and the one before it lie beyond
+    for r in range(R):
+        ids_cut[r][ids[r] * S >= short[r]] = -1
+    Oc, _ = oracle.sparse_attn_len(L["Q"], L["kv"], ids, short, pool_is_indexed=True)
+    Od, _ = oracle.sparse_attn(L["Q"], L["kv"], ids_cut, pool_is_indexed=True)
+    np.testing.assert_array_equal(Oc, Od)
+    # empty rows -> zeros; a single attended token -> its V row exactly
+    Oz, Oz64 = oracle.sparse_attn_len(L["Q"], L["kv"], ids, np.zeros(R, dtype=np.int64), pool_is_indexed=True)
+    assert not Oz.any() and not Oz64.any()
+    one = np.tile(np.array([[0] + [-1] * (SMALL.topk - 1)], dtype=np.int32), (R, 1))
+    O1, _ = oracle.sparse_attn_len(L["Q"], L["kv"], one, np.ones(R, dtype=np.int64), pool_is_indexed=True)
+    for b in range(SMALL.batch):
+        for h in range(SMALL.n_q_heads):
+            np.testing.assert_array_equal(O1[b, h], L["kv"][b * SMALL.n_kv_heads + h // SMALL.group, 0, 1, 0])

@@ -42,9 +42,24 @@ constexpr int GATHER_WIN = 1024;  // tasks compacted per window (32 per lane, he
 // first compacts the valid tasks of a window with ballots -- every CTA scans the whole window, CTA c takes the c-th
 // equal share of the VALID tasks, so the split is balanced whatever the pattern -- then lane 0 drives the bulk-copy
 // ring over its share.  An empty list costs one scan (a few microseconds), not one dependent load per slot.
-// door != nullptr (overlapped decode step): the launch is already resident when the layer's select runs; it waits for the
+// DOOR (overlapped decode step): the launch is already resident when the layer's select runs; it waits for the
 // select's doorbell (n_rows rows published) instead of for a kernel boundary, and reads ids only after it.
-__global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__ host_kv, const int32_t* __restrict__ ids,
+//
+// How ids is read depends on who wrote it.  Stream-ordered launches (DOOR = false): the list was complete before this kernel
+// began and stays read-only for its lifetime, which is what the non-coherent path (ld.global.nc, __ldg) is defined for.
+// DOOR = true: the select that WRITES ids runs concurrently with this kernel, so ids is not read-only over the kernel's
+// lifetime; ld.global.nc would be undefined there (the compiler may treat such a load as invariant and move it above the
+// door's acquire, and the acquire does not make non-coherent lines coherent).  That instantiation reads ids with ld.global.cg
+// (__ldcg: coherent at L2, where the select's st + fence + atomic published it), ordered after door_wait by its "memory" clobber
+// and the warp / CTA barrier.  ids carries no __restrict__ for the same reason.
+template <bool DOOR>
+__device__ __forceinline__ int32_t load_id(const int32_t* p) {
+    if (DOOR) return __ldcg(p);
+    return __ldg(p);
+}
+
+template <bool DOOR>
+__global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__ host_kv, const int32_t* ids,
                                                         char* __restrict__ pool, int n_rows, int n_blocks, int topk,
                                                         uint32_t block_bytes, unsigned int* door) {
     extern __shared__ __align__(128) char ring[];
@@ -60,7 +75,7 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
     __syncwarp();
     pdl_wait();                  // ids (and the pool's previous reader) belong to earlier kernels
     pdl_launch_dependents();
-    if (door) {
+    if (DOOR) {
         if (lane == 0) door_wait(door, (unsigned)n_rows);
         __syncwarp();
     }
@@ -83,7 +98,7 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
 #pragma unroll
     for (int j = 0; j < GATHER_WIN / 32; ++j) {
         const int64_t t = (int64_t)j * 32 + lane;
-        vn[j] = t < n_tasks ? __ldg(ids + t) : -1;
+        vn[j] = t < n_tasks ? load_id<DOOR>(ids + t) : -1;
     }
     for (int64_t base = 0; base < n_tasks; base += GATHER_WIN) {
         // ---- compact this window's valid tasks; keep the share [lo, hi) of this CTA
@@ -92,7 +107,7 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
         for (int j = 0; j < GATHER_WIN / 32; ++j) {
             v[j] = vn[j];
             const int64_t t = base + GATHER_WIN + j * 32 + lane;
-            vn[j] = t < n_tasks ? __ldg(ids + t) : -1;
+            vn[j] = t < n_tasks ? load_id<DOOR>(ids + t) : -1;
             nv += __popc(__ballot_sync(0xffffffffu, v[j] >= 0));
         }
         const int lo = (int)((int64_t)nv * blockIdx.x / gridDim.x), hi = (int)((int64_t)nv * (blockIdx.x + 1) / gridDim.x);
@@ -135,13 +150,14 @@ __global__ void __launch_bounds__(32) gather_tma_kernel(const char* __restrict__
 constexpr int LDG_UNROLL = 8;                       // 8 x 16 B in flight per lane
 constexpr int LDG_UNIT_BYTES = LDG_UNROLL * 32 * 16;  // 4 KiB per warp-iteration
 
-__global__ void __launch_bounds__(256) gather_ldg_kernel(const char* __restrict__ host_kv, const int32_t* __restrict__ ids,
+template <bool DOOR>
+__global__ void __launch_bounds__(256) gather_ldg_kernel(const char* __restrict__ host_kv, const int32_t* ids,
                                                          char* __restrict__ pool, int n_rows, int n_blocks, int topk,
                                                          uint32_t block_bytes, unsigned int* door) {
     const int lane = threadIdx.x & 31;
     pdl_wait();
     pdl_launch_dependents();
-    if (door) {
+    if (DOOR) {
         if (threadIdx.x == 0) door_wait(door, (unsigned)n_rows);
         __syncthreads();
     }
@@ -152,7 +168,7 @@ __global__ void __launch_bounds__(256) gather_ldg_kernel(const char* __restrict_
     for (int64_t u = warp; u < n_units; u += n_warps) {
         int64_t task = u / units_per_block;
         uint32_t c = (uint32_t)(u % units_per_block);
-        int32_t id = __ldg(ids + task);
+        int32_t id = load_id<DOOR>(ids + task);
         if (id < 0) continue;
         int64_t r = task / topk;
         const char* src = host_kv + ((r * n_blocks + id) * (int64_t)block_bytes + (int64_t)c * LDG_UNIT_BYTES) + lane * 16;
@@ -176,7 +192,8 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
         const int smem = GATHER_STAGES * GATHER_STAGE_BYTES;
         sparda_kernel_state& ks = ctx->kstate[SPARDA_K_GATHER_TMA];
         if (!ks.attr_set) {
-            SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(gather_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(gather_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(gather_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
             ks.attr_set = true;
         }
         cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
@@ -187,7 +204,8 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
         lc.stream = st;
         lc.attrs = at;
         lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
-        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_tma_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes, door));
+        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, door ? gather_tma_kernel<true> : gather_tma_kernel<false>, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks,
+                                                topk, block_bytes, door));
     } else {
         cudaLaunchAttribute at[1] = {sparda_pdl_attr()};
         cudaLaunchConfig_t lc = {};
@@ -196,7 +214,8 @@ int sparda_launch_gather(sparda_ctx* ctx, const void* host_kv, int n_blocks, con
         lc.stream = st;
         lc.attrs = at;
         lc.numAttrs = sparda_use_pdl(ctx) ? 1 : 0;
-        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, gather_ldg_kernel, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks, topk, block_bytes, door));
+        SPARDA_CUDA_TRY(ctx, cudaLaunchKernelEx(&lc, door ? gather_ldg_kernel<true> : gather_ldg_kernel<false>, (const char*)host_kv, ids, (char*)pool, ctx->R, n_blocks,
+                                                topk, block_bytes, door));
     }
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->launches++;

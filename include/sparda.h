@@ -234,7 +234,10 @@ const char* sparda_noalloc_last_error(void);
  * In overlap mode a layer's gather is launched together with its select and waits on the device for the select's
  * doorbell (one counter per layer in the context's workspace, zeroed at the top of the step), so no kernel boundary
  * sits between "block list out" and "first byte on the link"; a gather whose select never runs traps after ~15 s
- * instead of hanging the device.  One step per context at a time.  The select runs on a highest-priority stream of the
+ * instead of hanging the device.  The doorbell is used only while the gather grid cannot fill the device (cfg.gather_ctas <=
+ * SM count / 2 = 74 on B200: the select can then always become resident beside the waiting CTAs, also in a graph replay where
+ * nothing orders the two launches); a larger gather grid is launched behind the select's event instead (same results, one kernel
+ * boundary more on the chain).  One step per context at a time.  The select runs on a highest-priority stream of the
  * context; create prefetch_stream with the highest priority too (cudaStreamCreateWithPriority): beside a many-CTA kernel on
  * the compute stream the block scheduler serves the older kernel's pending CTAs first, and at equal priority a side-stream
  * kernel launched after it waits for most of it (measured: select 42 us instead of 20 beside a 4736-CTA HBM stream).
@@ -254,7 +257,12 @@ int sparda_set_step_candidates(sparda_ctx* ctx, int n_cand);
  * every selection of sparda_decode_step / _host / _cached is sparda_forecast_select_grid -- layers[l].Kpool then points to the
  * (32,16) compressed-key grid [R][4 n_blocks][D] of sparda_pool_keys_grid, and ids are init + local + top-k (Eq.1, P:L53;
  * reading q19: parity unpinned by the paper).  n_init + n_local <= topk.  grid = 0 restores the one-key-per-block form.
- * The cached step then runs the reuse plan as its own launch behind the select (no doorbell for that layer's gather).  */
+ * The cached step then runs the reuse plan as its own launch behind the select (no doorbell for that layer's gather).
+ * With a growing cache (sparda_set_step_candidates): sparda_append_kv maintains only the one-key-per-block Kpool, NOT the grid.
+ * The four grid keys of a block exist only after sparda_pool_keys_grid has run over it, so a caller that combines grid = 1 with a
+ * growing n_cand must re-run sparda_pool_keys_grid over every newly completed block (and, because the (32,16) windows straddle
+ * block boundaries, over the block before it) before the step that first ranks it; otherwise that block is ranked on stale or
+ * zero keys.  Nothing in the library detects this.                                                                          */
 int sparda_set_step_selector(sparda_ctx* ctx, int grid, int n_init, int n_local);
 
 /* The same step for a caller whose per-step tensors live in HOST memory (the end-to-end form bench.py times):

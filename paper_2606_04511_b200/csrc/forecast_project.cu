@@ -143,8 +143,8 @@ __global__ void __launch_bounds__(FP_THREADS, 1) forecast_project_kernel(FpParam
 
 }  // namespace
 
-int sparda_launch_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F, int ws, cudaStream_t st) {
-    (void)ws;   // the split-K partials live in the cluster's shared memory: no workspace, any number of launches in flight
+// (the split-K partials live in the cluster's shared memory: no workspace, any number of launches in flight)
+int sparda_launch_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F, cudaStream_t st) {
     FpParams p;
     p.X = (const uint16_t*)X;
     p.W = (const uint16_t*)WF;

@@ -173,7 +173,7 @@ int sparda_pool_keys(sparda_ctx* ctx, const void* kv, int64_t n_rows, int n_bloc
 int sparda_forecast_project(sparda_ctx* ctx, const void* X, const void* WF, int hidden, void* F_out, void* stream) {
     if (!ctx || !sparda_aligned(X, 16) || !sparda_aligned(WF, 16) || !sparda_aligned(F_out, 16)) return SPARDA_EINVAL;
     if (hidden < 64 || hidden > 8192 || hidden % 64 != 0) return SPARDA_EINVAL;
-    return sparda_launch_forecast_project(ctx, X, WF, hidden, F_out, 0, (cudaStream_t)stream);
+    return sparda_launch_forecast_project(ctx, X, WF, hidden, F_out, (cudaStream_t)stream);
 }
 
 int sparda_append_kv(sparda_ctx* ctx, const void* k_new, const void* v_new, int64_t t, void* kv_cache, int n_blocks, float* ksum,
@@ -318,7 +318,7 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
     // layer 0: same-layer selection with F0cur; its attention needs it, so it stays on the compute stream
     if (!io && layers[0].base.X && layers[0].base.WFcur) {   // Alg.2 l.1 for F_0^cur (Eq.3)
         if (!ctx->cfg.hidden) return SPARDA_EINVAL;
-        rc = sparda_launch_forecast_project(ctx, layers[0].base.X, layers[0].base.WFcur, ctx->cfg.hidden, const_cast<void*>(F0cur), 0, cs);
+        rc = sparda_launch_forecast_project(ctx, layers[0].base.X, layers[0].base.WFcur, ctx->cfg.hidden, const_cast<void*>(F0cur), cs);
         if (rc) return rc;
     }
     SPARDA_PROF_BEGIN(0, cs);
@@ -331,6 +331,13 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
               : sparda_forecast_select(ctx, F0cur, layers[0].base.Kpool, n_blocks, n_cand, topk, layers[0].base.ids, cs);
     if (rc) return rc;
     SPARDA_PROF_END(0, cs);
+    // Doorbell admission.  A waiting gather CTA holds its SM slot (TMA engine: ~104 KB of shared memory, two fit per SM; LDG
+    // engine: 256 threads, eight fit) until the select has rung, and nothing orders "select resident before gather" on the
+    // device -- least of all in a CUDA-graph replay, where the two are independent nodes.  With at most sm_count / 2 gather CTAs
+    // at least half of the SMs hold no gather CTA whatever the placement, so the select's clusters (and the attention) can
+    // always be scheduled and the wait ends.  Beyond that (cfg.gather_ctas up to 1024 is accepted, the peer tier asks for more
+    // CTAs) a grid of spinning CTAs could occupy every SM and the step would trap after ~15 s: such a grid is not given a door.
+    const bool door_fits = 2 * ctx->cfg.gather_ctas <= ctx->sm_count;
     struct PdlScope {   // launches behind an event wait do not ask for PDL (see sparda_ctx::pdl_next); restored on every return
         sparda_ctx* c;
         ~PdlScope() { c->pdl_next = 1; }
@@ -351,14 +358,15 @@ static int decode_step_impl(sparda_ctx* ctx, const sparda_cached_layer* layers, 
             ctx->pdl_next = overlap ? 0 : 1;   // overlap mode launches without PDL (measured: 0.38 ms per cached step against 0.43)
             if (!io && layers[l].base.X && layers[l].base.WF) {   // Alg.2 l.1: F_l = X_l . W_F (Eq.3), where its reader runs
                 if (!ctx->cfg.hidden) return SPARDA_EINVAL;
-                rc = sparda_launch_forecast_project(ctx, layers[l].base.X, layers[l].base.WF, ctx->cfg.hidden, const_cast<void*>(layers[l].base.F),
-                                                    (l + 1) & 1, xs);
+                rc = sparda_launch_forecast_project(ctx, layers[l].base.X, layers[l].base.WF, ctx->cfg.hidden, const_cast<void*>(layers[l].base.F), xs);
                 if (rc) return rc;
                 ctx->pdl_next = 1;   // the select follows the projection on its own stream, no event in between: its prologue
                                      // and the first ring of pooled keys overlap the projection (0.58 -> 0.55 ms per cached step, batch 4)
             }
-            // the doorbell needs the list the gather reads to come out of the ringing kernel: not so for grid select + separate plan
-            const bool use_door = overlap && !(grid && nx->slot_ids);
+            // the doorbell needs the list the gather reads to come out of the ringing kernel: not so for grid select + separate plan.
+            // It also needs the select to become resident while the gather CTAs spin: guaranteed only when the gather grid cannot
+            // fill the device (door_fits below); a larger grid is ordered behind the select by ev_sel, like grid + plan
+            const bool use_door = overlap && door_fits && !(grid && nx->slot_ids);
             ctx->door_next = use_door ? ctx->door + (l + 1) : nullptr;   // this select rings the layer's gather (below) row by row
             SPARDA_PROF_BEGIN(0, xs);
             if (grid) {

@@ -113,7 +113,7 @@ int sparda_launch_select(sparda_ctx*, const void* F, const void* Kpool, int n_bl
                          cudaStream_t);
 int sparda_launch_gather(sparda_ctx*, const void* host_kv, int n_blocks, const int32_t* ids, int topk, void* pool,
                          cudaStream_t);
-int sparda_launch_forecast_project(sparda_ctx*, const void* X, const void* WF, int hidden, void* F, int workspace /* 0 or 1 */, cudaStream_t);
+int sparda_launch_forecast_project(sparda_ctx*, const void* X, const void* WF, int hidden, void* F, cudaStream_t);
 int sparda_launch_pool_keys_grid(sparda_ctx*, const void* kv, int64_t n_rows, int n_blocks, void* kgrid, cudaStream_t);
 int sparda_launch_select_grid(sparda_ctx*, const void* F, const void* Kgrid, int n_blocks, int n_cand, int n_init, int n_local, int topk,
                               int32_t* ids, cudaStream_t);

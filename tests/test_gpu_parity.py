@@ -290,6 +290,46 @@ def test_decode_step_ldg_engine_through_the_doorbell(sp):
             assert torch.equal(a.view(torch.int16), b.view(torch.int16)), f"{key}: pool bytes differ"
 
 
+@pytest.mark.parametrize("mode_name,ctas", [("tma", 400), ("ldg", 1024), ("tma", 74), ("tma", 75)])
+def test_decode_step_with_a_gather_grid_that_could_fill_the_device(mode_name, ctas, sp):
+    """cfg.gather_ctas up to 1024 is accepted (the peer tier asks for more CTAs).  A grid of more than SM count / 2 CTAs must not be
+    given the select -> gather doorbell: 400 waiting TMA CTAs (two per SM) would hold every SM, the select could never become
+    resident and the step would trap after ~15 s.  Such a grid is ordered behind the select's event; 74 CTAs (the largest grid
+    that still gets the door on 148 SMs) and 75 (the first that does not) sit on either side of the rule.  Overlapped must stay
+    bit-identical to serial, steps repeated."""
+    cfg = G16.with_(n_layers=4, batch=3)
+    data = _pipeline_inputs(cfg, sp)
+    R, k, Nb, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim
+    ctx = sp.Sparda.from_config(cfg, max_layers=4, gather_mode=sp.GATHER_LDG if mode_name == "ldg" else sp.GATHER_TMA, gather_ctas=ctas)
+    assert ctx.gather_ctas == ctas
+    dev = []
+    for l, (L, kv_host) in enumerate(data):
+        kpool = torch.empty((R, Nb, D), dtype=torch.bfloat16, device="cuda")
+        ctx.pool_keys(L["kv"], R, Nb, kpool)
+        dev.append({"F": L["F"], "Q": L["Q"], "Kpool": kpool, "kv": L["kv"] if l == 0 else kv_host,
+                    "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                    "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda")})
+    arr = ctx.make_layers(dev)
+    cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
+    outs = {}
+    for mode in (sp.STEP_SERIAL, sp.STEP_OVERLAP):
+        pools = [torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+        for d in dev:
+            d["O"].zero_()
+            d["ids"].fill_(-9)
+        torch.cuda.synchronize()
+        for _ in range(3):
+            ctx.decode_step(arr, data[0][0]["F0cur"], Nb, k, pools[0], pools[1], cs, ps, mode)
+        torch.cuda.synchronize()
+        outs[mode] = ([d["O"].clone() for d in dev], [d["ids"].clone() for d in dev], [p.clone() for p in pools])
+    ctx.close()
+    for a, b in zip(outs[sp.STEP_SERIAL][0] + outs[sp.STEP_SERIAL][2], outs[sp.STEP_OVERLAP][0] + outs[sp.STEP_OVERLAP][2]):
+        assert torch.equal(a.view(torch.int16), b.view(torch.int16)), "overlapped != serialized"
+    for a, b in zip(outs[sp.STEP_SERIAL][1], outs[sp.STEP_OVERLAP][1]):
+        assert torch.equal(a, b)
+    assert not any(torch.isnan(o).any() for o in outs[sp.STEP_OVERLAP][0])
+
+
 def test_multi_step_decode_with_growing_cache(sp, oracle):
     """A true multi-step decode (Alg.2 l.2-7 over consecutive tokens): every step appends the new token's K / V to every layer's
     cache (layer 0 on the device, the others in pinned host memory through UVA), the pooled keys grow block by block, and the
@@ -358,6 +398,72 @@ def test_multi_step_decode_with_growing_cache(sp, oracle):
     assert checked == 5
     ctx.set_step_candidates(0)
     ctx.close()
+
+
+@pytest.mark.parametrize("mode_name", ["serial", "overlap"])
+def test_append_then_step_on_one_stream_without_host_sync(mode_name, sp):
+    """The README loop: sparda_append_kv for every layer, then the decode step, on ONE stream with no host synchronisation in
+    between -- across the token that completes a block (t % 64 == 63: its pooled key is written by the append right in front of
+    the select that must rank it).  The step's first select is launched with programmatic dependent launch and streams pooled
+    keys before its griddepcontrol.wait; append_kv never signals early, so the select may only start once the append has
+    completed and its writes are visible.  Every step of the unsynchronised run must be bit-identical to the same loop with a
+    device synchronisation between the appends and the step (and between steps)."""
+    cfg = synth.DecodeConfig("grow_nosync", batch=2, n_q_heads=8, n_kv_heads=2, head_dim=128, n_blocks=8, topk=4, n_layers=3, seed=62)
+    R, k, Nb, D, NL, S = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers, 64
+    mode = sp.STEP_SERIAL if mode_name == "serial" else sp.STEP_OVERLAP
+    t0, t1 = 5 * S + 50, 6 * S + 6                                   # block 5 completes at t = 383
+    g = torch.Generator(device="cuda").manual_seed(62)
+    kn = (torch.randn((t1, NL, R, D), generator=g, device="cuda") + 1.5 * torch.randn((t1, NL, R, 1), generator=g, device="cuda")).to(torch.bfloat16)
+    vn = torch.randn((t1, NL, R, D), generator=g, device="cuda").to(torch.bfloat16)
+    Fs = torch.randn((t1 - t0, NL + 1, R, D), generator=g, device="cuda").to(torch.bfloat16)      # slot NL = F0cur
+    Qs = torch.randn((t1 - t0, NL, cfg.batch, cfg.n_q_heads, D), generator=g, device="cuda").to(torch.bfloat16)
+    torch.cuda.synchronize()
+    runs = {}
+    for sync in (True, False):
+        ctx = sp.Sparda.from_config(cfg, max_layers=NL)
+        kv = [torch.zeros((R, Nb, 2, S, D), dtype=torch.bfloat16, device="cuda") if l == 0 else
+              torch.zeros((R, Nb, 2, S, D), dtype=torch.bfloat16).pin_memory() for l in range(NL)]
+        kpool = [torch.zeros((R, Nb, D), dtype=torch.bfloat16, device="cuda") for _ in range(NL)]
+        ksum = [torch.zeros((R, D), dtype=torch.float32, device="cuda") for _ in range(NL)]
+        dev = [{"F": torch.zeros((R, D), dtype=torch.bfloat16, device="cuda"), "Q": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                "Kpool": kpool[l], "kv": kv[l], "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda")} for l in range(NL)]
+        F0 = torch.zeros((R, D), dtype=torch.bfloat16, device="cuda")
+        arr = ctx.make_layers(dev)
+        pools = [torch.full((R, k, 2, S, D), float("nan"), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+        cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
+        torch.cuda.synchronize()
+        out = []
+        with torch.cuda.stream(cs):
+            for t in range(t1):
+                for l in range(NL):
+                    ctx.append_kv(kn[t, l], vn[t, l], t, kv[l], Nb, ksum[l], kpool[l], stream=cs)
+                if t < t0:
+                    continue
+                for l in range(NL):
+                    dev[l]["F"].copy_(Fs[t - t0, l])
+                    dev[l]["Q"].copy_(Qs[t - t0, l])
+                F0.copy_(Fs[t - t0, NL])
+                ctx.set_step_candidates((t + 1) // S)
+                if sync:
+                    torch.cuda.synchronize()
+                ctx.decode_step(arr, F0, Nb, k, pools[0], pools[1], cs, ps, mode)
+                out.append(([d["O"].clone() for d in dev], [d["ids"].clone() for d in dev]))
+                if sync:
+                    torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        runs[sync] = out
+        ctx.close()
+    assert len(runs[True]) == t1 - t0
+    for i, ((Oa, Ia), (Ob, Ib)) in enumerate(zip(runs[True], runs[False])):
+        t = t0 + i
+        for l in range(NL):
+            assert torch.equal(Ia[l], Ib[l]), f"t {t} layer {l}: ids differ without the host synchronisation"
+            assert torch.equal(Oa[l].view(torch.int16), Ob[l].view(torch.int16)), f"t {t} layer {l}: O differs without the host synchronisation"
+    # never a block beyond the complete ones; the completed block is ranked from the step that follows its last append
+    for i, (_, I) in enumerate(runs[False]):
+        assert max(int(x.max()) for x in I) < (t0 + i + 1) // S
+    assert any(int(x.max()) == 5 for _, I in runs[False][6 * S - 1 - t0:] for x in I), "block 5 never selected after it completed"
 
 
 def test_decode_step_with_the_grid_selector(sp, oracle):

@@ -192,6 +192,20 @@ int sparda_enable_peer_tier(sparda_ctx* ctx, int peer_device);
 int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, int topk,
                          int pool_is_indexed, int n_slots, void* O, void* stream);
 
+/* (a5/a6 + f2) The same attention over caches whose newest block is partly filled (reading q7).  Alg.2 l.2 appends the
+ * new token's K / V before the attention and Eq.1 always attends the local window that holds it, so a row's cache
+ * holds seq_len[r] tokens and its last block min(S, seq_len[r] - S*j) of them.  seq_len: device [R] int32.  For every listed
+ * block id j >= 0 of row r only its first min(S, seq_len[r] - S*j) tokens are attended; a block with none (S*j >= seq_len[r])
+ * counts like id -1.  Whatever bytes lie behind the last token of the open block are ignored (NaN included: their scores are
+ * replaced, their V rows zeroed in shared memory), so the cache need not be cleared.  ids holds BLOCK ids in both pool forms
+ * (with pool_is_indexed = 0, slot i of dev_pool holds block ids[r][i] as for sparda_sparse_decode).  The caller lists the open
+ * block itself: the selectors rank complete blocks only (sparda_set_step_candidates), so append its id (the highest: the
+ * list stays ascending) to the selection, gather it like any other block (sparda_append_kv has written it to the host cache), or
+ * attend a device-resident cache by id.  Every other rule, and the one-launch-per-context limit, as for sparda_sparse_decode.
+ * The decode steps do not pass seq_len yet: they attend complete blocks only.                                                */
+int sparda_sparse_decode_varlen(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, const int32_t* seq_len,
+                                int topk, int pool_is_indexed, int n_slots, void* O, void* stream);
+
 /* (a5/a6) The same attention for callers that must not allocate device memory, and so cannot use sparda_create at all
  * (it calls cudaMalloc for the split-K workspace, creates a stream and events).  Who that is:
  *   - a serving engine that hands the whole of HBM to its own pool at start-up: a later cudaMalloc from a library fails,

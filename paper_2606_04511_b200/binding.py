@@ -19,7 +19,7 @@ STEP_OVERLAP, STEP_SERIAL = 0, 1
 
 EXPORTS = [
     "sparda_create", "sparda_destroy", "sparda_pool_keys", "sparda_forecast_project", "sparda_append_kv", "sparda_pool_keys_grid", "sparda_forecast_select_grid", "sparda_forecast_select", "sparda_prefetch_launch",
-    "sparda_sparse_decode", "sparda_sparse_decode_noalloc", "sparda_noalloc_last_error", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
+    "sparda_sparse_decode", "sparda_sparse_decode_varlen", "sparda_sparse_decode_noalloc", "sparda_noalloc_last_error", "sparda_decode_step", "sparda_decode_step_host", "sparda_profile_enable",
     "sparda_reuse_plan", "sparda_forecast_select_plan", "sparda_decode_step_cached",
     "sparda_profile_read", "sparda_prefill_select", "sparda_prefill_select_baseline",
     "sparda_probe_launch", "sparda_set_layer_standin", "sparda_enable_peer_tier", "sparda_set_step_candidates", "sparda_set_step_selector",
@@ -71,6 +71,7 @@ def lib() -> ctypes.CDLL:
         L.sparda_forecast_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_prefetch_launch.argtypes = [vp, vp, i32, vp, i32, vp, vp]
         L.sparda_sparse_decode.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
+        L.sparda_sparse_decode_varlen.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_sparse_decode_noalloc.argtypes = [i32, i32, i32, i32, vp, vp, vp, i32, i32, i32, vp, vp]
         L.sparda_noalloc_last_error.argtypes = []
         L.sparda_decode_step.argtypes = [vp, ctypes.POINTER(SpardaLayer), i32, vp, i32, i32, vp, vp, vp, vp, i32]
@@ -200,6 +201,12 @@ class Sparda:
         self._check(self._L.sparda_sparse_decode(self._h, _ptr(Q), _ptr(dev_pool), _ptr(ids), topk,
                                                  1 if pool_is_indexed else 0, n_slots, _ptr(O), _stream(stream)),
                     "sparse_decode")
+
+    def sparse_decode_varlen(self, Q, dev_pool, ids, seq_len, topk, O, pool_is_indexed=False, n_slots=None, stream=None):
+        n_slots = topk if n_slots is None else n_slots
+        self._check(self._L.sparda_sparse_decode_varlen(self._h, _ptr(Q), _ptr(dev_pool), _ptr(ids), _ptr(seq_len), topk,
+                                                        1 if pool_is_indexed else 0, n_slots, _ptr(O), _stream(stream)),
+                    "sparse_decode_varlen")
 
     def make_layers(self, layers):
         """layers: list of dicts with tensors F, Q, Kpool, kv, O, ids -> ctypes array (keeps no references)."""

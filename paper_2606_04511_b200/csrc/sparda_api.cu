@@ -245,7 +245,17 @@ int sparda_sparse_decode(sparda_ctx* ctx, const void* Q, const void* dev_pool, c
         return SPARDA_EINVAL;
     if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
     if (pool_is_indexed ? (n_slots < 1 || n_slots > ctx->cfg.max_blocks) : (n_slots != topk)) return SPARDA_EINVAL;
-    return sparda_launch_attn(ctx, Q, dev_pool, ids, topk, pool_is_indexed ? 1 : 0, n_slots, O, (cudaStream_t)stream);
+    return sparda_launch_attn(ctx, Q, dev_pool, ids, nullptr, topk, pool_is_indexed ? 1 : 0, n_slots, O, (cudaStream_t)stream);
+}
+
+int sparda_sparse_decode_varlen(sparda_ctx* ctx, const void* Q, const void* dev_pool, const int32_t* ids, const int32_t* seq_len, int topk,
+                                int pool_is_indexed, int n_slots, void* O, void* stream) {
+    if (!ctx || !sparda_aligned(Q, 16) || !sparda_aligned(dev_pool, 16) || !sparda_aligned(ids, 4) || !sparda_aligned(O, 16) ||
+        !sparda_aligned(seq_len, 4))
+        return SPARDA_EINVAL;
+    if (topk < 1 || topk > ctx->cfg.topk) return SPARDA_EINVAL;
+    if (pool_is_indexed ? (n_slots < 1 || n_slots > ctx->cfg.max_blocks) : (n_slots != topk)) return SPARDA_EINVAL;
+    return sparda_launch_attn(ctx, Q, dev_pool, ids, seq_len, topk, pool_is_indexed ? 1 : 0, n_slots, O, (cudaStream_t)stream);
 }
 
 int sparda_prefill_select(sparda_ctx* ctx, const void* F, const void* Kpool, int T, int n_blocks, int row0, int n_rows,

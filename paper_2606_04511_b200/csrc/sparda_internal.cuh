@@ -22,6 +22,7 @@ struct sparda_kernel_state {
 enum {
     SPARDA_K_SELECT_128, SPARDA_K_SELECT_64, SPARDA_K_SELECT_GRID_128, SPARDA_K_SELECT_GRID_64,
     SPARDA_K_ATTN_128, SPARDA_K_ATTN_64, SPARDA_K_ATTN_CL_128, SPARDA_K_ATTN_CL_64,
+    SPARDA_K_ATTN_VL_128, SPARDA_K_ATTN_VL_64, SPARDA_K_ATTN_VL_CL_128, SPARDA_K_ATTN_VL_CL_64,   /* sparda_sparse_decode_varlen */
     SPARDA_K_GATHER_TMA, SPARDA_K_PROBE, SPARDA_K_STANDIN, SPARDA_K_PROJECT, SPARDA_K_ATTN_T5, SPARDA_K_ATTN_T5_CL,
     SPARDA_K_PF_0, /* 8 prefill instantiations: D x BASELINE x REPL */
     SPARDA_K_COUNT = SPARDA_K_PF_0 + 8
@@ -121,8 +122,8 @@ int sparda_launch_append_kv(sparda_ctx*, const void* k_new, const void* v_new, i
                             void* kpool, cudaStream_t);
 int sparda_launch_reuse_plan(sparda_ctx*, const int32_t* ids_new, int topk, int32_t* slot_ids, int32_t* fetch, int32_t* n_fetch,
                              cudaStream_t);
-int sparda_launch_attn(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
-                       int n_slots, void* O, cudaStream_t);
+int sparda_launch_attn(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, const int32_t* seq_len /* or nullptr */, int topk,
+                       int indexed, int n_slots, void* O, cudaStream_t);
 // the tcgen05 experiment (cfg.attn_impl = 1): SPARDA_OK, 1 = shape outside its range (fall back to the mma.sync kernel), or an error
 int sparda_launch_attn_tc5(sparda_ctx*, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
                            int n_slots, void* O, cudaStream_t);

@@ -50,6 +50,7 @@ struct AttnSmem {
 struct AttnParams {
     const uint32_t* Q;     // bf16 pairs
     const int32_t* ids;
+    const int32_t* seq_len; // [R] tokens in the row's cache, or nullptr = every listed block is complete (sparda_sparse_decode_varlen)
     __nv_bfloat16* O;
     float* part_O;         // [R][max_splits][16][D]
     float* part_ml;        // [R][max_splits][2][16]
@@ -70,7 +71,9 @@ __device__ __forceinline__ int flat_owner(int f, int quota, int rem) {
 // through distributed shared memory instead of the L2 workspace -- every CTA sends each head row's partial (m, l, O) to the
 // CTA that owns that head row (16 / s rows each), one cluster barrier, every CTA normalises and stores its rows.  No ticket,
 // no fence, no global round trip, and the final merge is spread over the cluster.
-template <int D, int NW, int MINB, bool CL>
+// VARLEN (sparda_sparse_decode_varlen): p.seq_len[r] tokens exist in row r's cache; the partly filled newest block is masked.  Its own
+// instantiation: the D = 128 kernel sits at the 255-register limit and the extra live values must not cost the default path.
+template <int D, int NW, int MINB, bool CL, bool VARLEN>
 __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __grid_constant__ CUtensorMap tmap, AttnParams p) {
     using SM = AttnSmem<D, NW>;
     constexpr int NT = NW * 32;
@@ -296,6 +299,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
         const int part = blockIdx.x - first_cta;
         const int b = r / p.Hkv, g = r % p.Hkv;
         const int32_t* ids_row = p.ids + (size_t)r * p.topk;
+        // tokens in row r's cache (varlen form): block j holds min(64, seq_row - 64 j) of them; INT_MAX = every block complete
+        const int seq_row = VARLEN ? __ldg(p.seq_len + r) : 0x7fffffff;
 
         // Q fragments (A operand, 16 heads x D): rows gid and gid+8, zero beyond G
         uint32_t qa[KSTEPS][4];
@@ -325,7 +330,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
             int nxt_r = r, nxt_s = cur_s + NW;
             bool have_n = true;
             if (nxt_s >= sg.s1) have_n = first_item(f, nxt_r, nxt_s);
-            const bool valid = __ldg(ids_row + cur_s) >= 0;
+            const int32_t id_cur = __ldg(ids_row + cur_s);
+            const int n_tok = VARLEN ? min(S_BLK, seq_row - id_cur * S_BLK) : S_BLK;   // tokens of this block that exist (id <= 8191: no overflow)
+            const bool valid = id_cur >= 0 && n_tok > 0;
             // ---- S = Q K^T
             mbar_wait(&bar_k[w], phase);
             if (first__) { TRACE(2); first__ = false; }
@@ -343,6 +350,16 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
                         mma_bf16_16816(s[nt], qa[2 * kp], b0, b1);
                         mma_bf16_16816(s[nt], qa[2 * kp + 1], b2, b3);
                     }
+                }
+            }
+            if (VARLEN && valid && n_tok < S_BLK) {
+                // the partly filled newest block: tokens >= n_tok do not exist.  Their scores are REPLACED (whatever bytes sit there,
+                // NaN included) so that they get weight exp2(-inf) = 0.  Columns of s[nt][.]: tokens nt*8 + tig*2 + {0, 1}
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) {
+                    const int c0 = nt * 8 + tig * 2;
+                    if (c0 >= n_tok) s[nt][0] = s[nt][2] = -INFINITY;
+                    if (c0 + 1 >= n_tok) s[nt][1] = s[nt][3] = -INFINITY;
                 }
             }
             __syncwarp();
@@ -382,6 +399,17 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
 
             // ---- O += P V
             mbar_wait(&bar_v[w], phase);
+            if (VARLEN && valid && n_tok < S_BLK) {
+                // weight 0 times a NaN / Inf left behind the tail would still poison O: zero the V rows that do not exist in the
+                // warp's stage (a row is 128 contiguous bytes per 64-column box whatever the swizzle); generic-proxy stores, ordered
+                // before the next TMA write into the stage by the fence in front of issue_v
+                const int n_chunks = (S_BLK - n_tok) * HALVES * 8;   // 16-byte chunks
+                for (int c = lane; c < n_chunks; c += 32) {
+                    const int row = n_tok + c / (HALVES * 8), h = (c / 8) % HALVES, q16 = c % 8;
+                    *reinterpret_cast<int4*>(stage + SM::TILE_BYTES + h * 8192 + row * 128 + q16 * 16) = make_int4(0, 0, 0, 0);
+                }
+                __syncwarp();
+            }
             if (valid) {
 #pragma unroll
                 for (int kt = 0; kt < 4; ++kt) {
@@ -510,11 +538,12 @@ __global__ void __launch_bounds__(NW * 32, MINB) sparse_decode_kernel(const __gr
 // Launch shape: 4 consumer warps (= 4 x 32 KiB K/V stages at D = 128), one CTA per SM (128 KiB of tiles in flight per SM).
 constexpr int ATT_NW = 4;
 
-template <int D, bool CL>
+template <int D, bool CL, bool VL = false>
 int launch(sparda_ctx* ctx, const CUtensorMap* map, const AttnParams& p, int C, int cluster, cudaStream_t st) {
-    auto kern = sparse_decode_kernel<D, ATT_NW, 1, CL>;
+    auto kern = sparse_decode_kernel<D, ATT_NW, 1, CL, VL>;
     constexpr int smem = AttnSmem<D, ATT_NW>::TOTAL;
-    sparda_kernel_state& ks = ctx->kstate[(CL ? SPARDA_K_ATTN_CL_128 : SPARDA_K_ATTN_128) + (D == 128 ? 0 : 1)];
+    sparda_kernel_state& ks = ctx->kstate[(VL ? (CL ? SPARDA_K_ATTN_VL_CL_128 : SPARDA_K_ATTN_VL_128) : (CL ? SPARDA_K_ATTN_CL_128 : SPARDA_K_ATTN_128)) +
+                                          (D == 128 ? 0 : 1)];
     if (!ks.attr_set) {
         SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         if (CL) SPARDA_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));   // clusters of 16
@@ -585,9 +614,9 @@ int sparda_resolve_splits(const sparda_ctx* ctx, int topk) {
     return (sparda_resolve_attn_ctas(ctx, topk) + ctx->R - 1) / ctx->R;
 }
 
-int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const int32_t* ids, int topk, int indexed,
+int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const int32_t* ids, const int32_t* seq_len, int topk, int indexed,
                        int n_slots, void* O, cudaStream_t st) {
-    if (ctx->cfg.attn_impl == 1) {   // the tcgen05 (swap-AB) experiment; shapes outside its range fall through
+    if (ctx->cfg.attn_impl == 1 && !seq_len) {   // the tcgen05 (swap-AB) experiment; shapes outside its range (and the varlen form) fall through
         const int rc5 = sparda_launch_attn_tc5(ctx, Q, pool, ids, topk, indexed, n_slots, O, st);
         if (rc5 != 1) return rc5;
     }
@@ -599,6 +628,7 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
     AttnParams p;
     p.Q = (const uint32_t*)Q;
     p.ids = ids;
+    p.seq_len = seq_len;
     p.O = (__nv_bfloat16*)O;
     p.part_O = ctx->part_O;
     p.part_ml = ctx->part_ml;
@@ -631,12 +661,14 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
             const int Cs = s * ctx->R;
             q.quota = q.W / Cs;
             q.rem = 0;
-            rc = D == 128 ? launch<128, true>(ctx, &map, q, Cs, s, st) : launch<64, true>(ctx, &map, q, Cs, s, st);
+            if (seq_len) rc = D == 128 ? launch<128, true, true>(ctx, &map, q, Cs, s, st) : launch<64, true, true>(ctx, &map, q, Cs, s, st);
+            else rc = D == 128 ? launch<128, true>(ctx, &map, q, Cs, s, st) : launch<64, true>(ctx, &map, q, Cs, s, st);
             if (rc != 1) used_cl = s;
             if (ctx->cfg.attn_splits > 0) break;
         }
     }
-    if (rc == 1) rc = D == 128 ? launch<128, false>(ctx, &map, p, C, 1, st) : launch<64, false>(ctx, &map, p, C, 1, st);
+    if (rc == 1 && seq_len) rc = D == 128 ? launch<128, false, true>(ctx, &map, p, C, 1, st) : launch<64, false, true>(ctx, &map, p, C, 1, st);
+    else if (rc == 1) rc = D == 128 ? launch<128, false>(ctx, &map, p, C, 1, st) : launch<64, false>(ctx, &map, p, C, 1, st);
     if (rc) return rc;
     SPARDA_CUDA_TRY(ctx, cudaGetLastError());
     ctx->last_attn_cluster = used_cl;
@@ -650,7 +682,7 @@ int sparda_launch_attn(sparda_ctx* ctx, const void* Q, const void* pool, const i
 // synchronisation, a plug-in with no set-up hook.  Such a caller cannot use sparda_create (cudaMalloc, stream and event
 // creation), so this entry point takes no context: the launcher state a context would hold sits in a host-side table with
 // one entry per device, and the split-K workspace (CTA partials + per-row tickets) is the fixed array below instead of
-// cudaMalloc'ed memory.  The kernel is sparse_decode_kernel<D, 4, 1, false> unchanged -- the flat split whose row
+// cudaMalloc'ed memory.  The kernel is sparse_decode_kernel<D, 4, 1, false, false> unchanged -- the flat split whose row
 // partials are merged by the last CTA to finish the row -- with its three workspace pointers aimed into the array.
 //
 // The array is part of this translation unit's device image: the driver places it on every GPU that loads the image and
@@ -715,9 +747,9 @@ int noalloc_setup(NoallocDevice& d, int dev) {
     e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch);   // the array's address ON THIS DEVICE
     if (e != cudaSuccess) return na_fail_cuda(e, "cudaGetSymbolAddress(g_noalloc_scratch)");
     if (!ptr) return na_fail(SPARDA_ECUDA, "cudaGetSymbolAddress(g_noalloc_scratch) returned a null device address");
-    e = cudaFuncSetAttribute(sparse_decode_kernel<128, ATT_NW, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128, ATT_NW>::TOTAL);
+    e = cudaFuncSetAttribute(sparse_decode_kernel<128, ATT_NW, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128, ATT_NW>::TOTAL);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(sparse_decode_kernel<64, ATT_NW, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64, ATT_NW>::TOTAL);
+        e = cudaFuncSetAttribute(sparse_decode_kernel<64, ATT_NW, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64, ATT_NW>::TOTAL);
     if (e != cudaSuccess) return na_fail_cuda(e, "cudaFuncSetAttribute(sparse_decode_kernel, MaxDynamicSharedMemorySize)");
     memset(&d.ctx, 0, sizeof(d.ctx));
     d.ctx.device = dev;
@@ -796,6 +828,7 @@ extern "C" int sparda_sparse_decode_noalloc(int batch, int n_q_heads, int n_kv_h
     AttnParams p;
     p.Q = (const uint32_t*)Q;
     p.ids = ids;
+    p.seq_len = nullptr;
     p.O = (__nv_bfloat16*)O;
     p.part_O = ctx->part_O;
     p.part_ml = ctx->part_ml;

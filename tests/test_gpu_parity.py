@@ -177,6 +177,65 @@ def test_sparse_decode(cfg, splits, sp, oracle):
     assert torch.equal(O.view(torch.int16), O3.view(torch.int16))
 
 
+@pytest.mark.parametrize("cfg,splits,want_cluster", [(MID, 0, 0), (MID64, 0, 0), (G16, 0, 16), (G16, 4, 4), (G1, 1, 0),
+                                                     (synth.DecodeConfig("vl_r32", batch=4, n_q_heads=32, n_kv_heads=8, head_dim=128, n_blocks=40, topk=16, seed=81), 0, 4)],
+                         ids=lambda v: getattr(v, "name", str(v)))
+def test_sparse_decode_varlen(cfg, splits, want_cluster, sp, oracle):
+    """sparda_sparse_decode_varlen against o16 (reading q7: the newest block of a row is partly filled and is attended, Alg.2 l.2
+    P:L300, Eq.1).  Rows of different lengths: a tail of 1, 9, 63 tokens, a row that ends on a block boundary, a row
+    of one token, a listed block wholly beyond the row's length, a padded row.  Everything behind a row's last token is NaN in
+    the cache (K and V): it must not reach O.  Both pool forms give the same bits; with every block complete the result is
+    sparda_sparse_decode's, bit for bit.  Every reduction path (workspace + ticket, clusters of 4 and 16)."""
+    L, ctx, _ = _setup(cfg, sp, attn_splits=splits)
+    R, k, Nb, S, D = cfg.rows, cfg.topk, cfg.n_blocks, cfg.block_size, cfg.head_dim
+    rng = np.random.default_rng(cfg.seed)
+    tails = [9, 0, 1, 63, 17, 40]
+    seq = np.array([rng.integers(max(Nb // 2, 1), Nb) * S + tails[r % len(tails)] for r in range(R)], dtype=np.int32)
+    seq[R - 1] = 1                                                    # one token in the whole cache
+    ids_np = np.full((R, k), -1, dtype=np.int32)
+    for r in range(R):
+        complete, tail = divmod(int(seq[r]), S)
+        chosen = sorted(rng.choice(complete, size=min(k - 1, complete), replace=False).tolist()) if complete else []
+        if tail:
+            chosen.append(complete)                                   # the open block: the highest id, so the list stays ascending
+        ids_np[r, :len(chosen)] = chosen
+    if R > 2 and k >= 3:
+        ids_np[2, k - 1] = min(int(seq[2]) // S + 2, Nb - 1)          # listed, but wholly beyond the row's tokens: contributes nothing
+        ids_np[0, k - k // 3:] = -1                                   # padded row (drops the open block of row 0 as well)
+    kv = L["kv"].clone()
+    flat = kv.view(R, Nb, 2, S, D)
+    for r in range(R):                                                # NaN behind the last token, K and V
+        j, t = divmod(int(seq[r]), S)
+        if j < Nb:
+            flat[r, j, :, t:] = float("nan")
+            flat[r, j + 1:] = float("nan")
+    ids = torch.from_numpy(ids_np).cuda()
+    seq_d = torch.from_numpy(seq).cuda()
+    O_idx = torch.full((cfg.batch, cfg.n_q_heads, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    ctx.sparse_decode_varlen(L["Q"], kv, ids, seq_d, k, O_idx, pool_is_indexed=True, n_slots=Nb)
+    torch.cuda.synchronize()
+    assert ctx.attn_cluster == want_cluster, f"reduction path {ctx.attn_cluster}, wanted {want_cluster}"
+    pool = torch.full((R, k, 2, S, D), float("nan"), dtype=torch.bfloat16, device="cuda")
+    ctx.prefetch_launch(kv, Nb, ids, k, pool)
+    O_pool = torch.full_like(O_idx, float("nan"))
+    ctx.sparse_decode_varlen(L["Q"], pool, ids, seq_d, k, O_pool)
+    torch.cuda.synchronize()
+    assert torch.equal(O_idx.view(torch.int16), O_pool.view(torch.int16)), "indexed and gathered forms differ"
+    want, _ = oracle.sparse_attn_len(_bits(L["Q"]), _bits(kv), ids_np, seq, pool_is_indexed=True)
+    parity.check_attn(_bits(O_idx), want, f"{cfg.name} varlen")
+    # every block complete: the masked kernel is the plain one
+    full = torch.full((R,), Nb * S, dtype=torch.int32, device="cuda")
+    ids_full = torch.from_numpy(np.sort(np.stack([rng.choice(Nb, size=min(k, Nb), replace=False) for _ in range(R)]), axis=1).astype(np.int32)).cuda()
+    if ids_full.shape[1] < k:
+        ids_full = torch.cat([ids_full, torch.full((R, k - ids_full.shape[1]), -1, dtype=torch.int32, device="cuda")], dim=1).contiguous()
+    Oa, Ob = torch.full_like(O_idx, float("nan")), torch.full_like(O_idx, float("nan"))
+    ctx.sparse_decode_varlen(L["Q"], L["kv"], ids_full, full, k, Oa, pool_is_indexed=True, n_slots=Nb)
+    ctx.sparse_decode(L["Q"], L["kv"], ids_full, k, Ob, pool_is_indexed=True, n_slots=Nb)
+    torch.cuda.synchronize()
+    assert torch.equal(Oa.view(torch.int16), Ob.view(torch.int16))
+    ctx.close()
+
+
 def test_sparse_equals_dense_when_all_blocks_selected(sp, oracle):
     """north_star: when top-k covers all blocks, sparse attention must equal dense attention."""
     cfg = synth.DecodeConfig("dense", batch=2, n_q_heads=32, n_kv_heads=2, head_dim=128, n_blocks=48, topk=48, seed=41)

@@ -309,6 +309,31 @@ def graph_time(torch, fn, n_sets, reps=10, best_of=3, flush=None):
     return best
 
 
+def isolated_time(torch, fn, n_sets, n=64):
+    """Seconds for ONE launch of fn(i, stream) as the decode step runs it: between two events of its own on the launching
+    stream, without programmatic dependent launch (the caller's context has no_pdl = 1), on the next of n_sets rotating buffer
+    sets (cold HBM), nothing of the same kind in flight before or behind it.  Median of n.  This is what one launch costs;
+    graph_time() beside it is the steady-state PERIOD of back-to-back launches, in which PDL hides each launch's gap, prologue
+    and first loads behind its predecessor's tail -- a pattern the step does not have."""
+    st = torch.cuda.current_stream()
+    for i in range(n_sets):
+        fn(i, st)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+    for i, (e0, e1) in enumerate(ev):
+        # a 150 us spin (no memory traffic) in front of the bracket: by the time the GPU reaches e0 the launch and e1 are already
+        # queued, so the bracket holds the GPU's time for the launch (kernel boundary included), not this Python loop's pace
+        torch.cuda._sleep(300_000)
+        e0.record(st)
+        fn(i % n_sets, st)
+        e1.record(st)
+        if i % 8 == 7:
+            torch.cuda.synchronize()
+    torch.cuda.synchronize()
+    ts = sorted(e0.elapsed_time(e1) for e0, e1 in ev)
+    return ts[len(ts) // 2] * 1e-3
+
+
 def kernel_entry(name, shape, t, nbytes, peak, ncu, key, ncu_src, **extra):
     m = ncu.get(key, {})
     traffic = (m.get("dram__bytes_read.sum", 0.0) + m.get("dram__bytes_write.sum", 0.0)) if "dram__bytes_read.sum" in m else None
@@ -360,7 +385,10 @@ def bench_kernels(torch, binding, peaks, ncu, ncu_src, batch):
     kpools = [torch.randn((R, Nb, D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16) for _ in range(NS_SEL)]
     t_sel = graph_time(torch, lambda i, s: ctx.forecast_select(Fs[i % 8], kpools[i], Nb, k, ids, stream=s), NS_SEL, reps=max(2, 160 // NS_SEL))
     cs_sel = ctx.select_cluster
-    del kpools
+    ctx_iso = binding.Sparda.from_config(cfg, no_pdl=1)      # plain launches: one launch in isolation (see isolated_time)
+    t_sel_iso = isolated_time(torch, lambda i, s: ctx_iso.forecast_select(Fs[i % 8], kpools[i], Nb, k, ids, stream=s), NS_SEL)
+    NS_PAIR = min(NS_SEL, max(2, -(-(256 << 20) // kp_bytes)))   # pooled-key sets kept for the pair: >= 256 MiB (2 x L2) of rotation
+    kpools = kpools[:NS_PAIR]
     pools = []
     for _ in range(NS_ATT):
         p = torch.empty((R, k, 2, 64, D), dtype=torch.bfloat16, device="cuda")
@@ -371,6 +399,17 @@ def bench_kernels(torch, binding, peaks, ncu, ncu_src, batch):
     ids_att = torch.arange(k, dtype=torch.int32, device="cuda").repeat(R, 1).contiguous()
     t_att = graph_time(torch, lambda i, s: ctx.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT, reps=max(2, 80 // NS_ATT))
     cl_att = ctx.attn_cluster
+    t_att_iso = isolated_time(torch, lambda i, s: ctx_iso.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT)
+
+    def pair(i, s):   # one layer's select + attention back to back on one stream, no PDL: the metric's "select+attn"
+        ctx_iso.forecast_select(Fs[i % 8], kpools[i % NS_PAIR], Nb, k, ids, stream=s)
+        ctx_iso.sparse_decode(Q, pools[i], ids_att, k, O, stream=s)
+    t_pair = isolated_time(torch, pair, NS_ATT)
+    # what the bracket itself costs: nothing between the two events, and one empty kernel (the launch floor inside the same bracket)
+    t_br0 = isolated_time(torch, lambda i, s: None, 1)
+    t_br1 = isolated_time(torch, lambda i, s: ctx_iso.probe_launch(0, stream=s), 1)
+    ctx_iso.close()
+    del kpools
     # the tcgen05 "swap-AB" experiment (cfg.attn_impl = 1) on the same pools: a measured comparison, not the product path
     ctx5 = binding.Sparda.from_config(cfg, attn_impl=1)
     t_att5 = graph_time(torch, lambda i, s: ctx5.sparse_decode(Q, pools[i], ids_att, k, O, stream=s), NS_ATT, reps=max(2, 80 // NS_ATT))
@@ -379,10 +418,17 @@ def bench_kernels(torch, binding, peaks, ncu, ncu_src, batch):
     sel_bytes = kp_bytes + R * D * 2 + R * k * 4
     att_bytes = pool_bytes + 2 * cfg.batch * cfg.n_q_heads * D * 2 + R * k * 4
     hbm = peaks["hbm_gbs"]
+    iso = lambda t, b: {"us_isolated": round(t * 1e6, 3), "frac_isolated": round(b / t / 1e9 / hbm, 4),
+                        "isolated": "one launch between two events behind a 150 us spin kernel, no PDL, cold buffers, median of 64; `us` / `frac` are the PDL back-to-back period"}
     out = [kernel_entry("forecast_select_kernel<128,false>", f"batch {batch}: R={R}, {Nb} blocks, top-{k}; cold HBM, graph replay", t_sel, sel_bytes,
-                        hbm, ncu, f"select_{tag}", ncu_src, cluster=cs_sel),
+                        hbm, ncu, f"select_{tag}", ncu_src, cluster=cs_sel, **iso(t_sel_iso, sel_bytes)),
            kernel_entry("sparse_decode_kernel<128>", f"batch {batch}: R={R}, top-{k} x 32 KiB; cold HBM, graph replay", t_att, att_bytes,
-                        hbm, ncu, f"attn_{tag}", ncu_src, cluster=cl_att, ctas_per_row=ctx.attn_splits(k)),
+                        hbm, ncu, f"attn_{tag}", ncu_src, cluster=cl_att, ctas_per_row=ctx.attn_splits(k), **iso(t_att_iso, att_bytes)),
+           {"kernel": "pair: forecast_select + sparse_decode", "shape": f"batch {batch}: one layer's select then attention on one stream, no PDL, cold HBM; "
+            "one pair between two events, median of 64", "bound": "hbm", "us_isolated": round(t_pair * 1e6, 3), "bytes": int(sel_bytes + att_bytes),
+            "achieved": round((sel_bytes + att_bytes) / t_pair / 1e9, 1), "peak": hbm, "unit": "GB/s",
+            "frac_isolated": round((sel_bytes + att_bytes) / t_pair / 1e9 / hbm, 4), "frac_of_8tbs": round((sel_bytes + att_bytes) / t_pair / 1e9 / 8000.0, 4),
+            "tag": f"pair_{tag}", "bracket_empty_us": round(t_br0 * 1e6, 3), "bracket_null_kernel_us": round(t_br1 * 1e6, 3)},
            kernel_entry("sparse_decode_tc5_kernel (experiment)", f"batch {batch}: same shape, tcgen05 swap-AB form (attn_impl=1); not the default", t_att5,
                         att_bytes, hbm, ncu, f"attn_tc5_{tag}", ncu_src, cluster=cl_att)]
     if batch == 32:
@@ -853,6 +899,43 @@ def bench_gather_sweep(torch, binding, peaks, ceiling, host_layer_b4):
 # ------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------
+def flat_scalars(roofline, gather_ctas, gather_mode):
+    """The per-kernel figures as SCALAR keys directly under `roofline` (a record that keeps only scalars still carries them).
+    *_isolated: one launch between two events without PDL on cold buffers; *_period: steady-state back-to-back period from
+    a graph replay with PDL (what `us` in roofline.kernels is).  frac = algorithmic bytes / time / measured HBM peak."""
+    out = {}
+    for e in roofline.get("kernels") or []:
+        shape = e.get("shape", "")
+        tag = "b32" if shape.startswith("batch 32") else "b4" if shape.startswith("batch 4") else None
+        if tag is None:
+            continue
+        if e["kernel"].startswith("forecast_select_kernel<128,false>"):
+            out.update({f"select_{tag}_us_isolated": e["us_isolated"], f"select_{tag}_us_period": e["us"],
+                        f"select_{tag}_frac_isolated": e["frac_isolated"], f"select_{tag}_frac_period": e["frac"]})
+        elif e["kernel"].startswith("sparse_decode_kernel<128>"):
+            out.update({f"attn_{tag}_us_isolated": e["us_isolated"], f"attn_{tag}_us_period": e["us"],
+                        f"attn_{tag}_frac_isolated": e["frac_isolated"], f"attn_{tag}_frac_period": e["frac"]})
+        elif e["kernel"].startswith("pair:"):
+            out.update({f"pair_{tag}_us": e["us_isolated"], f"pair_{tag}_frac": e["frac_isolated"], f"pair_{tag}_frac_of_8tbs": e["frac_of_8tbs"]})
+            if "bracket_null_kernel_us" in e:   # context for every *_isolated figure: the same bracket around nothing / around an empty kernel
+                out.update({"isolated_bracket_empty_us": e["bracket_empty_us"], "isolated_bracket_null_kernel_us": e["bracket_null_kernel_us"]})
+    pf = roofline.get("prefill_select")
+    if pf:
+        out.update({"prefill_chunked_us": pf["forecast_us_chunked"], "prefill_one_us": pf["forecast_us_one_launch"]})
+    ru = roofline.get("reuse_cache")
+    if ru:
+        out["floor_cached_step_ms"] = ru["compute_floor_ms_per_step"]
+    gs = roofline.get("gather_sweep")
+    if gs:
+        for blk in gs["sweep"]:
+            if blk["batch"] != 4:
+                continue
+            for row in blk["rows"]:
+                if row["engine"] == gather_mode and row["ctas"] == gather_ctas and "gbs_under_hbm_load" in row:
+                    out["gather_gbs_under_hbm_load"] = row["gbs_under_hbm_load"]
+    return out
+
+
 def run_sparda(args):
     import torch
     import torch.distributed as dist
@@ -984,6 +1067,33 @@ def run_sparda(args):
     ctx.profile_enable(False)
     t_gat = g_ms / g_n * 1e-3 if g_n else float("nan")
 
+    # ---- what the timed steps computed: after the timed regions, one more step in each form on NaN-poisoned pools.  The
+    # overlapped step must be bit-identical to the serial one (O and ids of every layer), the host-buffer step's O too; any
+    # block that arrived late, any stale slot, shows up as NaN or as a differing bit.  (Parity against the oracle at this
+    # size is tests/test_gpu_parity.py::test_full_size_32_layer_decode_step; bench.py must not import the oracle here.)
+    def snapshot(fn):
+        for p_ in pools:
+            p_.fill_(float("nan"))
+        for d in dev_layers:
+            d["O"].zero_()
+            d["ids"].fill_(-9)
+        torch.cuda.synchronize()
+        fn()
+        torch.cuda.synchronize()
+        return [d["O"].clone() for d in dev_layers], [d["ids"].clone() for d in dev_layers]
+    O_ser, I_ser = snapshot(lambda: step(binding.STEP_SERIAL))
+    O_ovl, I_ovl = snapshot(step)
+    checked = all(torch.equal(a, b) for a, b in zip(I_ser, I_ovl)) and \
+        all(torch.equal(a.view(torch.int16), b.view(torch.int16)) for a, b in zip(O_ser, O_ovl)) and \
+        not any(bool(torch.isnan(o).any()) for o in O_ovl) and all(int(i.min()) >= 0 for i in I_ovl)
+    for h in host_vals:
+        h["O"].zero_()
+    step_host()
+    torch.cuda.synchronize()
+    checked = checked and all(torch.equal(h["O"].view(torch.int16), o.cpu().view(torch.int16)) for h, o in zip(host_vals, O_ovl))
+    if not checked:
+        raise SystemExit("bench.py: the overlapped / host-buffer step is not bit-identical to the serial step; the timing above is void")
+
     ms_per_step = ms_total / args.steps
     tokens = cfg.batch * world
     value = shard.whole_job_value(cfg.batch, world, ms_per_step)
@@ -1041,6 +1151,7 @@ def run_sparda(args):
     roofline["reuse_cache_with_layer_standin"] = standin
     roofline["gather_sweep"] = gather_sweep
     roofline["numa"] = numa
+    roofline.update(flat_scalars(roofline, ctx.gather_ctas, args.gather_mode))
 
     base = None
     if not args.no_cpu_baseline and world == 1:
@@ -1073,6 +1184,7 @@ def run_sparda(args):
                 "h2d_staged_bytes_per_step": staged, "h2d_uva_gather_bytes_per_step": gather_bytes * (NL - 1),
                 "api": "sparda_decode_step_host: pinned host F/Q/O copied just in time inside the call; stream sync per step"},
         "gpu_launches": launches,
+        "checked": checked,      # overlapped == serial == host-buffer step, bit for bit, on poisoned pools after the timed regions
         "roofline": roofline,
         "cpu_baseline": base,
     }

@@ -811,6 +811,92 @@ def test_decode_step_cached_multi_step(cfg, sp, oracle):
     assert 0 < moved < (n_steps - 1) * (NL - 1) * R * k, "the drift should give partial reuse"
 
 
+def test_decode_step_cached_with_the_grid_selector_over_drifting_steps(sp, oracle):
+    """f3 inside f1: the (32,16) grid selector in the cached step while the Forecast drifts.  Here the reuse plan is its own launch
+    behind the select and the gather is ordered by an event instead of the doorbell -- which only matters once the slot tables
+    are populated, i.e. from the second step on.  Four steps: overlapped == serialized bit for bit (O, ids, pools, slot tables,
+    fetch lists); every step's ids against o15 on the GPU's compressed keys, slot tables / fetch lists against o11 chained over
+    the steps, pool bytes against o5 (poisoned before step 0), attention against o6 over the pool in slot order; partial reuse."""
+    cfg = G16.with_(n_layers=3, batch=3)
+    n_init, n_local, n_steps = 1, 8, 4
+    R, k, Nb, D, NL = cfg.rows, cfg.topk, cfg.n_blocks, cfg.head_dim, cfg.n_layers
+    data = _pipeline_inputs(cfg, sp)
+    g = torch.Generator(device="cuda").manual_seed(97)
+    Fs = [[(L["F"].float() + 0.5 * t * torch.randn(L["F"].shape, generator=g, device="cuda")).to(torch.bfloat16)
+           for (L, _) in data] for t in range(n_steps)]
+    F0s = [(data[0][0]["F0cur"].float() + 0.5 * t * torch.randn((R, D), generator=g, device="cuda")).to(torch.bfloat16)
+           for t in range(n_steps)]
+
+    def run(mode):
+        ctx = sp.Sparda.from_config(cfg, max_layers=4)
+        ctx.set_step_selector(True, n_init, n_local)
+        dev = []
+        for l, (L, kv_host) in enumerate(data):
+            kgrid = torch.empty((R, 4 * Nb, D), dtype=torch.bfloat16, device="cuda")
+            ctx.pool_keys_grid(L["kv"], R, Nb, kgrid)
+            dev.append({"F": L["F"].clone(), "Q": L["Q"], "Kpool": kgrid, "kv": L["kv"] if l == 0 else kv_host,
+                        "O": torch.zeros((cfg.batch, cfg.n_q_heads, D), dtype=torch.bfloat16, device="cuda"),
+                        "ids": torch.full((R, k), -9, dtype=torch.int32, device="cuda"),
+                        "pool": torch.full((R, k, 2, 64, D), float("nan"), dtype=torch.bfloat16, device="cuda") if l else None,
+                        "slot_ids": torch.full((R, k), -1, dtype=torch.int32, device="cuda") if l else None,
+                        "fetch": torch.full((R, k), -9, dtype=torch.int32, device="cuda") if l else None,
+                        "n_fetch": torch.zeros((R,), dtype=torch.int32, device="cuda") if l else None})
+        arr = ctx.make_cached_layers(dev)
+        F0 = F0s[0].clone()
+        cs, ps = torch.cuda.Stream(), torch.cuda.Stream(priority=-1)
+        hist = []
+        for t in range(n_steps):
+            for l in range(NL):
+                dev[l]["F"].copy_(Fs[t][l])
+            F0.copy_(F0s[t])
+            torch.cuda.synchronize()
+            ctx.decode_step_cached(arr, F0, Nb, k, cs, ps, mode)
+            torch.cuda.synchronize()
+            hist.append([{n: (d[n].clone() if d[n] is not None else None) for n in ("O", "ids", "pool", "slot_ids", "fetch", "n_fetch")}
+                         for d in dev])
+        grids = [_bits(d["Kpool"]) for d in dev]
+        ctx.close()
+        return hist, grids
+
+    h_ser, _ = run(sp.STEP_SERIAL)
+    h_ovl, grids = run(sp.STEP_OVERLAP)
+    for t in range(n_steps):
+        for l in range(NL):
+            for n in ("O", "ids", "pool", "slot_ids", "fetch"):
+                a, b = h_ser[t][l][n], h_ovl[t][l][n]
+                if a is not None:
+                    assert torch.equal(a.view(torch.int16) if a.dtype == torch.bfloat16 else a,
+                                       b.view(torch.int16) if b.dtype == torch.bfloat16 else b), f"step {t} layer {l} {n}"
+    kv_bits = [_bits(L["kv"]) for (L, _) in data]
+    forced = [b for b in range(Nb) if b < n_init or b >= Nb - n_local]
+    moved = 0
+    for t in range(n_steps):
+        for l in range(NL):
+            h = h_ovl[t][l]
+            f_bits = _bits(F0s[t]) if l == 0 else _bits(Fs[t][l - 1])
+            want_ids, bs = oracle.forecast_select_grid(f_bits, grids[l], k, Nb, n_init, n_local)
+            gids = h["ids"].cpu().numpy()
+            assert all(set(forced) <= set(gids[r].tolist()) for r in range(R))
+            parity.check_ids(gids, want_ids, np.where(np.isinf(bs), np.float32(3.0e38), bs), Nb)
+            q_bits = _bits(data[l][0]["Q"])
+            if l == 0:
+                want, _ = oracle.sparse_attn(q_bits, kv_bits[0], gids, pool_is_indexed=True)
+                parity.check_attn(_bits(h["O"]), want, f"grid cached step {t} layer 0")
+                continue
+            prev = h_ovl[t - 1][l]["slot_ids"].cpu().numpy() if t else np.full((R, k), -1, dtype=np.int32)
+            want_after, want_fetch = oracle.reuse_plan(gids, prev)
+            np.testing.assert_array_equal(h["slot_ids"].cpu().numpy(), want_after)
+            np.testing.assert_array_equal(h["fetch"].cpu().numpy(), want_fetch)
+            np.testing.assert_array_equal(h["n_fetch"].cpu().numpy(), (want_fetch >= 0).sum(1))
+            pool_ref = oracle.gather(kv_bits[l], want_after)
+            assert _bits(h["pool"]).tobytes() == pool_ref.tobytes(), f"grid cached step {t} layer {l}: pool bytes"
+            want, _ = oracle.sparse_attn(q_bits, pool_ref, want_after)
+            parity.check_attn(_bits(h["O"]), want, f"grid cached step {t} layer {l}")
+            if t:
+                moved += int((want_fetch >= 0).sum())
+    assert 0 < moved < (n_steps - 1) * (NL - 1) * R * k, "the drift should give partial reuse"
+
+
 @pytest.mark.parametrize("where", ["device", "host"])
 @pytest.mark.parametrize("cfg", [MID64.with_(n_blocks=6), G16.with_(n_blocks=5)], ids=lambda c: c.name)
 def test_append_kv_matches_oracle(cfg, where, sp, oracle):
